@@ -1,0 +1,186 @@
+/* crownb200.h -- C-ABI boundary of the B200-native bound-propagation hot path.
+ *
+ * What is computed (citations are /root/reference/PAPER.md line + section):
+ *   IBP interval forward                          PAPER.md:58-62  (sec. 2.1)
+ *   ReLU linear relaxation                        PAPER.md:64     (sec. 2.1)
+ *   CROWN / alpha-CROWN backward pass (Eq. 1)     PAPER.md:64-70  (sec. 2.1), :128 (sec. 3.3.2)
+ *   concretisation against the L_inf box          PAPER.md:27, :66 (reading G1 in DESIGN.md)
+ *   intermediate bounds choose the slopes         PAPER.md:130    (sec. 3.3.2)
+ *   verdict
+ *
+ * Conventions
+ *   - Every pointer named *_dev is a DEVICE pointer owned by the CALLER (the Python binding
+ *     allocates them as torch tensors).  Pointers named *_host are host pointers.
+ *   - The library never calls cudaMalloc: the caller passes ONE device workspace at init;
+ *     crown_workspace_bytes() says how large it must be.
+ *   - All tensors are dense float32, row-major, no padding.
+ *   - Work is issued asynchronously on the CUDA stream given to crown_init; results are valid
+ *     after the caller synchronises that stream.  (Host-buffer entry points *_host synchronise
+ *     before returning.)
+ *   - Every call returns 0 (CROWN_OK) or a negative crown_status; no C++ exception crosses.
+ *     crown_last_error() gives the text of the last failure on that context.
+ *   - There is no CPU fallback: without a CUDA device every compute call returns CROWN_ECUDA.
+ *
+ * Row layout of A-matrices and bias vectors ("branch-major"):
+ *   A_dev [2, B, R, n]   index ((br*B + b)*R + r)*n + j,  br = 0 lower branch, 1 upper branch
+ *   d_dev [2, B, R]
+ * Each (br, b, r) row is an independent linear bound  A x + d  (Eq. 1 is row-wise).
+ */
+#ifndef CROWNB200_H
+#define CROWNB200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  CROWN_OK = 0,
+  CROWN_EINVAL = -1,       /* bad shape / null pointer / non-topological node list / bad option   */
+  CROWN_ENOMEM = -2,       /* workspace smaller than crown_workspace_bytes(), or cap too small    */
+  CROWN_ECUDA = -3,        /* CUDA runtime / driver error (sticky); text via crown_last_error     */
+  CROWN_EUNSUPPORTED = -4  /* op or graph shape outside Linear/Conv2d/ReLU/Add/Flatten            */
+} crown_status;
+
+typedef enum {
+  CROWN_LINEAR = 1,  /* y = W x + b,  W [n_out, n_in] row-major                   */
+  CROWN_CONV2D = 2,  /* y = conv(x, W) + b, W [c_out, c_in, kh, kw], zero padding, NCHW         */
+  CROWN_RELU = 3,    /* y = max(x, 0)                                                            */
+  CROWN_ADD = 4,     /* y = in0 + in1 (residual add)                                            */
+  CROWN_FLATTEN = 5  /* row-major (C,H,W) -> (C*H*W)                                            */
+} crown_op;
+
+/* One node of a topologically ordered DAG.  Producers are node ids < own id; -1 = network input. */
+typedef struct {
+  int32_t op;                 /* crown_op                                                       */
+  int32_t in0, in1;           /* in1 only for CROWN_ADD, else -1                                */
+  int32_t n_out, n_in;        /* LINEAR: sizes.  Other ops: filled by the library (may be 0)    */
+  int32_t c_out, c_in, kh, kw, stride, pad, h_in, w_in; /* CONV2D                               */
+  const float* W_dev;         /* LINEAR [n_out,n_in]; CONV2D [c_out,c_in,kh,kw]; device memory  */
+  const float* b_dev;         /* [n_out] / [c_out]; device memory                               */
+  const float* W_host;        /* optional pinned-host copy, used when opts.stream_weights != 0  */
+} crown_node;
+
+typedef struct {
+  uint64_t mem_cap_bytes;   /* cap on workspace use; 0 = no cap.  Start-spec rows are chunked so
+                               that prepacked weights + live A buffers stay below it
+                               (single-GPU restatement of Eq. 2)               */
+  int32_t stream_weights;   /* 1: GEMM weight operands of layers wider than stream_min_elems are
+                               not resident; they are prepacked into pinned host memory at init
+                               and copied H2D on a side stream per use, double-buffered ("gather
+                               before / free after")                               */
+  int32_t mma_scheme;       /* 0 = 3xTF32 on tcgen05 tensor cores (fp32-accurate, never plain
+                               TF32); 2 = fp32 FFMA on CUDA cores (debug / odd shapes)           */
+  int32_t slope_rule;       /* fixed lower slope for unstable neurons when no alpha is given:
+                               0 adaptive (1 iff u > -l, reading G4), 1 all-zero, 2 all-one       */
+  int32_t k_drain;          /* 3xTF32: accumulate at most this many K in TMEM before the fp32
+                               CUDA-core running sum takes over (0 = library default)            */
+  uint64_t stream_min_elems;/* see stream_weights (0 = library default 2^28 elements)            */
+} crown_opts;
+
+typedef struct crown_ctx crown_ctx;   /* opaque; owned by the library; freed by crown_destroy */
+
+/* Bytes of device workspace crown_init needs for batches up to B_max properties and final
+ * specs up to S_max rows, under opts (mem_cap_bytes bounds the answer or CROWN_ENOMEM).
+ * in_c/in_h/in_w: input shape; for flat inputs pass (n0, 1, 1). */
+int crown_workspace_bytes(const crown_node* nodes, int n_nodes, int in_c, int in_h, int in_w,
+                          int B_max, int S_max, const crown_opts* opts, size_t* out_bytes);
+
+/* Builds the plan, prepacks GEMM weight operands (transpose + TF32 hi/lo split, a device kernel)
+ * into the workspace (or pinned host memory when streaming), creates TMA descriptors.
+ * cuda_stream: a cudaStream_t (0 = default stream). */
+int crown_init(crown_ctx** out, const crown_node* nodes, int n_nodes, int in_c, int in_h, int in_w,
+               int B_max, int S_max, void* workspace_dev, size_t workspace_bytes,
+               const crown_opts* opts, void* cuda_stream);
+
+/* O1 -- IBP for B properties with boxes [x_lo, x_hi] ([B, n0] each).
+ * l_dev[i], u_dev[i] (arrays of n_nodes device pointers, entries may be NULL = not wanted):
+ * interval of node i's OUTPUT, [B, size_i].  If C_dev != NULL ([B,S,n_L]) also writes the IBP
+ * bound of C.f(x) with C and the last Linear fused into one layer (reading G10) to
+ * lb_dev/ub_dev [B,S]. */
+int ibp_forward(crown_ctx* ctx, int B, const float* x_lo_dev, const float* x_hi_dev,
+                float* const* l_dev, float* const* u_dev,
+                const float* C_dev, int S, float* lb_dev, float* ub_dev);
+
+/* O3 -- one CROWN backward pass (PAPER.md:64-68 Eq. 1, :128 A <- A.Lambda_i W_i) from node
+ * `start` down to the input, for `rows` start-spec rows per property.
+ *   C_dev == NULL : start matrix = rows [row0, row0+rows) of the identity on node `start`'s
+ *                   output (intermediate bounds); `start` must be Linear or Conv2d.
+ *   C_dev != NULL : [B, rows, size_start] start matrix (row0 ignored).
+ *   l_dev/u_dev   : arrays of n_nodes pointers; for every ReLU node i below `start`, the
+ *                   pre-activation bounds of its INPUT, [B, size_i].
+ *   alpha_lo_dev / alpha_up_dev : arrays of n_nodes pointers or NULL; entry i, if non-NULL, is
+ *                   the lower-relaxation slope [B, rows, size_i] of ReLU i used by the lower /
+ *                   upper branch, clipped to [0,1]; NULL = opts.slope_rule.
+ *                   The two may alias.
+ *   A_dev [2,B,rows,n0], d_dev [2,B,rows] : outputs (branch-major, see top).  Either may be NULL
+ *                   when lb_dev/ub_dev are given.
+ *   x_lo_dev/x_hi_dev/lb_dev/ub_dev : if lb_dev != NULL the pass ends with the concretisation
+ *                   (same arithmetic as concretize()) into lb_dev/ub_dev [B, rows]. */
+int crown_backward(crown_ctx* ctx, int B, int start, int row0, int rows, const float* C_dev,
+                   const float* const* l_dev, const float* const* u_dev,
+                   const float* const* alpha_lo_dev, const float* const* alpha_up_dev,
+                   float* A_dev, float* d_dev,
+                   const float* x_lo_dev, const float* x_hi_dev, float* lb_dev, float* ub_dev);
+
+/* Numbers from Eq. 1 over the box (Hoelder dual of the L_inf ball):
+ *   lb = A_lo.x_c - |A_lo|.x_r + d_lo,  ub = A_up.x_c + |A_up|.x_r + d_up,
+ *   x_c = (x_lo+x_hi)/2, x_r = (x_hi-x_lo)/2.   A_dev [2,B,rows,n0], d_dev [2,B,rows].
+ * lb_dev/ub_dev: element (b, r) is written at lb_dev[b*out_stride + r]. */
+int concretize(crown_ctx* ctx, int B, int rows, const float* A_dev, const float* d_dev,
+               const float* x_lo_dev, const float* x_hi_dev,
+               float* lb_dev, float* ub_dev, int out_stride);
+
+/* The whole hot path for a batch (O4 then O5 then the verdict):
+ *   intermediate = 0: CROWN intermediate bounds for every ReLU in topological order (first
+ *                     layer by IBP, which coincides), row-chunked under mem_cap;
+ *   intermediate = 1: IBP for every pre-activation (cfg5, reading G22);
+ *   then the final pass from the last node with C_dev [B,S,n_L] and alpha (array of n_nodes
+ *   pointers, entry i = [B,S,size_i] for ReLU i, or NULL array/entries = slope rule).
+ * Outputs: l_dev/u_dev (arrays of n_nodes pointers; entries for ReLU nodes must be non-NULL
+ * [B,size_i] and receive that ReLU's pre-activation bounds), lb_dev/ub_dev [B,S],
+ * verified_dev [B] uint8 (1 iff min_s lb > 0). */
+int crown_run(crown_ctx* ctx, int B, const float* x_lo_dev, const float* x_hi_dev,
+              const float* C_dev, int S, const float* const* alpha_dev, int intermediate,
+              float* const* l_dev, float* const* u_dev,
+              float* lb_dev, float* ub_dev, uint8_t* verified_dev);
+
+/* Same as crown_run with HOST buffers: copies x_lo/x_hi/C/alpha H2D, runs, copies lb/ub/verified
+ * D2H, synchronises.  Staging comes from the workspace.  alpha_host entries as in crown_run. */
+int crown_run_host(crown_ctx* ctx, int B, const float* x_lo_host, const float* x_hi_host,
+                   const float* C_host, int S, const float* const* alpha_host, int intermediate,
+                   float* lb_host, float* ub_host, uint8_t* verified_host);
+
+/* D[M,N] = A[M,K] . W[K,N] (row-major fp32) through the same contraction kernel the backward
+ * pass uses (scheme: 0 = 3xTF32 tcgen05, 2 = FFMA); exposed for parity tests and roofline
+ * measurement of kernel 1.  Wt_hi/Wt_lo [N,K] and A_hi/A_lo [M,K] are produced by
+ * crown_split_tf32 (transpose=1 for W). */
+int crown_gemm(crown_ctx* ctx, int scheme, int M, int N, int K,
+               const float* A_hi_dev, const float* A_lo_dev,
+               const float* Wt_hi_dev, const float* Wt_lo_dev, float* D_dev);
+int crown_split_tf32(crown_ctx* ctx, const float* X_dev, int rows, int cols, int transpose,
+                     float* hi_dev, float* lo_dev);
+
+/* Introspection. */
+int crown_peak_bytes(crown_ctx* ctx, size_t* out);         /* high-water mark of workspace use   */
+int crown_launch_count(crown_ctx* ctx, uint64_t* out);      /* kernels launched so far            */
+int crown_gemm_flops(crown_ctx* ctx, double* out);          /* useful 2MNK flops of A.W so far    */
+int crown_timing(crown_ctx* ctx, int enable);               /* 1: record CUDA events per kernel class */
+int crown_timing_read(crown_ctx* ctx, int kernel_class, double* ms_total, uint64_t* launches,
+                      double* bytes_total, double* flops_total);
+const char* crown_last_error(crown_ctx* ctx);
+int crown_destroy(crown_ctx* ctx);
+const char* crown_version(void);
+
+/* kernel classes for crown_timing_read */
+enum {
+  CROWN_K_IBP = 0, CROWN_K_COEFF = 1, CROWN_K_RELAX = 2, CROWN_K_GEMM_TC = 3, CROWN_K_GEMM_FFMA = 4,
+  CROWN_K_CONCRETIZE = 5, CROWN_K_CONV = 6, CROWN_K_MISC = 7, CROWN_K_NUM = 8
+};
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CROWNB200_H */

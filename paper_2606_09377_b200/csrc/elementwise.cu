@@ -1,0 +1,396 @@
+// HBM-bound kernels of the CROWN hot path (SURVEY.md sec. 8(a) rows a3, a4, a8, a9 and helpers).
+// Every kernel here streams its operands once with 128-bit coalesced accesses; row reductions use
+// warp shuffles (one warp owns a row pair, so bias accumulation needs no atomics).
+#include "common.cuh"
+#include "kernels.h"
+
+namespace crownb200 {
+
+// ------------------------------------------------------------------------------------------------
+// a3 -- relaxation coefficients.  Classification order active -> inactive -> unstable
+// (reading G3); adaptive rule lambda = 1 iff u > -l (reading G4).
+// ------------------------------------------------------------------------------------------------
+__global__ void relax_coeffs_kernel(const float* __restrict__ l, const float* __restrict__ u,
+                                    float4* __restrict__ coef, long long count, int rule) {
+  long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= count) return;
+  float lo = l[i], hi = u[i];
+  float4 c;
+  if (lo >= 0.f) {
+    c = make_float4(1.f, 0.f, 1.f, 0.f);
+  } else if (hi <= 0.f) {
+    c = make_float4(0.f, 0.f, 0.f, 0.f);
+  } else {
+    float den = hi - lo;
+    float dU = hi / den;
+    float bU = (-lo * hi) / den;
+    float dL = rule == 0 ? (hi > -lo ? 1.f : 0.f) : (rule == 2 ? 1.f : 0.f);
+    c = make_float4(dU, bU, dL, 1.f);
+  }
+  coef[i] = c;
+}
+
+void launch_relax_coeffs(const float* l, const float* u, float4* coef, long long count, int rule,
+                         cudaStream_t s) {
+  if (count <= 0) return;
+  int threads = 256;
+  relax_coeffs_kernel<<<ceil_div(count, threads), threads, 0, s>>>(l, u, coef, count, rule);
+}
+
+// ------------------------------------------------------------------------------------------------
+// a4 -- fused relaxation.  One warp owns one (property b, row r) pair and walks the neuron axis for
+// BOTH branches, so the coefficient vectors and alpha are read once per pair.
+//   lower: Abar = A+ * dL + A- * dU,  d += A- . bU        (Eq. 1)
+//   upper: Abar = A+ * dU + A- * dL,  d += A+ . bU
+//   both : d += Abar . bias           (bias of the linear layer the contraction goes through next)
+// ------------------------------------------------------------------------------------------------
+struct RelaxDev {
+  const float* A; long long sBr, sB, ld;
+  const float4* coef;
+  const float* alpha_lo; const float* alpha_up;
+  const float* bias; int bias_div;
+  float* out; float* out_lo; float* d;
+  int B, R, n;
+};
+
+__device__ __forceinline__ float clip01(float a) { return fminf(fmaxf(a, 0.f), 1.f); }
+
+// one element, both branches.  Returns contributions to d.
+template <bool RELU, bool ALPHA>
+__device__ __forceinline__ void relax_elem(float aL, float aU, const float4& c, float alL, float alU,
+                                           float bias, float& oL, float& oU, float& dLacc, float& dUacc) {
+  if (RELU) {
+    float dU = c.x, bU = c.y;
+    float sL = c.z, sU = c.z;
+    if (ALPHA) {
+      if (c.w != 0.f) { sL = clip01(alL); sU = clip01(alU); }
+    }
+    float pL = fmaxf(aL, 0.f), mL = fminf(aL, 0.f);
+    float pU = fmaxf(aU, 0.f), mU = fminf(aU, 0.f);
+    oL = pL * sL + mL * dU;
+    oU = pU * dU + mU * sU;
+    dLacc = fmaf(mL, bU, dLacc);
+    dUacc = fmaf(pU, bU, dUacc);
+  } else {
+    oL = aL; oU = aU;
+  }
+  dLacc = fmaf(oL, bias, dLacc);
+  dUacc = fmaf(oU, bias, dUacc);
+}
+
+template <bool RELU, bool ALPHA, bool SPLIT, int VEC>
+__global__ void __launch_bounds__(256) relax_kernel(RelaxDev p) {
+  const int lane = threadIdx.x & 31;
+  const long long pair = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (pair >= (long long)p.B * p.R) return;
+  const int b = (int)(pair / p.R), r = (int)(pair % p.R);
+  const float* a0 = p.A + (long long)b * p.sB + (long long)r * p.ld;
+  const float* a1 = a0 + p.sBr;
+  const float4* cf = RELU ? p.coef + (long long)b * p.n : nullptr;
+  const long long arow = ((long long)b * p.R + r) * p.n;
+  const float* alL = ALPHA ? p.alpha_lo + arow : nullptr;
+  const float* alU = ALPHA ? p.alpha_up + arow : nullptr;
+  const long long BR = (long long)p.B * p.R;
+  float* o0 = p.out + (pair) * (long long)p.n;
+  float* o1 = p.out + (BR + pair) * (long long)p.n;
+  float* q0 = SPLIT ? p.out_lo + (pair) * (long long)p.n : nullptr;
+  float* q1 = SPLIT ? p.out_lo + (BR + pair) * (long long)p.n : nullptr;
+  float accL = 0.f, accU = 0.f;
+
+  if (VEC == 4) {
+    for (int j = lane * 4; j < p.n; j += 128) {
+      float4 xL = ldg_stream4(a0 + j);
+      float4 xU = ldg_stream4(a1 + j);
+      float4 c0 = make_float4(0, 0, 0, 0), c1 = c0, c2 = c0, c3 = c0;
+      if (RELU) { c0 = __ldg(cf + j); c1 = __ldg(cf + j + 1); c2 = __ldg(cf + j + 2); c3 = __ldg(cf + j + 3); }
+      float4 tL = make_float4(0, 0, 0, 0), tU = tL;
+      if (ALPHA) {
+        tL = ldg_stream4(alL + j);
+        tU = (alU == alL) ? tL : ldg_stream4(alU + j);
+      }
+      float4 bs = make_float4(0, 0, 0, 0);
+      if (p.bias) {
+        if (p.bias_div == 1) bs = __ldg(reinterpret_cast<const float4*>(p.bias + j));
+        else { bs.x = __ldg(p.bias + (j) / p.bias_div); bs.y = __ldg(p.bias + (j + 1) / p.bias_div);
+               bs.z = __ldg(p.bias + (j + 2) / p.bias_div); bs.w = __ldg(p.bias + (j + 3) / p.bias_div); }
+      }
+      float4 yL, yU;
+      relax_elem<RELU, ALPHA>(xL.x, xU.x, c0, tL.x, tU.x, bs.x, yL.x, yU.x, accL, accU);
+      relax_elem<RELU, ALPHA>(xL.y, xU.y, c1, tL.y, tU.y, bs.y, yL.y, yU.y, accL, accU);
+      relax_elem<RELU, ALPHA>(xL.z, xU.z, c2, tL.z, tU.z, bs.z, yL.z, yU.z, accL, accU);
+      relax_elem<RELU, ALPHA>(xL.w, xU.w, c3, tL.w, tU.w, bs.w, yL.w, yU.w, accL, accU);
+      if (SPLIT) {
+        float4 hL, lL, hU, lU;
+        tf32_split(yL.x, hL.x, lL.x); tf32_split(yL.y, hL.y, lL.y);
+        tf32_split(yL.z, hL.z, lL.z); tf32_split(yL.w, hL.w, lL.w);
+        tf32_split(yU.x, hU.x, lU.x); tf32_split(yU.y, hU.y, lU.y);
+        tf32_split(yU.z, hU.z, lU.z); tf32_split(yU.w, hU.w, lU.w);
+        stg_stream4(o0 + j, hL); stg_stream4(q0 + j, lL);
+        stg_stream4(o1 + j, hU); stg_stream4(q1 + j, lU);
+      } else {
+        stg_stream4(o0 + j, yL);
+        stg_stream4(o1 + j, yU);
+      }
+    }
+  } else {
+    for (int j = lane; j < p.n; j += 32) {
+      float xL = a0[j], xU = a1[j];
+      float4 c = RELU ? cf[j] : make_float4(0, 0, 0, 0);
+      float tL = ALPHA ? alL[j] : 0.f, tU = ALPHA ? alU[j] : 0.f;
+      float bs = p.bias ? p.bias[j / p.bias_div] : 0.f;
+      float yL, yU;
+      relax_elem<RELU, ALPHA>(xL, xU, c, tL, tU, bs, yL, yU, accL, accU);
+      if (SPLIT) {
+        float h, l2;
+        tf32_split(yL, h, l2); o0[j] = h; q0[j] = l2;
+        tf32_split(yU, h, l2); o1[j] = h; q1[j] = l2;
+      } else { o0[j] = yL; o1[j] = yU; }
+    }
+  }
+  accL = warp_sum(accL);
+  accU = warp_sum(accU);
+  if (lane == 0 && p.d) {
+    p.d[pair] += accL;
+    p.d[BR + pair] += accU;
+  }
+}
+
+template <bool RELU, bool ALPHA, bool SPLIT>
+static void relax_dispatch_vec(const RelaxDev& p, bool vec, int blocks, cudaStream_t s) {
+  if (vec) relax_kernel<RELU, ALPHA, SPLIT, 4><<<blocks, 256, 0, s>>>(p);
+  else relax_kernel<RELU, ALPHA, SPLIT, 1><<<blocks, 256, 0, s>>>(p);
+}
+
+void launch_relax(const RelaxArgs& a, cudaStream_t s) {
+  RelaxDev p;
+  p.A = a.A.p; p.sBr = a.A.sBr; p.sB = a.A.sB; p.ld = a.A.ld;
+  p.coef = a.coef; p.alpha_lo = a.alpha_lo; p.alpha_up = a.alpha_up ? a.alpha_up : a.alpha_lo;
+  if (!p.alpha_lo) p.alpha_lo = p.alpha_up;
+  p.bias = a.bias; p.bias_div = a.bias_div > 0 ? a.bias_div : 1;
+  p.out = a.out; p.out_lo = a.out_lo; p.d = a.d; p.B = a.B; p.R = a.R; p.n = a.n;
+  long long pairs = (long long)a.B * a.R;
+  if (pairs <= 0 || a.n <= 0) return;
+  int blocks = ceil_div(pairs * 32, 256);
+  auto al16 = [](const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; };
+  bool vec = (a.n % 4 == 0) && (p.ld % 4 == 0) && (p.sB % 4 == 0) && (p.sBr % 4 == 0) && al16(p.A) &&
+             al16(p.out) && (!p.out_lo || al16(p.out_lo)) && (!p.alpha_lo || al16(p.alpha_lo)) &&
+             (!p.alpha_up || al16(p.alpha_up)) && (!p.bias || p.bias_div != 1 || al16(p.bias));
+  bool relu = a.coef != nullptr, alpha = relu && p.alpha_lo != nullptr, split = a.out_lo != nullptr;
+#define CROWN_RELAX_CASE(R_, A_, S_) relax_dispatch_vec<R_, A_, S_>(p, vec, blocks, s)
+  if (relu) {
+    if (alpha) { if (split) CROWN_RELAX_CASE(true, true, true); else CROWN_RELAX_CASE(true, true, false); }
+    else       { if (split) CROWN_RELAX_CASE(true, false, true); else CROWN_RELAX_CASE(true, false, false); }
+  } else {
+    if (split) CROWN_RELAX_CASE(false, false, true); else CROWN_RELAX_CASE(false, false, false);
+  }
+#undef CROWN_RELAX_CASE
+}
+
+// ------------------------------------------------------------------------------------------------
+// a8 -- concretisation.  One warp per (b, r) pair, both branches (x_c, x_r shared).
+// ------------------------------------------------------------------------------------------------
+template <int VEC>
+__global__ void __launch_bounds__(256) concretize_kernel(const float* __restrict__ A, long long sBr,
+                                                         long long sB, long long ld, int n,
+                                                         const float* __restrict__ d,
+                                                         const float* __restrict__ x_lo,
+                                                         const float* __restrict__ x_hi,
+                                                         float* __restrict__ lb, float* __restrict__ ub,
+                                                         int out_stride, int B, int R) {
+  const int lane = threadIdx.x & 31;
+  const long long pair = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (pair >= (long long)B * R) return;
+  const int b = (int)(pair / R), r = (int)(pair % R);
+  const float* a0 = A + (long long)b * sB + (long long)r * ld;
+  const float* a1 = a0 + sBr;
+  const float* xl = x_lo + (long long)b * n;
+  const float* xh = x_hi + (long long)b * n;
+  float dotL = 0.f, absL = 0.f, dotU = 0.f, absU = 0.f;
+  if (VEC == 4) {
+    for (int j = lane * 4; j < n; j += 128) {
+      float4 vL = ldg_stream4(a0 + j), vU = ldg_stream4(a1 + j);
+      float4 lo = __ldg(reinterpret_cast<const float4*>(xl + j));
+      float4 hi = __ldg(reinterpret_cast<const float4*>(xh + j));
+      float cx = 0.5f * (lo.x + hi.x), rx = 0.5f * (hi.x - lo.x);
+      float cy = 0.5f * (lo.y + hi.y), ry = 0.5f * (hi.y - lo.y);
+      float cz = 0.5f * (lo.z + hi.z), rz = 0.5f * (hi.z - lo.z);
+      float cw = 0.5f * (lo.w + hi.w), rw = 0.5f * (hi.w - lo.w);
+      dotL = fmaf(vL.x, cx, dotL); absL = fmaf(fabsf(vL.x), rx, absL);
+      dotL = fmaf(vL.y, cy, dotL); absL = fmaf(fabsf(vL.y), ry, absL);
+      dotL = fmaf(vL.z, cz, dotL); absL = fmaf(fabsf(vL.z), rz, absL);
+      dotL = fmaf(vL.w, cw, dotL); absL = fmaf(fabsf(vL.w), rw, absL);
+      dotU = fmaf(vU.x, cx, dotU); absU = fmaf(fabsf(vU.x), rx, absU);
+      dotU = fmaf(vU.y, cy, dotU); absU = fmaf(fabsf(vU.y), ry, absU);
+      dotU = fmaf(vU.z, cz, dotU); absU = fmaf(fabsf(vU.z), rz, absU);
+      dotU = fmaf(vU.w, cw, dotU); absU = fmaf(fabsf(vU.w), rw, absU);
+    }
+  } else {
+    for (int j = lane; j < n; j += 32) {
+      float vL = a0[j], vU = a1[j];
+      float c = 0.5f * (xl[j] + xh[j]), rr = 0.5f * (xh[j] - xl[j]);
+      dotL = fmaf(vL, c, dotL); absL = fmaf(fabsf(vL), rr, absL);
+      dotU = fmaf(vU, c, dotU); absU = fmaf(fabsf(vU), rr, absU);
+    }
+  }
+  dotL = warp_sum(dotL); absL = warp_sum(absL);
+  dotU = warp_sum(dotU); absU = warp_sum(absU);
+  if (lane == 0) {
+    const long long BR = (long long)B * R;
+    float dl = d ? d[pair] : 0.f, du = d ? d[BR + pair] : 0.f;
+    lb[(long long)b * out_stride + r] = (dotL - absL) + dl;
+    ub[(long long)b * out_stride + r] = (dotU + absU) + du;
+  }
+}
+
+void launch_concretize(const AView& A, const float* d, const float* x_lo, const float* x_hi,
+                       float* lb, float* ub, int out_stride, int B, int R, cudaStream_t s) {
+  long long pairs = (long long)B * R;
+  if (pairs <= 0) return;
+  int blocks = ceil_div(pairs * 32, 256);
+  auto al16 = [](const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; };
+  bool vec = (A.n % 4 == 0) && (A.ld % 4 == 0) && (A.sB % 4 == 0) && (A.sBr % 4 == 0) && al16(A.p) &&
+             al16(x_lo) && al16(x_hi);
+  if (vec) concretize_kernel<4><<<blocks, 256, 0, s>>>(A.p, A.sBr, A.sB, A.ld, A.n, d, x_lo, x_hi, lb, ub, out_stride, B, R);
+  else concretize_kernel<1><<<blocks, 256, 0, s>>>(A.p, A.sBr, A.sB, A.ld, A.n, d, x_lo, x_hi, lb, ub, out_stride, B, R);
+}
+
+// ------------------------------------------------------------------------------------------------
+// helpers
+// ------------------------------------------------------------------------------------------------
+__global__ void init_d_kernel(float* d, const float* bias, int row0, int B, int R) {
+  long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  long long tot = 2LL * B * R;
+  if (i >= tot) return;
+  int r = (int)(i % R);
+  d[i] = bias ? bias[row0 + r] : 0.f;
+}
+void launch_init_d(float* d, const float* bias, int row0, int B, int R, cudaStream_t s) {
+  long long tot = 2LL * B * R;
+  if (tot <= 0) return;
+  init_d_kernel<<<ceil_div(tot, 256), 256, 0, s>>>(d, bias, row0, B, R);
+}
+
+__global__ void __launch_bounds__(256) rowdot_bias_kernel(const float* __restrict__ A, long long sBr,
+                                                          long long sB, long long ld, int n,
+                                                          const float* __restrict__ bias, int bias_div,
+                                                          float* d, int B, int R) {
+  const int lane = threadIdx.x & 31;
+  const long long m = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const long long BR = (long long)B * R;
+  if (m >= 2 * BR) return;
+  int br = (int)(m / BR);
+  long long pair = m % BR;
+  int b = (int)(pair / R), r = (int)(pair % R);
+  const float* a = A + br * sBr + (long long)b * sB + (long long)r * ld;
+  float acc = 0.f;
+  for (int j = lane; j < n; j += 32) acc = fmaf(a[j], bias[j / bias_div], acc);
+  acc = warp_sum(acc);
+  if (lane == 0) d[m] += acc;
+}
+void launch_rowdot_bias(const AView& A, const float* bias, int bias_div, float* d, int B, int R,
+                        cudaStream_t s) {
+  long long rows = 2LL * B * R;
+  if (rows <= 0 || !bias) return;
+  rowdot_bias_kernel<<<ceil_div(rows * 32, 256), 256, 0, s>>>(A.p, A.sBr, A.sB, A.ld, A.n, bias,
+                                                             bias_div > 0 ? bias_div : 1, d, B, R);
+}
+
+__global__ void view_add_kernel(const float* __restrict__ a, long long aBr, long long aB, long long ald,
+                                const float* __restrict__ b2, long long bBr, long long bB, long long bld,
+                                float* __restrict__ out, int B, int R, int n) {
+  long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  long long tot = 2LL * B * R * n;
+  if (i >= tot) return;
+  int j = (int)(i % n);
+  long long m = i / n;
+  int r = (int)(m % R);
+  long long t = m / R;
+  int b = (int)(t % B), br = (int)(t / B);
+  float v = a[br * aBr + b * aB + r * ald + j];
+  if (b2) v += b2[br * bBr + b * bB + r * bld + j];
+  out[i] = v;
+}
+void launch_view_add(const AView& a, const AView* b, float* out, int B, int R, cudaStream_t s) {
+  long long tot = 2LL * B * R * a.n;
+  if (tot <= 0) return;
+  view_add_kernel<<<ceil_div(tot, 256), 256, 0, s>>>(a.p, a.sBr, a.sB, a.ld, b ? b->p : nullptr,
+                                                    b ? b->sBr : 0, b ? b->sB : 0, b ? b->ld : 0, out,
+                                                    B, R, a.n);
+}
+
+__global__ void verdict_kernel(const float* __restrict__ lb, uint8_t* __restrict__ v, int B, int S) {
+  int b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= B) return;
+  float m = INFINITY;
+  for (int s = 0; s < S; ++s) m = fminf(m, lb[(long long)b * S + s]);
+  v[b] = (m > 0.f) ? 1 : 0;
+}
+void launch_verdict(const float* lb, uint8_t* verified, int B, int S, cudaStream_t s) {
+  if (B <= 0) return;
+  verdict_kernel<<<ceil_div(B, 128), 128, 0, s>>>(lb, verified, B, S);
+}
+
+__global__ void ibp_relu_kernel(const float* l, const float* u, float* lo, float* uo, long long count) {
+  long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= count) return;
+  lo[i] = fmaxf(l[i], 0.f);
+  uo[i] = fmaxf(u[i], 0.f);
+}
+void launch_ibp_relu(const float* l, const float* u, float* lo, float* uo, long long count, cudaStream_t s) {
+  if (count <= 0) return;
+  ibp_relu_kernel<<<ceil_div(count, 256), 256, 0, s>>>(l, u, lo, uo, count);
+}
+__global__ void ibp_add_kernel(const float* l0, const float* u0, const float* l1, const float* u1,
+                               float* lo, float* uo, long long count) {
+  long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= count) return;
+  lo[i] = l0[i] + l1[i];
+  uo[i] = u0[i] + u1[i];
+}
+void launch_ibp_add(const float* l0, const float* u0, const float* l1, const float* u1, float* lo,
+                    float* uo, long long count, cudaStream_t s) {
+  if (count <= 0) return;
+  ibp_add_kernel<<<ceil_div(count, 256), 256, 0, s>>>(l0, u0, l1, u1, lo, uo, count);
+}
+
+// X [rows, cols] -> hi/lo TF32 parts; transpose=1 writes [cols, rows] through a 32x33 smem tile.
+__global__ void split_tf32_kernel(const float* __restrict__ X, int rows, int cols, int transpose,
+                                  float* __restrict__ hi, float* __restrict__ lo) {
+  __shared__ float tile[32][33];
+  int bx = blockIdx.x * 32, by = blockIdx.y * 32;
+  int tx = threadIdx.x, ty = threadIdx.y;  // 32 x 8
+  if (!transpose) {
+    for (int k = ty; k < 32; k += 8) {
+      int r = by + k, c = bx + tx;
+      if (r < rows && c < cols) {
+        float h, l2;
+        tf32_split(X[(long long)r * cols + c], h, l2);
+        hi[(long long)r * cols + c] = h;
+        lo[(long long)r * cols + c] = l2;
+      }
+    }
+    return;
+  }
+  for (int k = ty; k < 32; k += 8) {
+    int r = by + k, c = bx + tx;
+    tile[k][tx] = (r < rows && c < cols) ? X[(long long)r * cols + c] : 0.f;
+  }
+  __syncthreads();
+  for (int k = ty; k < 32; k += 8) {
+    int c = bx + k, r = by + tx;  // output [c, r]
+    if (r < rows && c < cols) {
+      float h, l2;
+      tf32_split(tile[tx][k], h, l2);
+      hi[(long long)c * rows + r] = h;
+      lo[(long long)c * rows + r] = l2;
+    }
+  }
+}
+void launch_split_tf32(const float* X, int rows, int cols, int transpose, float* hi, float* lo,
+                       cudaStream_t s) {
+  if (rows <= 0 || cols <= 0) return;
+  dim3 grid(ceil_div(cols, 32), ceil_div(rows, 32)), block(32, 8);
+  split_tf32_kernel<<<grid, block, 0, s>>>(X, rows, cols, transpose, hi, lo);
+}
+
+}  // namespace crownb200

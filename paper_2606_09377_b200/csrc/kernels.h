@@ -1,0 +1,91 @@
+// Host-side launchers of the crownb200 kernels.  One declaration per kernel; each says which step
+// of SURVEY.md sec. 8(a) / which passage of PAPER.md it implements.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace crownb200 {
+
+// A strided view of an A-matrix [2, B, R, n] (branch-major).  sBr / sB may be 0 when both branches /
+// all properties still share the same rows (start of a pass: A = W_k rows or C.W_L).
+struct AView {
+  const float* p = nullptr;   // fp32 values (or TF32 "hi" part when lo != nullptr)
+  const float* lo = nullptr;  // TF32 "lo" part, same addressing, or nullptr
+  long long sBr = 0, sB = 0;  // element strides of the branch and property axes
+  long long ld = 0;           // row stride (elements)
+  int n = 0;                  // row length
+};
+
+// a3 -- relaxation coefficients of a ReLU from its pre-activation bounds.
+// coef[b*n+j] = {dU, bU, dL_fixed, unstable?1:0}.  rule: 0 adaptive, 1 zero, 2 one.
+void launch_relax_coeffs(const float* l, const float* u, float4* coef, long long count, int rule,
+                         cudaStream_t s);
+
+// a4 -- fused relaxation of A through a ReLU, both branches, with the bias
+// accumulation of the ReLU (bU through the sign-selected part of A) and of the linear layer below
+// (d += Abar . b), and the TF32 hi/lo operand split for the contraction that follows.
+struct RelaxArgs {
+  AView A;                   // input view (fp32)
+  const float4* coef;        // [B, n] or nullptr: no ReLU here (split / bias only)
+  const float* alpha_lo;     // [B, R, n] or nullptr (fixed rule)
+  const float* alpha_up;     // [B, R, n] or nullptr
+  const float* bias;         // bias of the layer below, [n / bias_div], or nullptr
+  int bias_div;              // 1 for Linear; H'*W' for a Conv2d bias per channel
+  float* out;                // [2,B,R,n] contiguous: fp32 result, or TF32 hi part when out_lo given
+  float* out_lo;             // TF32 lo part or nullptr
+  float* d;                  // [2,B,R] in/out: d += ...
+  int B, R, n;
+};
+void launch_relax(const RelaxArgs& a, cudaStream_t s);
+
+// a8 -- concretisation: lb = A.x_c - |A|.x_r + d (br 0), ub = A.x_c + |A|.x_r + d.
+void launch_concretize(const AView& A, const float* d, const float* x_lo, const float* x_hi,
+                       float* lb, float* ub, int out_stride, int B, int R, cudaStream_t s);
+
+// a1 -- IBP through a Linear layer in centre/radius form:
+// c' = W c + b, r' = |W| r; l' = c' - r', u' = c' + r'.  relu_in: clamp the input interval at 0 first.
+void launch_ibp_linear(const float* W, const float* bias, const float* l_in, const float* u_in,
+                       int relu_in, float* l_out, float* u_out, int B, int n_out, int n_in,
+                       cudaStream_t s);
+
+// IBP through ReLU / Add (elementwise).
+void launch_ibp_relu(const float* l, const float* u, float* lo, float* uo, long long count, cudaStream_t s);
+void launch_ibp_add(const float* l0, const float* u0, const float* l1, const float* u1,
+                    float* lo, float* uo, long long count, cudaStream_t s);
+
+// d[br,b,r] = bias[row0 + r] (start of an identity pass: d = I . b_k), or 0 when bias == nullptr.
+void launch_init_d(float* d, const float* bias, int row0, int B, int R, cudaStream_t s);
+// d[br,b,r] += sum_j A[br,b,r,j] * bias[j / bias_div]   (unfused bias of a Linear / Conv2d layer)
+void launch_rowdot_bias(const AView& A, const float* bias, int bias_div, float* d, int B, int R,
+                        cudaStream_t s);
+// out[2,B,R,n] contiguous = view a (+ view b)
+void launch_view_add(const AView& a, const AView* b, float* out, int B, int R, cudaStream_t s);
+// a9 -- verdict: verified[b] = min_s lb[b,s] > 0
+void launch_verdict(const float* lb, uint8_t* verified, int B, int S, cudaStream_t s);
+
+// X [rows, cols] -> TF32 hi/lo parts, optionally transposed to [cols, rows] (weight prepack).
+void launch_split_tf32(const float* X, int rows, int cols, int transpose, float* hi, float* lo,
+                       cudaStream_t s);
+
+// a5 fallback -- fp32 FFMA contraction D[M,N] = A[M,K] . W[K,N] (arbitrary shapes, CUDA cores).
+void launch_gemm_ffma(const float* A, long long lda, const float* W, long long ldw, float* D,
+                      long long ldd, int M, int N, int K, cudaStream_t s);
+
+// a5 -- 3xTF32 contraction on tcgen05 tensor cores: D[M,N] = (A_hi + A_lo)[M,K] . (Wt_hi + Wt_lo)[N,K]^T
+// with the three products hi.hi + hi.lo + lo.hi accumulated in fp32 (TMEM), drained to an fp32
+// CUDA-core running sum every k_drain elements of K.
+struct TmapSet;  // opaque TMA descriptors of one (A, W) operand pair, built on the host
+int gemm_tc_supported(int M, int N, int K);
+int launch_gemm_tc(const float* A_hi, const float* A_lo, const float* Wt_hi, const float* Wt_lo,
+                   float* D, long long ldd, int M, int N, int K, int k_drain, int num_sms,
+                   cudaStream_t s, const char** err);
+
+// a2 / a6 -- Conv2d IBP (centre/radius) and conv-transpose backward of A.
+void launch_ibp_conv(const float* W, const float* bias, const float* l_in, const float* u_in,
+                     int relu_in, float* l_out, float* u_out, int B, int c_in, int h, int w,
+                     int c_out, int kh, int kw, int stride, int pad, int ho, int wo, cudaStream_t s);
+void launch_conv_transpose(const AView& A, const float* W, const float* addend, float* out,
+                           int rows_total, int c_in, int h, int w, int c_out, int kh, int kw,
+                           int stride, int pad, int ho, int wo, cudaStream_t s);
+
+}  // namespace crownb200
