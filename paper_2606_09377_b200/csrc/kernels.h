@@ -85,7 +85,7 @@ void launch_ibp_conv(const float* W, const float* bias, const float* l_in, const
                      int relu_in, float* l_out, float* u_out, int B, int c_in, int h, int w,
                      int c_out, int kh, int kw, int stride, int pad, int ho, int wo, cudaStream_t s);
 void launch_conv_transpose(const AView& A, const float* W, const float* addend, float* out,
-                           int rows_total, int c_in, int h, int w, int c_out, int kh, int kw,
+                           int B, int R, int c_in, int h, int w, int c_out, int kh, int kw,
                            int stride, int pad, int ho, int wo, cudaStream_t s);
 
 }  // namespace crownb200
