@@ -122,6 +122,8 @@ float* ibp_tmp_u(crown_ctx* ctx, int i) {
   return reinterpret_cast<float*>(ctx->ibp_base + ctx->ibp_off[i] + align_up((size_t)ctx->B_max * ctx->nodes[i].size * 4));
 }
 
+}  // namespace
+
 // Interval of every node's output.  L/U receive the pointer actually used per node (caller's or scratch).
 // only_first_layer: stop after the Linear/Conv nodes fed directly by the network input.
 int ibp_internal(crown_ctx* ctx, int B, const float* x_lo, const float* x_hi, float* const* l_dev,
@@ -206,7 +208,6 @@ int ibp_internal(crown_ctx* ctx, int B, const float* x_lo, const float* x_hi, fl
   return CROWN_OK;
 }
 
-}  // namespace
 
 extern "C" int ibp_forward(crown_ctx* ctx, int B, const float* x_lo_dev, const float* x_hi_dev,
                            float* const* l_dev, float* const* u_dev, const float* C_dev, int S,

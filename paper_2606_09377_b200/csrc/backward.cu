@@ -1,0 +1,372 @@
+// O3 -- the CROWN backward pass (PAPER.md:64-68 Eq. 1, :128 A <- A.Lambda_i W_i), the concretisation
+// and the whole-path drivers crown_run / crown_run_host (O4, O5, verdict).
+// Host scheduling only: every arithmetic step is a kernel of kernels.h.
+#include "ctx.h"
+
+namespace {
+
+struct Pass {
+  crown_ctx* ctx;
+  int B, R;
+  std::map<int, Pending> pend;   // node id (-1 = network input) -> A w.r.t. that node's OUTPUT
+};
+
+// a fresh contiguous [2,B,R,n] buffer from the pool
+int new_buf(Pass& ps, float*& ptr) {
+  int id = pool_get(ps.ctx);
+  if (id < 0) return -1;
+  ptr = pool_ptr(ps.ctx, id);
+  return id;
+}
+
+// d += A . bias of Linear/Conv node j, unless the view already carries it
+void add_bias(Pass& ps, Pending& p, int j) {
+  crown_ctx* ctx = ps.ctx;
+  if (p.bias_done_for == j) return;
+  const NodeInfo& nj = ctx->nodes[j];
+  if (!nj.n.b_dev) return;
+  int div = nj.n.op == CROWN_CONV2D ? nj.h * nj.w : 1;
+  Scope sc(ctx, CROWN_K_MISC, 4.0 * 2 * ps.B * ps.R * p.v.n);
+  launch_rowdot_bias(p.v, nj.n.b_dev, div, ctx->d_buf, ps.B, ps.R, ctx->stream);
+}
+
+// Add a contribution to node `idx`.  A node with several consumers (residual fork) receives the SUM of
+// their contributions.
+int contribute(Pass& ps, int idx, Pending p) {
+  crown_ctx* ctx = ps.ctx;
+  auto it = ps.pend.find(idx);
+  if (it == ps.pend.end()) { ps.pend[idx] = p; return CROWN_OK; }
+  Pending& q = it->second;
+  float* out = nullptr;
+  int nb = new_buf(ps, out);
+  if (nb < 0) return fail(ctx, CROWN_ENOMEM, "backward: A-buffer pool exhausted at a fork");
+  int done = -2;
+  if (idx >= 0 && (ctx->nodes[idx].n.op == CROWN_LINEAR || ctx->nodes[idx].n.op == CROWN_CONV2D)) {
+    add_bias(ps, q, idx); add_bias(ps, p, idx); done = idx;   // each part carries its own A.b before the sum
+  }
+  { Scope sc(ctx, CROWN_K_MISC, 12.0 * 2 * ps.B * ps.R * p.v.n);
+    launch_view_add(q.v, &p.v, out, ps.B, ps.R, ctx->stream); }
+  release(ctx, q); release(ctx, p);
+  Pending m; m.v = canon_view(out, ps.B, ps.R, p.v.n); m.buf = nb; m.bias_done_for = done;
+  it->second = m;
+  return CROWN_OK;
+}
+
+
+float4* coef_ptr(crown_ctx* ctx, int i) { return reinterpret_cast<float4*>(ctx->coef_base + ctx->coef_off[i]); }
+
+// One backward pass.  coef_ready: per node, 1 if coef_ptr(i) already holds the coefficients of ReLU i for the
+// bounds in l_dev/u_dev (crown_run computes each ReLU's coefficients once); may be nullptr.
+int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_dev,
+             const float* const* l_dev, const float* const* u_dev, const float* const* alpha_lo,
+             const float* const* alpha_up, float* A_dev, float* d_dev, const float* x_lo, const float* x_hi,
+             float* lb, float* ub, int out_stride, std::vector<char>* coef_ready) {
+  const int n = (int)ctx->nodes.size();
+  cudaStream_t s = ctx->stream;
+  if (B <= 0 || B > ctx->B_max || R <= 0 || R > ctx->plan.rows_cap || start < 0 || start >= n)
+    return fail(ctx, CROWN_EINVAL, "crown_backward: bad B / rows / start");
+  if (lb && (!ub || !x_lo || !x_hi)) return fail(ctx, CROWN_EINVAL, "crown_backward: concretisation needs ub, x_lo, x_hi");
+  std::fill(ctx->pool_ref.begin(), ctx->pool_ref.end(), 0);
+  Pass ps; ps.ctx = ctx; ps.B = B; ps.R = R;
+  const NodeInfo& sn = ctx->nodes[start];
+  int first = start;   // first node to visit in the reverse sweep
+  if (C_dev) {
+    { Scope sc(ctx, CROWN_K_MISC); launch_init_d(ctx->d_buf, nullptr, 0, B, R, s); }
+    Pending p; p.v.p = C_dev; p.v.ld = sn.size; p.v.n = sn.size; p.v.sB = (long long)R * sn.size; p.v.sBr = 0;
+    ps.pend[start] = p;
+  } else {
+    // rows [row0, row0+R) of the identity on a Linear node: I.W = those rows of W, I.b = those biases
+    if (sn.n.op != CROWN_LINEAR) return fail(ctx, CROWN_EUNSUPPORTED, "crown_backward: identity start needs a Linear node");
+    if (row0 < 0 || row0 + R > sn.size) return fail(ctx, CROWN_EINVAL, "crown_backward: row range outside the start node");
+    { Scope sc(ctx, CROWN_K_MISC); launch_init_d(ctx->d_buf, sn.n.b_dev, row0, B, R, s); }
+    Pending p; p.v.p = sn.n.W_dev + (long long)row0 * sn.n.n_in; p.v.ld = sn.n.n_in; p.v.n = sn.n.n_in;
+    p.v.sB = 0; p.v.sBr = 0;
+    ps.pend[sn.n.in0] = p;
+    first = start - 1;
+  }
+  for (int i = first; i >= 0; --i) {
+    auto it = ps.pend.find(i);
+    if (it == ps.pend.end()) continue;
+    Pending cur = it->second;
+    ps.pend.erase(it);
+    const NodeInfo& ni = ctx->nodes[i];
+    const crown_node& nd = ni.n;
+    int rc = CROWN_OK;
+    switch (nd.op) {
+      case CROWN_RELU: {
+        if (!l_dev || !u_dev || !l_dev[i] || !u_dev[i]) return fail(ctx, CROWN_EINVAL, "crown_backward: bounds of a ReLU below start are missing");
+        if (!coef_ready || !(*coef_ready)[i]) {
+          Scope sc(ctx, CROWN_K_COEFF, 24.0 * B * ni.size);
+          launch_relax_coeffs(l_dev[i], u_dev[i], coef_ptr(ctx, i), (long long)B * ni.size, ctx->opts.slope_rule, s);
+          if (coef_ready) (*coef_ready)[i] = 1;
+        }
+        const int j = nd.in0;
+        const bool lin_below = j >= 0 && (ctx->nodes[j].n.op == CROWN_LINEAR || ctx->nodes[j].n.op == CROWN_CONV2D);
+        // the product that follows runs on the tensor cores when the producer is a prepacked Linear
+        const bool tc = lin_below && ctx->nodes[j].tc_ok && gemm_tc_supported(2 * B * R, ctx->nodes[j].n.n_in, ctx->nodes[j].n.n_out);
+        RelaxArgs ra;
+        ra.A = cur.v; ra.coef = coef_ptr(ctx, i);
+        ra.alpha_lo = alpha_lo ? alpha_lo[i] : nullptr;
+        ra.alpha_up = alpha_up ? alpha_up[i] : nullptr;
+        ra.bias = lin_below ? ctx->nodes[j].n.b_dev : nullptr;
+        ra.bias_div = (lin_below && ctx->nodes[j].n.op == CROWN_CONV2D) ? ctx->nodes[j].h * ctx->nodes[j].w : 1;
+        ra.d = ctx->d_buf; ra.B = B; ra.R = R; ra.n = ni.size;
+        Pending out;
+        out.buf = new_buf(ps, ra.out);
+        if (out.buf < 0) return fail(ctx, CROWN_ENOMEM, "backward: A-buffer pool exhausted");
+        ra.out_lo = nullptr;
+        if (tc) { out.buf_lo = new_buf(ps, ra.out_lo); if (out.buf_lo < 0) return fail(ctx, CROWN_ENOMEM, "backward: A-buffer pool exhausted"); }
+        const double elems = 2.0 * B * R * ni.size;
+        { Scope sc(ctx, CROWN_K_RELAX, elems * (tc ? 12.0 : 8.0) + ((ra.alpha_lo || ra.alpha_up) ? 4.0 * B * R * ni.size : 0.0));
+          launch_relax(ra, s); }
+        out.v = canon_view(ra.out, B, R, ni.size); out.v.lo = ra.out_lo;
+        out.bias_done_for = lin_below ? j : -2;
+        release(ctx, cur);
+        rc = contribute(ps, j, out);
+        break; }
+      case CROWN_LINEAR: {
+        add_bias(ps, cur, i);
+        const int M_full = 2 * B * R;
+        Pending out;
+        float* D = nullptr;
+        if (ni.tc_ok && gemm_tc_supported(M_full, nd.n_in, nd.n_out)) {
+          const float *hi = cur.v.p, *lo = cur.v.lo;
+          Pending tmp;
+          if (!lo) {   // operand not split yet (start matrix, fork sum): split pass, also makes it contiguous
+            RelaxArgs ra; ra.A = cur.v; ra.coef = nullptr; ra.alpha_lo = ra.alpha_up = nullptr; ra.bias = nullptr; ra.bias_div = 1;
+            ra.d = nullptr; ra.B = B; ra.R = R; ra.n = ni.size;
+            tmp.buf = new_buf(ps, ra.out); tmp.buf_lo = new_buf(ps, ra.out_lo);
+            if (tmp.buf < 0 || tmp.buf_lo < 0) return fail(ctx, CROWN_ENOMEM, "backward: A-buffer pool exhausted");
+            { Scope sc(ctx, CROWN_K_RELAX, 12.0 * M_full * ni.size); launch_relax(ra, s); }
+            hi = ra.out; lo = ra.out_lo;
+            release(ctx, cur); cur = tmp;
+          }
+          out.buf = new_buf(ps, D);
+          if (out.buf < 0) return fail(ctx, CROWN_ENOMEM, "backward: A-buffer pool exhausted");
+          const char* e = nullptr;
+          { Scope sc(ctx, CROWN_K_GEMM_TC, 4.0 * ((double)M_full * nd.n_out + (double)nd.n_out * nd.n_in + (double)M_full * nd.n_in),
+                     2.0 * M_full * (double)nd.n_in * nd.n_out);
+            if (launch_gemm_tc(hi, lo, ni.Wt_hi, ni.Wt_lo, D, nd.n_in, M_full, nd.n_in, nd.n_out, ctx->opts.k_drain, ctx->num_sms, s, &e))
+              return fail(ctx, CROWN_ECUDA, std::string("gemm_tc: ") + (e ? e : "?")); }
+          ctx->gemm_flops += 2.0 * M_full * (double)nd.n_in * nd.n_out;
+          out.v = canon_view(D, B, R, nd.n_in);
+        } else {
+          // CUDA-core contraction; rows shared between branches / properties are multiplied once
+          int m_eff = 0;
+          if (!view_uniform(cur.v, B, R, m_eff)) return fail(ctx, CROWN_EINVAL, "backward: non-uniform A view");
+          out.buf = new_buf(ps, D);
+          if (out.buf < 0) return fail(ctx, CROWN_ENOMEM, "backward: A-buffer pool exhausted");
+          { Scope sc(ctx, CROWN_K_GEMM_FFMA, 4.0 * ((double)m_eff * nd.n_out + (double)nd.n_out * nd.n_in + (double)m_eff * nd.n_in),
+                     2.0 * m_eff * (double)nd.n_in * nd.n_out);
+            launch_gemm_ffma(cur.v.p, cur.v.ld, nd.W_dev, nd.n_in, D, nd.n_in, m_eff, nd.n_in, nd.n_out, s); }
+          ctx->gemm_flops += 2.0 * m_eff * (double)nd.n_in * nd.n_out;
+          out.v.p = D; out.v.ld = nd.n_in; out.v.n = nd.n_in;
+          out.v.sB = cur.v.sB ? (long long)R * nd.n_in : 0;
+          out.v.sBr = cur.v.sBr ? (long long)(cur.v.sB ? B : 1) * R * nd.n_in : 0;
+        }
+        release(ctx, cur);
+        rc = contribute(ps, nd.in0, out);
+        break; }
+      case CROWN_CONV2D: {
+        add_bias(ps, cur, i);
+        Pending out;
+        float* D = nullptr;
+        out.buf = new_buf(ps, D);
+        if (out.buf < 0) return fail(ctx, CROWN_ENOMEM, "backward: A-buffer pool exhausted");
+        const int in_size = nd.c_in * nd.h_in * nd.w_in;
+        { Scope sc(ctx, CROWN_K_CONV, 4.0 * 2 * B * R * ((double)ni.size + in_size),
+                   2.0 * 2 * B * R * (double)ni.size * nd.c_in * nd.kh * nd.kw);
+          launch_conv_transpose(cur.v, nd.W_dev, nullptr, D, B, R, nd.c_in, nd.h_in, nd.w_in, nd.c_out, nd.kh, nd.kw,
+                                nd.stride, nd.pad, ni.h, ni.w, s); }
+        out.v = canon_view(D, B, R, in_size);
+        release(ctx, cur);
+        rc = contribute(ps, nd.in0, out);
+        break; }
+      case CROWN_ADD: {
+        Pending second = cur;
+        pool_retain(ctx, second.buf); pool_retain(ctx, second.buf_lo);
+        rc = contribute(ps, nd.in0, cur);
+        if (rc == CROWN_OK) rc = contribute(ps, nd.in1, second);
+        break; }
+      case CROWN_FLATTEN:
+        rc = contribute(ps, nd.in0, cur);
+        break;
+      default:
+        return fail(ctx, CROWN_EUNSUPPORTED, "crown_backward: unsupported op");
+    }
+    if (rc) return rc;
+  }
+  // A w.r.t. the network input
+  auto it = ps.pend.find(-1);
+  if (it == ps.pend.end()) return fail(ctx, CROWN_EINVAL, "crown_backward: start node does not reach the input");
+  Pending a0 = it->second;
+  if (a0.v.n != ctx->n0) return fail(ctx, CROWN_EINVAL, "crown_backward: internal size mismatch at the input");
+  if (A_dev) { Scope sc(ctx, CROWN_K_MISC, 8.0 * 2 * B * R * ctx->n0); launch_view_add(a0.v, nullptr, A_dev, B, R, s); }
+  if (d_dev) CK(ctx, cudaMemcpyAsync(d_dev, ctx->d_buf, (size_t)2 * B * R * 4, cudaMemcpyDeviceToDevice, s));
+  if (lb) { Scope sc(ctx, CROWN_K_CONCRETIZE, 4.0 * 2 * B * R * ctx->n0, 4.0 * 2 * B * R * ctx->n0);
+            launch_concretize(a0.v, ctx->d_buf, x_lo, x_hi, lb, ub, out_stride, B, R, s); }
+  release(ctx, a0);
+  CK(ctx, cudaGetLastError());
+  return CROWN_OK;
+}
+
+}  // namespace
+
+extern "C" int crown_backward(crown_ctx* ctx, int B, int start, int row0, int rows, const float* C_dev,
+                              const float* const* l_dev, const float* const* u_dev,
+                              const float* const* alpha_lo_dev, const float* const* alpha_up_dev,
+                              float* A_dev, float* d_dev, const float* x_lo_dev, const float* x_hi_dev,
+                              float* lb_dev, float* ub_dev) {
+  if (!ctx) return CROWN_EINVAL;
+  if (!A_dev && !d_dev && !lb_dev) return fail(ctx, CROWN_EINVAL, "crown_backward: no output requested");
+  return run_pass(ctx, B, start, row0, rows, C_dev, l_dev, u_dev, alpha_lo_dev, alpha_up_dev, A_dev, d_dev,
+                  x_lo_dev, x_hi_dev, lb_dev, ub_dev, rows, nullptr);
+}
+
+extern "C" int concretize(crown_ctx* ctx, int B, int rows, const float* A_dev, const float* d_dev,
+                          const float* x_lo_dev, const float* x_hi_dev, float* lb_dev, float* ub_dev,
+                          int out_stride) {
+  if (!ctx) return CROWN_EINVAL;
+  if (B <= 0 || rows <= 0 || !A_dev || !x_lo_dev || !x_hi_dev || !lb_dev || !ub_dev || out_stride < rows)
+    return fail(ctx, CROWN_EINVAL, "concretize: bad arguments");
+  AView v = canon_view(A_dev, B, rows, ctx->n0);
+  { Scope sc(ctx, CROWN_K_CONCRETIZE, 4.0 * 2 * B * rows * ctx->n0, 4.0 * 2 * B * rows * ctx->n0);
+    launch_concretize(v, d_dev, x_lo_dev, x_hi_dev, lb_dev, ub_dev, out_stride, B, rows, ctx->stream); }
+  CK(ctx, cudaGetLastError());
+  return CROWN_OK;
+}
+
+// ================================================================================================
+// O4 + O5 + verdict: the whole hot path for one batch
+// ================================================================================================
+extern "C" int crown_run(crown_ctx* ctx, int B, const float* x_lo_dev, const float* x_hi_dev,
+                         const float* C_dev, int S, const float* const* alpha_dev, int intermediate,
+                         float* const* l_dev, float* const* u_dev, float* lb_dev, float* ub_dev,
+                         uint8_t* verified_dev) {
+  if (!ctx) return CROWN_EINVAL;
+  const int n = (int)ctx->nodes.size();
+  if (B <= 0 || B > ctx->B_max || S <= 0 || S > ctx->S_max || !x_lo_dev || !x_hi_dev || !C_dev || !l_dev ||
+      !u_dev || !lb_dev || !ub_dev || (intermediate != 0 && intermediate != 1))
+    return fail(ctx, CROWN_EINVAL, "crown_run: bad arguments");
+  std::vector<int> relus;
+  for (int i = 0; i < n; ++i)
+    if (ctx->nodes[i].n.op == CROWN_RELU) {
+      if (!l_dev[i] || !u_dev[i]) return fail(ctx, CROWN_EINVAL, "crown_run: l_dev/u_dev entry of a ReLU node is NULL");
+      if (ctx->nodes[i].n.in0 < 0) return fail(ctx, CROWN_EUNSUPPORTED, "crown_run: ReLU directly on the input");
+      relus.push_back(i);
+    }
+  // IBP writes the OUTPUT interval of node in0(relu) straight into the caller's pre-activation buffers
+  std::vector<float*> lmap(n, nullptr), umap(n, nullptr), L, U;
+  std::vector<const float*> lc(n, nullptr), uc(n, nullptr);
+  for (int i : relus) {
+    const int src = ctx->nodes[i].n.in0;
+    if (lmap[src]) return fail(ctx, CROWN_EUNSUPPORTED, "crown_run: two ReLUs on one node");
+    lmap[src] = l_dev[i]; umap[src] = u_dev[i];
+    lc[i] = l_dev[i]; uc[i] = u_dev[i];
+  }
+  std::vector<char> coef_ready(n, 0);
+  int rc;
+  if (intermediate == 1) {
+    rc = ibp_internal(ctx, B, x_lo_dev, x_hi_dev, lmap.data(), umap.data(), L, U, false);
+    if (rc) return rc;
+  } else {
+    rc = ibp_internal(ctx, B, x_lo_dev, x_hi_dev, lmap.data(), umap.data(), L, U, true);
+    if (rc) return rc;
+    for (int i : relus) {
+      const int src = ctx->nodes[i].n.in0;
+      const crown_node& sn = ctx->nodes[src].n;
+      if ((sn.op == CROWN_LINEAR || sn.op == CROWN_CONV2D) && sn.in0 < 0) continue;   // first layer: O1 (exact)
+      if (sn.op != CROWN_LINEAR)
+        return fail(ctx, CROWN_EUNSUPPORTED, "crown_run: CROWN intermediate bounds need Linear pre-activations (use intermediate=1)");
+      const int size = ctx->nodes[src].size;
+      for (int row0 = 0; row0 < size; row0 += ctx->plan.rc) {
+        const int rows = std::min(ctx->plan.rc, size - row0);
+        rc = run_pass(ctx, B, src, row0, rows, nullptr, lc.data(), uc.data(), nullptr, nullptr, nullptr, nullptr,
+                      x_lo_dev, x_hi_dev, l_dev[i] + row0, u_dev[i] + row0, size, &coef_ready);
+        if (rc) return rc;
+      }
+    }
+  }
+  rc = run_pass(ctx, B, n - 1, 0, S, C_dev, lc.data(), uc.data(), alpha_dev, alpha_dev, nullptr, nullptr,
+                x_lo_dev, x_hi_dev, lb_dev, ub_dev, S, &coef_ready);
+  if (rc) return rc;
+  if (verified_dev) { Scope sc(ctx, CROWN_K_MISC); launch_verdict(lb_dev, verified_dev, B, S, ctx->stream); }
+  CK(ctx, cudaGetLastError());
+  return CROWN_OK;
+}
+
+extern "C" int crown_run_host(crown_ctx* ctx, int B, const float* x_lo_host, const float* x_hi_host,
+                              const float* C_host, int S, const float* const* alpha_host, int intermediate,
+                              float* lb_host, float* ub_host, uint8_t* verified_host) {
+  if (!ctx) return CROWN_EINVAL;
+  const int n = (int)ctx->nodes.size();
+  if (B <= 0 || B > ctx->B_max || S <= 0 || S > ctx->S_max || !x_lo_host || !x_hi_host || !C_host || !lb_host || !ub_host)
+    return fail(ctx, CROWN_EINVAL, "crown_run_host: bad arguments");
+  cudaStream_t s = ctx->stream;
+  uint8_t* cur = ctx->io_base;
+  auto take = [&](size_t bytes) { uint8_t* p = cur; cur += align_up(bytes); return p; };
+  std::vector<float*> l(n, nullptr), u(n, nullptr);
+  std::vector<const float*> al(n, nullptr);
+  bool any_alpha = false;
+  for (int i = 0; i < n; ++i) {
+    if (ctx->nodes[i].n.op != CROWN_RELU) continue;
+    const size_t sz = ctx->nodes[i].size;
+    float* a = reinterpret_cast<float*>(take((size_t)ctx->B_max * ctx->S_max * sz * 4));
+    l[i] = reinterpret_cast<float*>(take((size_t)ctx->B_max * sz * 4));
+    u[i] = reinterpret_cast<float*>(take((size_t)ctx->B_max * sz * 4));
+    if (alpha_host && alpha_host[i]) {
+      CK(ctx, cudaMemcpyAsync(a, alpha_host[i], (size_t)B * S * sz * 4, cudaMemcpyHostToDevice, s));
+      al[i] = a; any_alpha = true;
+    }
+  }
+  float* xl = reinterpret_cast<float*>(take((size_t)ctx->B_max * ctx->n0 * 4));
+  float* xh = reinterpret_cast<float*>(take((size_t)ctx->B_max * ctx->n0 * 4));
+  const size_t nL = ctx->nodes.back().size;
+  float* C = reinterpret_cast<float*>(take((size_t)ctx->B_max * ctx->S_max * nL * 4));
+  float* lb = reinterpret_cast<float*>(take((size_t)ctx->B_max * ctx->S_max * 4));
+  float* ub = reinterpret_cast<float*>(take((size_t)ctx->B_max * ctx->S_max * 4));
+  uint8_t* ver = take((size_t)ctx->B_max);
+  CK(ctx, cudaMemcpyAsync(xl, x_lo_host, (size_t)B * ctx->n0 * 4, cudaMemcpyHostToDevice, s));
+  CK(ctx, cudaMemcpyAsync(xh, x_hi_host, (size_t)B * ctx->n0 * 4, cudaMemcpyHostToDevice, s));
+  CK(ctx, cudaMemcpyAsync(C, C_host, (size_t)B * S * nL * 4, cudaMemcpyHostToDevice, s));
+  int rc = crown_run(ctx, B, xl, xh, C, S, any_alpha ? al.data() : nullptr, intermediate, l.data(), u.data(), lb, ub, ver);
+  if (rc) return rc;
+  CK(ctx, cudaMemcpyAsync(lb_host, lb, (size_t)B * S * 4, cudaMemcpyDeviceToHost, s));
+  CK(ctx, cudaMemcpyAsync(ub_host, ub, (size_t)B * S * 4, cudaMemcpyDeviceToHost, s));
+  if (verified_host) CK(ctx, cudaMemcpyAsync(verified_host, ver, (size_t)B, cudaMemcpyDeviceToHost, s));
+  CK(ctx, cudaStreamSynchronize(s));
+  return CROWN_OK;
+}
+
+// ================================================================================================
+// kernel 1 exposed on its own (parity tests, roofline measurement)
+// ================================================================================================
+extern "C" int crown_split_tf32(crown_ctx* ctx, const float* X_dev, int rows, int cols, int transpose,
+                                float* hi_dev, float* lo_dev) {
+  if (!ctx) return CROWN_EINVAL;
+  if (!X_dev || !hi_dev || !lo_dev || rows <= 0 || cols <= 0) return fail(ctx, CROWN_EINVAL, "crown_split_tf32: bad arguments");
+  { Scope sc(ctx, CROWN_K_MISC); launch_split_tf32(X_dev, rows, cols, transpose, hi_dev, lo_dev, ctx->stream); }
+  CK(ctx, cudaGetLastError());
+  return CROWN_OK;
+}
+
+extern "C" int crown_gemm(crown_ctx* ctx, int scheme, int M, int N, int K, const float* A_hi_dev,
+                          const float* A_lo_dev, const float* Wt_hi_dev, const float* Wt_lo_dev, float* D_dev) {
+  if (!ctx) return CROWN_EINVAL;
+  if (M <= 0 || N <= 0 || K <= 0 || !A_hi_dev || !Wt_hi_dev || !D_dev) return fail(ctx, CROWN_EINVAL, "crown_gemm: bad arguments");
+  if (scheme == 0) {
+    if (!A_lo_dev || !Wt_lo_dev) return fail(ctx, CROWN_EINVAL, "crown_gemm: 3xTF32 needs the lo parts");
+    const char* e = nullptr;
+    Scope sc(ctx, CROWN_K_GEMM_TC, 4.0 * ((double)M * K + (double)K * N + (double)M * N), 2.0 * M * (double)N * K);
+    if (launch_gemm_tc(A_hi_dev, A_lo_dev, Wt_hi_dev, Wt_lo_dev, D_dev, N, M, N, K, ctx->opts.k_drain, ctx->num_sms, ctx->stream, &e))
+      return fail(ctx, CROWN_EINVAL, std::string("crown_gemm: ") + (e ? e : "?"));
+  } else if (scheme == 2) {
+    // FFMA path takes W [K,N] row-major in Wt_hi_dev (NOT transposed) and fp32 A in A_hi_dev
+    Scope sc(ctx, CROWN_K_GEMM_FFMA, 4.0 * ((double)M * K + (double)K * N + (double)M * N), 2.0 * M * (double)N * K);
+    launch_gemm_ffma(A_hi_dev, K, Wt_hi_dev, N, D_dev, N, M, N, K, ctx->stream);
+  } else {
+    return fail(ctx, CROWN_EINVAL, "crown_gemm: unknown scheme");
+  }
+  CK(ctx, cudaGetLastError());
+  return CROWN_OK;
+}

@@ -228,3 +228,7 @@ bool view_uniform(const AView& v, int B, int R, int& m_eff) {
 }
 
 }  // namespace
+
+// api.cu: interval of every node's OUTPUT (O1).  L/U receive the pointer used per node (caller's or scratch).
+int ibp_internal(crown_ctx* ctx, int B, const float* x_lo, const float* x_hi, float* const* l_dev,
+                 float* const* u_dev, std::vector<float*>& L, std::vector<float*>& U, bool only_first_layer);

@@ -1,0 +1,153 @@
+"""GPU parity (`-m gpu`): the CUDA path, called through the C-ABI binding, against the float64 oracle on
+the same seeded inputs, element by element.  Tolerance (BASELINE.json north_star, reading G18):
+|gpu - oracle| <= 1e-5 + 1e-4 |oracle|.  Forced-bounds protocol: where the oracle needs intermediate bounds
+it is given the GPU's own (l, u) upcast to float64, so a relaxation-class flip at a discontinuity
+cannot masquerade as (or hide) an arithmetic error; free-running parity is checked in addition."""
+import numpy as np
+import pytest
+
+import workloads as W
+from oracle import crown_oracle as O
+
+pytestmark = pytest.mark.gpu
+
+ATOL, RTOL = 1e-5, 1e-4
+
+
+def _ctx(net, B, S, **kw):
+    from paper_2606_09377_b200 import CrownContext
+    return CrownContext(net, B, S, **kw)
+
+
+def _close(gpu, ref, what, atol=ATOL, rtol=RTOL):
+    gpu = np.asarray(gpu, np.float64)
+    ref = np.asarray(ref, np.float64)
+    err = np.abs(gpu - ref) - (atol + rtol * np.abs(ref))
+    assert np.all(err <= 0), f"{what}: worst excess {err.max():.3e} at {np.unravel_index(err.argmax(), err.shape)}"
+
+
+def _np(t):
+    return t.detach().cpu().numpy()
+
+
+# ------------------------------------------------------------------------------------------ kernel 1
+@pytest.mark.parametrize("M,N,K", [(128, 128, 32), (256, 384, 512), (300, 260, 1000), (1152, 784, 256),
+                                   (128, 4096, 16384)])
+def test_gemm_3xtf32_matches_fp64(M, N, K):
+    import torch
+    rng = np.random.default_rng(M * 7 + N * 3 + K)
+    A = rng.standard_normal((M, K)).astype(np.float32)
+    Wm = (rng.standard_normal((K, N)) * np.sqrt(2.0 / K)).astype(np.float32)
+    net = W.small_mlp([4, 4, 2], 0).net
+    ctx = _ctx(net, 1, 1)
+    D = _np(ctx.gemm(torch.from_numpy(A), torch.from_numpy(Wm), scheme=0))
+    ref = A.astype(np.float64) @ Wm.astype(np.float64)
+    # fp32-accurate: error relative to the row/column magnitude, not to the (possibly cancelling) result
+    scale = np.abs(A).astype(np.float64) @ np.abs(Wm).astype(np.float64)
+    assert np.max(np.abs(D - ref) / scale) < 2e-6, np.max(np.abs(D - ref) / scale)
+
+
+@pytest.mark.parametrize("M,N,K", [(18, 256, 10), (65, 130, 33), (512, 784, 256)])
+def test_gemm_ffma_matches_fp64(M, N, K):
+    import torch
+    rng = np.random.default_rng(M + N + K)
+    A = rng.standard_normal((M, K)).astype(np.float32)
+    Wm = rng.standard_normal((K, N)).astype(np.float32)
+    ctx = _ctx(W.small_mlp([4, 4, 2], 0).net, 1, 1)
+    D = _np(ctx.gemm(torch.from_numpy(A), torch.from_numpy(Wm), scheme=2))
+    ref = A.astype(np.float64) @ Wm.astype(np.float64)
+    scale = np.abs(A).astype(np.float64) @ np.abs(Wm).astype(np.float64)
+    assert np.max(np.abs(D - ref) / scale) < 1e-6
+
+
+# ------------------------------------------------------------------------------------------ whole path
+def _oracle_forced(wl, gpu_pre, props):
+    """Oracle bounds with the GPU's (l,u) forced for EARLIER ReLUs (layer-wise parity, G18)."""
+    lo, hi = wl.box()
+    out = []
+    for p in props:
+        forced = {i: (_np(l)[p].astype(np.float64), _np(u)[p].astype(np.float64)) for i, (l, u) in gpu_pre.items()}
+        pre = O.crown_bounds(wl.net, lo[p], hi[p], wl.intermediate, forced=forced)
+        al = None if wl.alpha is None else {i: a[p] for i, a in zip(wl.net.relu_ids(), wl.alpha)}
+        lb, ub, _ = O.final_bounds(wl.net, lo[p], hi[p], wl.C[p], forced, al, al)
+        out.append((pre, lb, ub))
+    return out
+
+
+def _check_workload(wl, props=None, free_running=True, **kw):
+    lo, hi = wl.box()
+    ctx = _ctx(wl.net, wl.B, wl.S, **kw)
+    res = ctx.run(lo, hi, wl.C, wl.alpha, wl.intermediate)
+    props = range(wl.B) if props is None else props
+    forced = _oracle_forced(wl, res["pre"], props)
+    lb, ub = _np(res["lb"]), _np(res["ub"])
+    for k, p in enumerate(props):
+        pre, olb, oub = forced[k]
+        for i in wl.net.relu_ids():
+            _close(_np(res["pre"][i][0])[p], pre[i][0], f"prop {p} relu {i} l")
+            _close(_np(res["pre"][i][1])[p], pre[i][1], f"prop {p} relu {i} u")
+        _close(lb[p], olb, f"prop {p} lb")
+        _close(ub[p], oub, f"prop {p} ub")
+        assert np.all(lb[p] <= ub[p] + ATOL)
+        assert bool(_np(res["verified"])[p]) == bool(np.min(lb[p]) > 0)
+    if free_running:
+        flagged = 0
+        for p in props:
+            r = O.run_property(wl.net, lo[p], hi[p], wl.C[p], None if wl.alpha is None else [a[p] for a in wl.alpha],
+                               wl.intermediate)
+            risky = any(np.any(np.minimum(np.minimum(np.abs(l), np.abs(u)), np.abs(u + l)) < 1e-5 * (1 + np.abs(u - l)))
+                        for l, u in r["pre"].values())
+            if risky:
+                flagged += 1
+                continue
+            _close(lb[p], r["lb"], f"free-running prop {p} lb")
+            _close(ub[p], r["ub"], f"free-running prop {p} ub")
+    # soundness on samples (O6), slack = parity tolerance (G17)
+    for p in list(props)[:2]:
+        X = W.sample_points(max(wl.cfg, 1), lo[p], hi[p], 512, 128)
+        ok, vlo, vhi, _, _ = O.sample_check(wl.net, wl.C[p], X, lb[p], ub[p], slack_rel=RTOL, slack_abs=ATOL)
+        assert ok, (vlo, vhi)
+    return ctx, res
+
+
+@pytest.mark.parametrize("scheme", [2, 0])
+def test_small_mlp(scheme):
+    wl = W.small_mlp([6, 9, 7, 5, 3], seed=3, B=3, eps=0.2)
+    _check_workload(wl, mma_scheme=scheme)
+
+
+@pytest.mark.parametrize("scheme", [2, 0])
+def test_cfg1(scheme):
+    _check_workload(W.make(1), mma_scheme=scheme)
+
+
+def test_cfg2_subset():
+    wl = W.make(2, B=8)
+    _check_workload(wl, props=[0, 3, 7])
+
+
+def test_cfg3_scaled():
+    wl = W.make(3, scale=16, B=4)     # 256-1024-1024-1024-10
+    _check_workload(wl, props=[0, 3])
+
+
+def test_cfg3_scaled_chunked_equals_unchunked():
+    import torch
+    wl = W.make(3, scale=16, B=2)
+    lo, hi = wl.box()
+    r_full = _ctx(wl.net, wl.B, wl.S).run(lo, hi, wl.C, None, "crown")
+    c2 = _ctx(wl.net, wl.B, wl.S, mem_cap_bytes=48 << 20)
+    r_chunk = c2.run(lo, hi, wl.C, None, "crown")
+    assert c2.peak_bytes() <= 48 << 20
+    for k in ("lb", "ub"):
+        assert torch.equal(r_full[k], r_chunk[k]), k     # rows are independent: chunking is bitwise neutral
+
+
+def test_cfg4_scaled():
+    wl = W.make(4, scale=64, B=2)     # 64-4096-64-10
+    _check_workload(wl)
+
+
+def test_cfg5_scaled():
+    wl = W.make(5, scale=4, B=2)
+    _check_workload(wl)
