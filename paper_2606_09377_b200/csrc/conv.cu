@@ -102,11 +102,194 @@ conv_transpose_kernel(const float* __restrict__ A, long long sBr, long long sB, 
   }
 }
 
+
+// ---- a6, fast path: register-tiled gather.  Block = RB rows x CG input-channel groups x PT pixel threads.
+// A thread owns 4 output pixels of ONE stride-parity class (same valid filter taps for all four, spaced XQ apart
+// in the class's x index so that a warp reads consecutive shared-memory words and writes consecutive outputs)
+// times CT input channels: 4*CT accumulators.  Per (co, tap): 4 LDS of A, CT/4 broadcast LDS.128 of W, 4*CT FFMA.
+// A_out of the block's rows is staged, zero-haloed, in shared memory COC output channels at a time together
+// with the filter slice transposed to [co][tap][ci] (ci fastest).
+struct ConvBwdGeom {
+  int c_in, h, w, c_out, ho, wo, pad;
+  int NY, NX, XQ, PT, CG, RB, COC;      // per-class rows / cols / x-quads, thread split, co chunk
+  int omin_y, omin_x, PH, PW;           // shared-memory tile origin and size
+};
+
+template <int KH, int KW, int S, int CT>
+__global__ void __launch_bounds__(256)
+conv_bwd_tiled_kernel(const float* __restrict__ A, long long sBr, long long sB, long long ld, int B, int R,
+                      const float* __restrict__ W, const float* __restrict__ addend, float* __restrict__ out,
+                      ConvBwdGeom g) {
+  extern __shared__ __align__(16) float smem_f[];
+  const int cgct = g.CG * CT;
+  float* Ws = smem_f;                                  // [COC][KH*KW][cgct]
+  float* As = smem_f + g.COC * KH * KW * cgct;         // [RB][COC][PH][PW]
+  const int tid = threadIdx.x;
+  const int nthreads = g.PT * g.CG * g.RB;
+  const int pt = tid % g.PT, cg = (tid / g.PT) % g.CG, rb = tid / (g.PT * g.CG);
+  const long long rows = 2LL * B * R;
+  const long long m_base = (long long)blockIdx.x * g.RB;
+  const int ci_base = blockIdx.y * cgct;
+  // pixel thread -> (parity class, yy, xq)
+  const int per_class = g.NY * g.XQ;
+  const int cls = pt / per_class, rem = pt % per_class;
+  const int cy = cls / S, cx = cls % S;
+  const int yy = rem / g.XQ, xq = rem % g.XQ;
+  const int y = cy + S * yy;
+  const bool active = tid < nthreads;
+  // tap table (loop-invariant): offset inside the tile, or -1 when the tap does not hit this parity class
+  int toff[KH * KW];
+#pragma unroll
+  for (int i = 0; i < KH; ++i)
+#pragma unroll
+    for (int j = 0; j < KW; ++j) {
+      const int ny_ = cy + g.pad - i, nx_ = cx + g.pad - j;
+      const bool ok = (((ny_ % S) + S) % S == 0) && (((nx_ % S) + S) % S == 0);
+      const int oy = ok ? ny_ / S : 0, ox = ok ? nx_ / S : 0;
+      toff[i * KW + j] = ok ? (yy + oy - g.omin_y) * g.PW + (ox - g.omin_x) : -1;
+    }
+  int u[4]; bool uv[4];
+#pragma unroll
+  for (int t = 0; t < 4; ++t) {
+    const int ut = xq + t * g.XQ;
+    uv[t] = active && ut < g.NX && (cx + S * ut) < g.w && y < g.h;
+    u[t] = uv[t] ? ut : 0;
+  }
+  float acc[4][CT];
+#pragma unroll
+  for (int t = 0; t < 4; ++t)
+#pragma unroll
+    for (int c = 0; c < CT; ++c) acc[t][c] = 0.f;
+
+  const int tile = g.PH * g.PW;
+  for (int co0 = 0; co0 < g.c_out; co0 += g.COC) {
+    const int cc = min(g.COC, g.c_out - co0);
+    __syncthreads();
+    // filter slice -> Ws[co][tap][ci]
+    for (int idx = tid; idx < cc * KH * KW * cgct; idx += blockDim.x) {
+      const int c = idx % cgct, tap = (idx / cgct) % (KH * KW), co = idx / (cgct * KH * KW);
+      const int ci = ci_base + c;
+      Ws[idx] = ci < g.c_in ? __ldg(W + ((long long)(co0 + co) * g.c_in + ci) * (KH * KW) + tap) : 0.f;
+    }
+    // A_out rows -> As[rb][co][p][q], zero outside [0,ho) x [0,wo)
+    for (int idx = tid; idx < g.RB * cc * tile; idx += blockDim.x) {
+      const int q = idx % g.PW + g.omin_x, p = (idx / g.PW) % g.PH + g.omin_y;
+      const int co = (idx / tile) % cc, r_ = idx / (tile * cc);
+      const long long m = m_base + r_;
+      float v = 0.f;
+      if (m < rows && p >= 0 && p < g.ho && q >= 0 && q < g.wo) {
+        const int r = (int)(m % R);
+        const long long tt = m / R;
+        const int b = (int)(tt % B), br = (int)(tt / B);
+        v = __ldg(A + br * sBr + b * sB + (long long)r * ld + ((long long)(co0 + co) * g.ho + p) * g.wo + q);
+      }
+      As[(r_ * g.COC + co) * tile + (idx % tile)] = v;
+    }
+    __syncthreads();
+    if (active) {
+      for (int co = 0; co < cc; ++co) {
+        const float* ap = As + (rb * g.COC + co) * tile;
+        const float* wp = Ws + co * (KH * KW) * cgct + cg * CT;
+#pragma unroll
+        for (int tap = 0; tap < KH * KW; ++tap) {
+          if (toff[tap] < 0) continue;
+          float a[4];
+#pragma unroll
+          for (int t = 0; t < 4; ++t) a[t] = ap[toff[tap] + u[t]];
+#pragma unroll
+          for (int c4 = 0; c4 < CT; c4 += 4) {
+            const float4 wv = *reinterpret_cast<const float4*>(wp + tap * cgct + c4);
+#pragma unroll
+            for (int t = 0; t < 4; ++t) {
+              acc[t][c4 + 0] = fmaf(a[t], wv.x, acc[t][c4 + 0]);
+              acc[t][c4 + 1] = fmaf(a[t], wv.y, acc[t][c4 + 1]);
+              acc[t][c4 + 2] = fmaf(a[t], wv.z, acc[t][c4 + 2]);
+              acc[t][c4 + 3] = fmaf(a[t], wv.w, acc[t][c4 + 3]);
+            }
+          }
+        }
+      }
+    }
+  }
+  const long long m = m_base + rb;
+  if (!active || m >= rows) return;
+#pragma unroll
+  for (int c = 0; c < CT; ++c) {
+    const int ci = ci_base + cg * CT + c;
+    if (ci >= g.c_in) continue;
+#pragma unroll
+    for (int t = 0; t < 4; ++t) {
+      if (!uv[t]) continue;
+      const long long o = ((m * g.c_in + ci) * g.h + y) * (long long)g.w + (cx + S * u[t]);
+      out[o] = addend ? acc[t][c] + addend[o] : acc[t][c];
+    }
+  }
+}
+
+template <int KH, int KW, int S, int CT>
+static bool launch_conv_bwd_tiled(const AView& A, const float* W, const float* addend, float* out, int B, int R,
+                                  int c_in, int h, int w, int c_out, int pad, int ho, int wo, cudaStream_t s) {
+  ConvBwdGeom g;
+  g.c_in = c_in; g.h = h; g.w = w; g.c_out = c_out; g.ho = ho; g.wo = wo; g.pad = pad;
+  g.NY = (h + S - 1) / S; g.NX = (w + S - 1) / S; g.XQ = (g.NX + 3) / 4;
+  g.PT = S * S * g.NY * g.XQ;
+  if (g.PT > 256) return false;
+  const int groups = (c_in + CT - 1) / CT;
+  g.CG = 256 / g.PT < groups ? 256 / g.PT : groups;
+  if (g.CG < 1) g.CG = 1;
+  g.RB = 256 / (g.PT * g.CG);
+  if (g.RB < 1) g.RB = 1;
+  if (g.RB > 4) g.RB = 4;
+  int omin_y = 0, omax_y = 0, omin_x = 0, omax_x = 0;
+  for (int c = 0; c < S; ++c) {
+    for (int i = 0; i < KH; ++i) { int n = c + pad - i; if (((n % S) + S) % S == 0) { omin_y = n / S < omin_y ? n / S : omin_y; omax_y = n / S > omax_y ? n / S : omax_y; } }
+    for (int j = 0; j < KW; ++j) { int n = c + pad - j; if (((n % S) + S) % S == 0) { omin_x = n / S < omin_x ? n / S : omin_x; omax_x = n / S > omax_x ? n / S : omax_x; } }
+  }
+  g.omin_y = omin_y; g.omin_x = omin_x;
+  g.PH = g.NY + omax_y - omin_y;
+  g.PW = g.NX + omax_x - omin_x;
+  const int cgct = g.CG * CT;
+  const size_t budget = 64 * 1024;
+  const size_t per_co = ((size_t)KH * KW * cgct + (size_t)g.RB * g.PH * g.PW) * sizeof(float);
+  int coc = (int)(budget / per_co);
+  if (coc < 1) return false;
+  if (coc > c_out) coc = c_out;
+  g.COC = coc;
+  const size_t smem = per_co * coc;
+  static bool attr = false;
+  if (!attr) {
+    if (cudaFuncSetAttribute(conv_bwd_tiled_kernel<KH, KW, S, CT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)budget) != cudaSuccess) return false;
+    attr = true;
+  }
+  const long long rows = 2LL * B * R;
+  dim3 grid((unsigned)((rows + g.RB - 1) / g.RB), (unsigned)((groups + g.CG - 1) / g.CG));
+  const int threads = ((g.PT * g.CG * g.RB + 31) / 32) * 32;
+  conv_bwd_tiled_kernel<KH, KW, S, CT><<<grid, threads, smem, s>>>(A.p, A.sBr, A.sB, A.ld, B, R, W, addend, out, g);
+  return true;
+}
+
+template <int KH, int KW, int S>
+static bool launch_conv_bwd_ct(const AView& A, const float* W, const float* addend, float* out, int B, int R,
+                               int c_in, int h, int w, int c_out, int pad, int ho, int wo, cudaStream_t s) {
+  if (c_in % 16 == 0) return launch_conv_bwd_tiled<KH, KW, S, 16>(A, W, addend, out, B, R, c_in, h, w, c_out, pad, ho, wo, s);
+  if (c_in > 4) return launch_conv_bwd_tiled<KH, KW, S, 8>(A, W, addend, out, B, R, c_in, h, w, c_out, pad, ho, wo, s);
+  return launch_conv_bwd_tiled<KH, KW, S, 4>(A, W, addend, out, B, R, c_in, h, w, c_out, pad, ho, wo, s);
+}
+
 void launch_conv_transpose(const AView& A, const float* W, const float* addend, float* out, int B, int R,
                            int c_in, int h, int w, int c_out, int kh, int kw, int stride, int pad, int ho,
                            int wo, cudaStream_t s) {
   long long rows = 2LL * B * R;
   if (rows <= 0) return;
+  if ((A.sB % 1 == 0) && rows < (1LL << 31)) {
+    bool done = false;
+    if (kh == 3 && kw == 3 && stride == 1) done = launch_conv_bwd_ct<3, 3, 1>(A, W, addend, out, B, R, c_in, h, w, c_out, pad, ho, wo, s);
+    else if (kh == 3 && kw == 3 && stride == 2) done = launch_conv_bwd_ct<3, 3, 2>(A, W, addend, out, B, R, c_in, h, w, c_out, pad, ho, wo, s);
+    else if (kh == 1 && kw == 1 && stride == 1) done = launch_conv_bwd_ct<1, 1, 1>(A, W, addend, out, B, R, c_in, h, w, c_out, pad, ho, wo, s);
+    else if (kh == 1 && kw == 1 && stride == 2) done = launch_conv_bwd_ct<1, 1, 2>(A, W, addend, out, B, R, c_in, h, w, c_out, pad, ho, wo, s);
+    if (done) return;
+  }
   int threads = 256;
   while (threads > 32 && threads / 2 >= h * w) threads /= 2;
   dim3 grid(ceil_div(h * w, threads), c_in, (unsigned)(rows < 32768 ? rows : 32768));
