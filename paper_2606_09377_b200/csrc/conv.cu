@@ -102,18 +102,31 @@ conv_transpose_kernel(const float* __restrict__ A, long long sBr, long long sB, 
   }
 }
 
-
 // ---- a6, fast path: register-tiled gather.  Block = RB rows x CG input-channel groups x PT pixel threads.
 // A thread owns 4 output pixels of ONE stride-parity class (same valid filter taps for all four, spaced XQ apart
 // in the class's x index so that a warp reads consecutive shared-memory words and writes consecutive outputs)
 // times CT input channels: 4*CT accumulators.  Per (co, tap): 4 LDS of A, CT/4 broadcast LDS.128 of W, 4*CT FFMA.
 // A_out of the block's rows is staged, zero-haloed, in shared memory COC output channels at a time together
-// with the filter slice transposed to [co][tap][ci] (ci fastest).
+// with the filter slice transposed to [co][tap][ci] (ci fastest).  Staging is asynchronous (cp.async, 4-byte
+// copies because the halo shifts alignment) and double-buffered: chunk c+1 is in flight while chunk c is
+// multiplied.  Each thread precomputes once which tile elements it copies (the tile geometry is the same for
+// every (row, co)), so the copy loop has no divisions.
 struct ConvBwdGeom {
   int c_in, h, w, c_out, ho, wo, pad;
   int NY, NX, XQ, PT, CG, RB, COC;      // per-class rows / cols / x-quads, thread split, co chunk
   int omin_y, omin_x, PH, PW;           // shared-memory tile origin and size
+  int stage_floats;                     // floats per pipeline stage (filters + A tiles)
 };
+
+constexpr int kConvFillMax = 6;         // tile elements per thread (tile <= 6 * blockDim)
+
+__device__ __forceinline__ void cp_async4(float* dst_smem, const float* src) {
+  const uint32_t d = static_cast<uint32_t>(__cvta_generic_to_shared(dst_smem));
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" :: "r"(d), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" :: "n"(N) : "memory"); }
 
 template <int KH, int KW, int S, int CT>
 __global__ void __launch_bounds__(256)
@@ -121,15 +134,17 @@ conv_bwd_tiled_kernel(const float* __restrict__ A, long long sBr, long long sB, 
                       const float* __restrict__ W, const float* __restrict__ addend, float* __restrict__ out,
                       ConvBwdGeom g) {
   extern __shared__ __align__(16) float smem_f[];
+  __shared__ const float* rowp[4];
+  constexpr int KK = KH * KW;
   const int cgct = g.CG * CT;
-  float* Ws = smem_f;                                  // [COC][KH*KW][cgct]
-  float* As = smem_f + g.COC * KH * KW * cgct;         // [RB][COC][PH][PW]
+  const int w_floats = g.COC * KK * cgct;              // stage layout: Ws [COC][KK][cgct], then As [RB][COC][PH][PW]
   const int tid = threadIdx.x;
   const int nthreads = g.PT * g.CG * g.RB;
   const int pt = tid % g.PT, cg = (tid / g.PT) % g.CG, rb = tid / (g.PT * g.CG);
   const long long rows = 2LL * B * R;
   const long long m_base = (long long)blockIdx.x * g.RB;
   const int ci_base = blockIdx.y * cgct;
+  const int tile = g.PH * g.PW;
   // pixel thread -> (parity class, yy, xq)
   const int per_class = g.NY * g.XQ;
   const int cls = pt / per_class, rem = pt % per_class;
@@ -137,8 +152,59 @@ conv_bwd_tiled_kernel(const float* __restrict__ A, long long sBr, long long sB, 
   const int yy = rem / g.XQ, xq = rem % g.XQ;
   const int y = cy + S * yy;
   const bool active = tid < nthreads;
+
+  if (tid < g.RB) {
+    const long long m = m_base + tid;
+    const float* ptr = nullptr;
+    if (m < rows) {
+      const int r = (int)(m % R);
+      const long long tt = m / R;
+      ptr = A + (tt / B) * sBr + (tt % B) * sB + (long long)r * ld;
+    }
+    rowp[tid] = ptr;
+  }
+  // zero both stages once: the halo (and rows past the end) stay zero, the copies only touch the interior
+  for (int i = tid; i < 2 * g.stage_floats; i += blockDim.x) smem_f[i] = 0.f;
+  // this thread's share of a tile: source offset inside one (row, co) map, or -1 for halo elements
+  int soff[kConvFillMax], doff[kConvFillMax];
+#pragma unroll
+  for (int k = 0; k < kConvFillMax; ++k) {
+    const int idx = tid + k * blockDim.x;
+    const int p = idx / g.PW + g.omin_y, q = idx % g.PW + g.omin_x;
+    const bool in = idx < tile && p >= 0 && p < g.ho && q >= 0 && q < g.wo;
+    soff[k] = in ? p * g.wo + q : -1;
+    doff[k] = idx;
+  }
+  __syncthreads();
+
+  auto fill = [&](int co0, int stage) {
+    float* Ws = smem_f + stage * g.stage_floats;
+    float* As = Ws + w_floats;
+    const int cc = min(g.COC, g.c_out - co0);
+    for (int idx = tid; idx < cc * KK * cgct; idx += blockDim.x) {
+      const int c = idx % cgct, t2 = idx / cgct;
+      const int tap = t2 % KK, co = t2 / KK;
+      const int ci = ci_base + c;
+      if (ci < g.c_in) cp_async4(Ws + idx, W + ((long long)(co0 + co) * g.c_in + ci) * KK + tap);
+    }
+    for (int r_ = 0; r_ < g.RB; ++r_) {
+      const float* base = rowp[r_];
+      if (base == nullptr) continue;
+      base += (long long)co0 * g.ho * g.wo;
+      float* dst = As + r_ * g.COC * tile;
+      for (int co = 0; co < cc; ++co) {
+#pragma unroll
+        for (int k = 0; k < kConvFillMax; ++k)
+          if (soff[k] >= 0) cp_async4(dst + doff[k], base + soff[k]);
+        base += g.ho * g.wo;
+        dst += tile;
+      }
+    }
+    cp_async_commit();
+  };
+
   // tap table (loop-invariant): offset inside the tile, or -1 when the tap does not hit this parity class
-  int toff[KH * KW];
+  int toff[KK];
 #pragma unroll
   for (int i = 0; i < KH; ++i)
 #pragma unroll
@@ -161,38 +227,22 @@ conv_bwd_tiled_kernel(const float* __restrict__ A, long long sBr, long long sB, 
 #pragma unroll
     for (int c = 0; c < CT; ++c) acc[t][c] = 0.f;
 
-  const int tile = g.PH * g.PW;
-  for (int co0 = 0; co0 < g.c_out; co0 += g.COC) {
-    const int cc = min(g.COC, g.c_out - co0);
-    __syncthreads();
-    // filter slice -> Ws[co][tap][ci]
-    for (int idx = tid; idx < cc * KH * KW * cgct; idx += blockDim.x) {
-      const int c = idx % cgct, tap = (idx / cgct) % (KH * KW), co = idx / (cgct * KH * KW);
-      const int ci = ci_base + c;
-      Ws[idx] = ci < g.c_in ? __ldg(W + ((long long)(co0 + co) * g.c_in + ci) * (KH * KW) + tap) : 0.f;
-    }
-    // A_out rows -> As[rb][co][p][q], zero outside [0,ho) x [0,wo)
-    for (int idx = tid; idx < g.RB * cc * tile; idx += blockDim.x) {
-      const int q = idx % g.PW + g.omin_x, p = (idx / g.PW) % g.PH + g.omin_y;
-      const int co = (idx / tile) % cc, r_ = idx / (tile * cc);
-      const long long m = m_base + r_;
-      float v = 0.f;
-      if (m < rows && p >= 0 && p < g.ho && q >= 0 && q < g.wo) {
-        const int r = (int)(m % R);
-        const long long tt = m / R;
-        const int b = (int)(tt % B), br = (int)(tt / B);
-        v = __ldg(A + br * sBr + b * sB + (long long)r * ld + ((long long)(co0 + co) * g.ho + p) * g.wo + q);
-      }
-      As[(r_ * g.COC + co) * tile + (idx % tile)] = v;
-    }
+  const int nchunks = (g.c_out + g.COC - 1) / g.COC;
+  fill(0, 0);
+  for (int ch = 0; ch < nchunks; ++ch) {
+    const int stage = ch & 1;
+    if (ch + 1 < nchunks) { fill((ch + 1) * g.COC, stage ^ 1); cp_async_wait<1>(); }
+    else cp_async_wait<0>();
     __syncthreads();
     if (active) {
-      for (int co = 0; co < cc; ++co) {
-        const float* ap = As + (rb * g.COC + co) * tile;
-        const float* wp = Ws + co * (KH * KW) * cgct + cg * CT;
+      const int cc = min(g.COC, g.c_out - ch * g.COC);
+      const float* Ws = smem_f + stage * g.stage_floats;
+      const float* ap = Ws + w_floats + rb * g.COC * tile;
+      const float* wp = Ws + cg * CT;
+      for (int co = 0; co < cc; ++co, ap += tile, wp += KK * cgct) {
 #pragma unroll
-        for (int tap = 0; tap < KH * KW; ++tap) {
-          if (toff[tap] < 0) continue;
+        for (int tap = 0; tap < KK; ++tap) {
+          if (S > 1 && toff[tap] < 0) continue;
           float a[4];
 #pragma unroll
           for (int t = 0; t < 4; ++t) a[t] = ap[toff[tap] + u[t]];
@@ -210,6 +260,7 @@ conv_bwd_tiled_kernel(const float* __restrict__ A, long long sBr, long long sB, 
         }
       }
     }
+    __syncthreads();      // the stage is refilled by the next iteration's fill
   }
   const long long m = m_base + rb;
   if (!active || m >= rows) return;
@@ -248,23 +299,26 @@ static bool launch_conv_bwd_tiled(const AView& A, const float* W, const float* a
   g.omin_y = omin_y; g.omin_x = omin_x;
   g.PH = g.NY + omax_y - omin_y;
   g.PW = g.NX + omax_x - omin_x;
+  const int threads = ((g.PT * g.CG * g.RB + 31) / 32) * 32;
+  if (g.PH * g.PW > kConvFillMax * threads) return false;
   const int cgct = g.CG * CT;
-  const size_t budget = 64 * 1024;
+  const size_t budget = 96 * 1024;                       // two stages; two blocks per SM still fit
   const size_t per_co = ((size_t)KH * KW * cgct + (size_t)g.RB * g.PH * g.PW) * sizeof(float);
-  int coc = (int)(budget / per_co);
+  int coc = (int)(budget / 2 / per_co);
   if (coc < 1) return false;
   if (coc > c_out) coc = c_out;
   g.COC = coc;
-  const size_t smem = per_co * coc;
+  g.stage_floats = (int)(per_co * coc / sizeof(float));
+  g.stage_floats = (g.stage_floats + 3) / 4 * 4;
+  const size_t smem = (size_t)2 * g.stage_floats * sizeof(float);
   static bool attr = false;
   if (!attr) {
     if (cudaFuncSetAttribute(conv_bwd_tiled_kernel<KH, KW, S, CT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)budget) != cudaSuccess) return false;
+                             (int)budget + 64) != cudaSuccess) return false;
     attr = true;
   }
   const long long rows = 2LL * B * R;
   dim3 grid((unsigned)((rows + g.RB - 1) / g.RB), (unsigned)((groups + g.CG - 1) / g.CG));
-  const int threads = ((g.PT * g.CG * g.RB + 31) / 32) * 32;
   conv_bwd_tiled_kernel<KH, KW, S, CT><<<grid, threads, smem, s>>>(A.p, A.sBr, A.sB, A.ld, B, R, W, addend, out, g);
   return true;
 }
