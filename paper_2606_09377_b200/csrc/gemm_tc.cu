@@ -8,11 +8,16 @@
 //     split once at crown_init); TMA (cp.async.bulk.tensor, 128B swizzle) stages 4 operand tiles per
 //     pipeline stage into shared memory; one elected thread issues tcgen05.mma.kind::tf32 (UMMA 128 x BN x 8)
 //     with the accumulator in TMEM;
-//   * warp roles: warp 0 TMA producer, warp 1 MMA issuer, warp 2 TMEM allocator, warps 4.. epilogue;
-//   * the accumulator is double-buffered in TMEM; K is cut into "drain chunks" of k_drain elements: each
-//     chunk is accumulated in TMEM, then added into an fp32 register running sum by the epilogue warps
-//     (round-to-nearest CUDA-core adds) while the tensor core works on the next chunk.  This bounds the
-//     length of any tensor-core accumulation chain, whose internal rounding is not round-to-nearest;
+//   * warp roles: warp 0 TMA producer, warp 1 MMA issuer, warp 2 TMEM allocator, warps 4-11 epilogue
+//     (two warps per TMEM lane quadrant, 64 columns each, one tcgen05.ld.32x32b.x64 per drain);
+//   * measured on B200: the tensor core's fp32 accumulation truncates, ~0.5 ulp of the running sum per MMA,
+//     so the error grows linearly with the length of an accumulation chain.  Two measures keep the result at
+//     CUDA-core FFMA accuracy: (1) two accumulators in TMEM, "big" for hi.hi and "small" for lo.hi + hi.lo
+//     (2^-11 of big), so big sees one MMA per k-step and small's truncation is 2^-11 smaller; (2) K is cut into
+//     drain chunks of k_drain elements (default 128 = 16 MMAs on big): each chunk of big is accumulated in
+//     TMEM, then added into an fp32 register running sum by the epilogue warps (round-to-nearest) while the
+//     tensor core fills the other buffer; small is drained every 16384 elements of K.  All four accumulators
+//     (big/small x double buffer) use the full 512 TMEM columns;
 //   * persistent grid (one CTA per SM), static tile order grouped along M for L2 reuse of W.
 #include <cuda.h>
 #include <cuda_runtime.h>
@@ -37,9 +42,10 @@ struct Cfg {
   static constexpr int A_BYTES = BM * BK * 4;
   static constexpr int B_BYTES = BN * BK * 4;
   static constexpr int STAGE_BYTES = 2 * A_BYTES + 2 * B_BYTES;
-  static constexpr int EPI_WARPS = BN / 32;          // 4 lane quadrants x (BN/128) column halves
+  static constexpr int EPI_WARPS = 8;                // 4 lane quadrants x 2 column halves of BN/2
+  static constexpr int EPI_COLS = BN / 2;            // columns drained by one epilogue warp
   static constexpr int THREADS = 128 + EPI_WARPS * 32;
-  static constexpr int TMEM_COLS = 2 * BN;           // double-buffered accumulator
+  static constexpr int TMEM_COLS = 4 * BN;           // {big, small} accumulators, each double-buffered
   static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align slack*/ + 256 /*barriers*/;
 };
 
@@ -134,6 +140,23 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
         "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
       : "r"(taddr) : "memory");
 }
+__device__ __forceinline__ void tmem_ld64(uint32_t taddr, uint32_t (&v)[64]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x64.b32 "
+      "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,"
+      "%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,"
+      "%32,%33,%34,%35,%36,%37,%38,%39,%40,%41,%42,%43,%44,%45,%46,%47,"
+      "%48,%49,%50,%51,%52,%53,%54,%55,%56,%57,%58,%59,%60,%61,%62,%63}, [%64];"
+      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+        "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+        "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+        "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31]),
+        "=r"(v[32]), "=r"(v[33]), "=r"(v[34]), "=r"(v[35]), "=r"(v[36]), "=r"(v[37]), "=r"(v[38]), "=r"(v[39]),
+        "=r"(v[40]), "=r"(v[41]), "=r"(v[42]), "=r"(v[43]), "=r"(v[44]), "=r"(v[45]), "=r"(v[46]), "=r"(v[47]),
+        "=r"(v[48]), "=r"(v[49]), "=r"(v[50]), "=r"(v[51]), "=r"(v[52]), "=r"(v[53]), "=r"(v[54]), "=r"(v[55]),
+        "=r"(v[56]), "=r"(v[57]), "=r"(v[58]), "=r"(v[59]), "=r"(v[60]), "=r"(v[61]), "=r"(v[62]), "=r"(v[63])
+      : "r"(taddr) : "memory");
+}
 __device__ __forceinline__ void tmem_ld_wait() {
   asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 }
@@ -168,18 +191,22 @@ template <int BN>
 __global__ void __launch_bounds__(Cfg<BN>::THREADS, 1)
 gemm_tf32x3_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant__ CUtensorMap tmA_lo,
                    const __grid_constant__ CUtensorMap tmB_hi, const __grid_constant__ CUtensorMap tmB_lo,
-                   float* __restrict__ D, long long ldd, int M, int N, int K, int kb_per_chunk) {
+                   float* __restrict__ D, long long ldd, int M, int N, int K, int kb_per_chunk,
+                   int chunks_per_small) {
   using C = Cfg<BN>;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t raw = smem_u32(smem_raw);
   const uint32_t base = (raw + 1023u) & ~1023u;
   const uint32_t bar_base = base + C::STAGES * C::STAGE_BYTES;
-  // barriers: full[STAGES], empty[STAGES], tmem_full[2], tmem_empty[2]; then the TMEM base address slot
+  // barriers: full[STAGES], empty[STAGES], bfull[2], bempty[2] (big accumulator), sfull[2], sempty[2] (small
+  // accumulator); then the TMEM base address slot
   auto full_bar = [&](int s) { return bar_base + 8u * s; };
   auto empty_bar = [&](int s) { return bar_base + 8u * (C::STAGES + s); };
-  auto tfull_bar = [&](int b) { return bar_base + 8u * (2 * C::STAGES + b); };
-  auto tempty_bar = [&](int b) { return bar_base + 8u * (2 * C::STAGES + 2 + b); };
-  const uint32_t tmem_slot = bar_base + 8u * (2 * C::STAGES + 4);
+  auto bfull_bar = [&](int b) { return bar_base + 8u * (2 * C::STAGES + b); };
+  auto bempty_bar = [&](int b) { return bar_base + 8u * (2 * C::STAGES + 2 + b); };
+  auto sfull_bar = [&](int b) { return bar_base + 8u * (2 * C::STAGES + 4 + b); };
+  auto sempty_bar = [&](int b) { return bar_base + 8u * (2 * C::STAGES + 6 + b); };
+  const uint32_t tmem_slot = bar_base + 8u * (2 * C::STAGES + 8);
   volatile uint32_t* tmem_slot_ptr =
       reinterpret_cast<volatile uint32_t*>(smem_raw + (tmem_slot - raw));
 
@@ -194,7 +221,10 @@ gemm_tf32x3_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_cons
   }
   if (warp == 1 && lane == 0) {
     for (int s = 0; s < C::STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-    for (int b = 0; b < 2; ++b) { mbar_init(tfull_bar(b), 1); mbar_init(tempty_bar(b), C::EPI_WARPS); }
+    for (int b = 0; b < 2; ++b) {
+      mbar_init(bfull_bar(b), 1); mbar_init(bempty_bar(b), C::EPI_WARPS);
+      mbar_init(sfull_bar(b), 1); mbar_init(sempty_bar(b), C::EPI_WARPS);
+    }
     fence_barrier_init();
   }
   if (warp == 2) {
@@ -205,6 +235,7 @@ gemm_tf32x3_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_cons
   __syncthreads();
   tcgen05_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
+  // TMEM columns: big[b] at b*BN, small[b] at 2*BN + b*BN
 
   if (warp == 0) {
     // ===================== TMA producer =====================
@@ -230,18 +261,25 @@ gemm_tf32x3_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_cons
     }
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
+    // Two accumulators of different magnitude: "big" takes hi.hi (one MMA per k-step, drained to the CUDA-core
+    // running sum every chunk), "small" takes lo.hi + hi.lo (2^-11 of big; drained every chunks_per_small chunks).
+    // The tensor core's fp32 accumulation truncates, ~0.5 ulp of the accumulator per MMA: keeping the two apart
+    // means big sees a third of the MMAs and small's truncation is 2^-11 smaller in absolute terms.
     if (lane == 0) {
       constexpr uint32_t idesc = make_idesc_tf32(BM, BN);
       int stage = 0; uint32_t parity = 0;
-      uint32_t acc_cnt = 0;
+      uint32_t big_cnt = 0, small_cnt = 0;
       for (int t = blockIdx.x; t < num_tiles; t += gridDim.x) {
+        uint32_t acc_small = 0;
         for (int c = 0; c < num_chunks; ++c) {
-          const uint32_t buf = acc_cnt & 1u;
-          mbar_wait(tempty_bar(buf), ((acc_cnt >> 1) & 1u) ^ 1u);
+          const uint32_t bbuf = big_cnt & 1u, sbuf = small_cnt & 1u;
+          mbar_wait(bempty_bar(bbuf), ((big_cnt >> 1) & 1u) ^ 1u);
+          if (acc_small == 0) mbar_wait(sempty_bar(sbuf), ((small_cnt >> 1) & 1u) ^ 1u);
           tcgen05_fence_after();
-          const uint32_t tmem_d = tmem_base + buf * BN;
+          const uint32_t tmem_big = tmem_base + bbuf * BN;
+          const uint32_t tmem_small = tmem_base + 2 * BN + sbuf * BN;
           const int kb_end = min(num_kb, (c + 1) * kb_per_chunk);
-          uint32_t accumulate = 0;
+          uint32_t acc_big = 0;
           for (int kb = c * kb_per_chunk; kb < kb_end; ++kb) {
             mbar_wait(full_bar(stage), parity);
             tcgen05_fence_after();
@@ -256,16 +294,20 @@ gemm_tf32x3_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_cons
               const uint64_t dA_lo = make_kmajor_sw128_desc(sA_lo + koff);
               const uint64_t dB_hi = make_kmajor_sw128_desc(sB_hi + koff);
               const uint64_t dB_lo = make_kmajor_sw128_desc(sB_lo + koff);
-              umma_tf32(tmem_d, dA_lo, dB_hi, idesc, accumulate);   // small terms first
-              umma_tf32(tmem_d, dA_hi, dB_lo, idesc, 1u);
-              umma_tf32(tmem_d, dA_hi, dB_hi, idesc, 1u);
-              accumulate = 1u;
+              umma_tf32(tmem_small, dA_lo, dB_hi, idesc, acc_small);
+              umma_tf32(tmem_small, dA_hi, dB_lo, idesc, 1u);
+              umma_tf32(tmem_big, dA_hi, dB_hi, idesc, acc_big);
+              acc_small = 1u; acc_big = 1u;
             }
             umma_commit(empty_bar(stage));   // frees the smem stage once these MMAs have read it
             if (++stage == C::STAGES) { stage = 0; parity ^= 1u; }
           }
-          umma_commit(tfull_bar(buf));       // accumulator chunk complete
-          ++acc_cnt;
+          umma_commit(bfull_bar(bbuf));      // big chunk complete
+          ++big_cnt;
+          if ((c + 1) % chunks_per_small == 0 || c == num_chunks - 1) {
+            umma_commit(sfull_bar(sbuf));    // small accumulator complete
+            ++small_cnt; acc_small = 0;
+          }
         }
       }
     }
@@ -273,37 +315,54 @@ gemm_tf32x3_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_cons
     // ===================== epilogue: TMEM -> fp32 running sum -> global =====================
     const int ew = warp - 4;
     const int quad = warp & 3;               // TMEM lane quadrant this warp may access
-    const int chalf = ew >> 2;               // which 128-column half (BN == 256)
-    uint32_t acc_cnt = 0;
+    const int chalf = ew >> 2;               // which half of the BN columns
+    constexpr int EC = C::EPI_COLS;
+    uint32_t big_cnt = 0, small_cnt = 0;
     for (int t = blockIdx.x; t < num_tiles; t += gridDim.x) {
       int mb, nb; tile_coords(t, m_tiles, n_tiles, mb, nb);
-      float acc[128];
+      float acc[EC];
 #pragma unroll
-      for (int i = 0; i < 128; ++i) acc[i] = 0.f;
+      for (int i = 0; i < EC; ++i) acc[i] = 0.f;
       for (int c = 0; c < num_chunks; ++c) {
-        const uint32_t buf = acc_cnt & 1u;
-        mbar_wait(tfull_bar(buf), (acc_cnt >> 1) & 1u);
-        tcgen05_fence_after();
-        const uint32_t taddr = tmem_base + ((uint32_t)(quad * 32) << 16) + buf * BN + chalf * 128;
-#pragma unroll
-        for (int g = 0; g < 4; ++g) {
-          uint32_t v[32];
-          tmem_ld32(taddr + g * 32, v);
+        {
+          const uint32_t buf = big_cnt & 1u;
+          mbar_wait(bfull_bar(buf), (big_cnt >> 1) & 1u);
+          tcgen05_fence_after();
+          const uint32_t taddr = tmem_base + ((uint32_t)(quad * 32) << 16) + buf * BN + chalf * EC;
+          static_assert(EC == 64, "epilogue drains 64 columns per warp");
+          uint32_t v[64];
+          tmem_ld64(taddr, v);
           tmem_ld_wait();
 #pragma unroll
-          for (int i = 0; i < 32; ++i) acc[g * 32 + i] += __uint_as_float(v[i]);
+          for (int i = 0; i < 64; ++i) acc[i] += __uint_as_float(v[i]);
+          tcgen05_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(bempty_bar(buf));
+          ++big_cnt;
         }
-        tcgen05_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(tempty_bar(buf));
-        ++acc_cnt;
+        if ((c + 1) % chunks_per_small == 0 || c == num_chunks - 1) {
+          const uint32_t buf = small_cnt & 1u;
+          mbar_wait(sfull_bar(buf), (small_cnt >> 1) & 1u);
+          tcgen05_fence_after();
+          const uint32_t taddr = tmem_base + ((uint32_t)(quad * 32) << 16) + 2 * BN + buf * BN + chalf * EC;
+          static_assert(EC == 64, "epilogue drains 64 columns per warp");
+          uint32_t v[64];
+          tmem_ld64(taddr, v);
+          tmem_ld_wait();
+#pragma unroll
+          for (int i = 0; i < 64; ++i) acc[i] += __uint_as_float(v[i]);
+          tcgen05_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(sempty_bar(buf));
+          ++small_cnt;
+        }
       }
       const int row = mb * BM + quad * 32 + lane;
-      const int col0 = nb * BN + chalf * 128;
+      const int col0 = nb * BN + chalf * EC;
       if (row < M) {
         float* drow = D + (long long)row * ldd + col0;
 #pragma unroll
-        for (int i = 0; i < 128; i += 4) {
+        for (int i = 0; i < EC; i += 4) {
           if (col0 + i + 3 < N) {
             *reinterpret_cast<float4*>(drow + i) = make_float4(acc[i], acc[i + 1], acc[i + 2], acc[i + 3]);
           } else {
@@ -377,10 +436,13 @@ static int launch_bn(const float* A_hi, const float* A_lo, const float* Wt_hi, c
   int m_tiles = (M + BM - 1) / BM, n_tiles = (N + BN - 1) / BN;
   long long tiles = (long long)m_tiles * n_tiles;
   int grid = (int)(tiles < num_sms ? tiles : num_sms);
-  if (k_drain <= 0) k_drain = 128;   // 48 MMAs per TMEM chain: accumulator truncation bias ~1e-6 rel
+  if (k_drain <= 0) k_drain = 128;   // 16 hi.hi MMAs per TMEM chain: truncation bias ~4e-7 rel
   int kb_per_chunk = (k_drain + BK - 1) / BK;
   if (kb_per_chunk < 1) kb_per_chunk = 1;
-  gemm_tf32x3_kernel<BN><<<grid, C::THREADS, C::SMEM_BYTES, s>>>(ta, tb, tc_, td, D, ldd, M, N, K, kb_per_chunk);
+  int chunks_per_small = 16384 / (kb_per_chunk * BK);   // small accumulator drained every 16384 elements of K
+  if (chunks_per_small < 1) chunks_per_small = 1;
+  gemm_tf32x3_kernel<BN><<<grid, C::THREADS, C::SMEM_BYTES, s>>>(ta, tb, tc_, td, D, ldd, M, N, K, kb_per_chunk,
+                                                                 chunks_per_small);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) { if (err) *err = cudaGetErrorString(e); return -1; }
   return 0;
