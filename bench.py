@@ -47,6 +47,8 @@ def parse_args():
     ap.add_argument("--scale", type=int, default=1, help="width divisor (debug only; 1 = the named config)")
     ap.add_argument("--batch", type=int, default=0, help="override B (debug only)")
     ap.add_argument("--mem-cap-gb", type=float, default=0.0)
+    ap.add_argument("--stream-weights", action="store_true",
+                    help="layers with >= 2^28 weights are streamed from pinned host memory (a7), not resident")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     return ap.parse_args()
@@ -203,7 +205,8 @@ def run_b200(args):
     cap = int(args.mem_cap_gb * (1 << 30))
     if cap == 0 and cfg in (3, 4):
         cap = 64 << 30
-    ctx = CrownContext(wl.net, B, S, device=f"cuda:{local}", mem_cap_bytes=cap)
+    ctx = CrownContext(wl.net, B, S, device=f"cuda:{local}", mem_cap_bytes=cap,
+                       stream_weights=int(args.stream_weights))
     inter = 1 if wl.intermediate == "ibp" else 0
 
     # ---- inputs resident in HBM -------------------------------------------------------------------
@@ -277,6 +280,7 @@ def run_b200(args):
     ms_step = timed(step_device, args.steps, max(args.warmup - 1, 0))
     clocks = clk.stop()
     flops_step = (ctx.gemm_flops() - f0) / (args.steps + max(args.warmup - 1, 0))
+    w_h2d_step = ctx.h2d_bytes() / (args.steps + max(args.warmup - 1, 0) + 1)
     verified = int(io["verified"].sum().item())      # of the last eps batch
     # end-to-end: host buffers in, host results out, wall clock around the blocking C-ABI call
     ms_e2e = timed(step_host, args.steps, max(args.warmup, 1), host_clock=True)
@@ -331,7 +335,8 @@ def run_b200(args):
             "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32 (3xTF32 products, fp32 accumulate)", "data": "synthetic",
             "config": dict(workload_desc(wl, args.workload), l2="flushed between timed steps (256 MB write)",
-                           mem_cap_bytes=cap),
+                           mem_cap_bytes=cap, stream_weights=bool(args.stream_weights),
+                           streamed_layers=len(ctx.streamed_ids), weight_h2d_bytes_per_step=w_h2d_step),
             "verified_last_batch": verified, "aw_tflops": aw_tflops, "aw_flops_per_step": flops_step,
             "peak_hbm_gb": {"workspace_high_water": peak_ws / 1e9, "torch_max_allocated": peak_torch / 1e9},
             "kernel_time_shares": shares,

@@ -58,19 +58,25 @@ typedef struct {
   int32_t in0, in1;           /* in1 only for CROWN_ADD, else -1                                */
   int32_t n_out, n_in;        /* LINEAR: sizes.  Other ops: filled by the library (may be 0)    */
   int32_t c_out, c_in, kh, kw, stride, pad, h_in, w_in; /* CONV2D                               */
-  const float* W_dev;         /* LINEAR [n_out,n_in]; CONV2D [c_out,c_in,kh,kw]; device memory  */
+  const float* W_dev;         /* LINEAR [n_out,n_in]; CONV2D [c_out,c_in,kh,kw]; device memory.
+                                 May be NULL for a LINEAR layer that is streamed (see W_host)     */
   const float* b_dev;         /* [n_out] / [c_out]; device memory                               */
-  const float* W_host;        /* optional pinned-host copy, used when opts.stream_weights != 0  */
+  const float* W_host;        /* optional PINNED host copy of W (caller-owned, must outlive the context).
+                                 With opts.stream_weights != 0 and n_in*n_out >= stream_min_elems
+                                 the layer is STREAMED: nothing of it stays resident; IBP copies raw
+                                 row slabs from here, the backward pass copies N-slabs of the
+                                 prepacked operand the library keeps in its own pinned host memory */
 } crown_node;
 
 typedef struct {
   uint64_t mem_cap_bytes;   /* cap on workspace use; 0 = no cap.  Start-spec rows are chunked so
                                that prepacked weights + live A buffers stay below it
                                (single-GPU restatement of Eq. 2)               */
-  int32_t stream_weights;   /* 1: GEMM weight operands of layers wider than stream_min_elems are
-                               not resident; they are prepacked into pinned host memory at init
-                               and copied H2D on a side stream per use, double-buffered ("gather
-                               before / free after")                               */
+  int32_t stream_weights;   /* 1: LINEAR layers with >= stream_min_elems weights and a W_host are not
+                               resident: their GEMM operand is prepacked into pinned host memory at
+                               init and copied H2D on a side stream per use through two staging
+                               buffers of <= 1 GiB in the workspace ("gather before / free after",
+                               PAPER.md:146); results are bitwise those of the resident mode      */
   int32_t mma_scheme;       /* 0 = 3xTF32 on tcgen05 tensor cores (fp32-accurate, never plain
                                TF32); 2 = fp32 FFMA on CUDA cores (debug / odd shapes)           */
   int32_t slope_rule;       /* fixed lower slope for unstable neurons when no alpha is given:
@@ -78,6 +84,7 @@ typedef struct {
   int32_t k_drain;          /* 3xTF32: accumulate at most this many K in TMEM before the fp32
                                CUDA-core running sum takes over (0 = library default)            */
   uint64_t stream_min_elems;/* see stream_weights (0 = library default 2^28 elements)            */
+  uint64_t stream_stage_bytes; /* size cap of each of the two staging buffers (0 = default 1 GiB) */
 } crown_opts;
 
 typedef struct crown_ctx crown_ctx;   /* opaque; owned by the library; freed by crown_destroy */
@@ -167,6 +174,7 @@ int crown_split_tf32(crown_ctx* ctx, const float* X_dev, int rows, int cols, int
 int crown_peak_bytes(crown_ctx* ctx, size_t* out);         /* high-water mark of workspace use   */
 int crown_launch_count(crown_ctx* ctx, uint64_t* out);      /* kernels launched so far            */
 int crown_gemm_flops(crown_ctx* ctx, double* out);          /* useful 2MNK flops of A.W so far    */
+int crown_h2d_bytes(crown_ctx* ctx, double* out);           /* weight bytes streamed H2D so far   */
 int crown_timing(crown_ctx* ctx, int enable);               /* 1: record CUDA events per kernel class */
 int crown_timing_read(crown_ctx* ctx, int kernel_class, double* ms_total, uint64_t* launches,
                       double* bytes_total, double* flops_total);

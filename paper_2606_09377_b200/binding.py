@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libcrownb200.so")
 OP_CODES = {"linear": 1, "conv": 2, "relu": 3, "add": 4, "flatten": 5}
 K_CLASSES = ["ibp", "coeff", "relax", "gemm_tc", "gemm_ffma", "concretize", "conv", "misc"]
 
-EXPORTS = ["crown_workspace_bytes", "crown_init", "ibp_forward", "crown_backward", "concretize", "crown_run",
+EXPORTS = ["crown_h2d_bytes", "crown_workspace_bytes", "crown_init", "ibp_forward", "crown_backward", "concretize", "crown_run",
            "crown_run_host", "crown_gemm", "crown_split_tf32", "crown_peak_bytes", "crown_launch_count",
            "crown_gemm_flops", "crown_timing", "crown_timing_read", "crown_last_error", "crown_destroy",
            "crown_version"]
@@ -33,7 +33,8 @@ class CrownNode(C.Structure):
 
 class CrownOpts(C.Structure):
     _fields_ = [("mem_cap_bytes", C.c_uint64), ("stream_weights", C.c_int32), ("mma_scheme", C.c_int32),
-                ("slope_rule", C.c_int32), ("k_drain", C.c_int32), ("stream_min_elems", C.c_uint64)]
+                ("slope_rule", C.c_int32), ("k_drain", C.c_int32), ("stream_min_elems", C.c_uint64),
+                ("stream_stage_bytes", C.c_uint64)]
 
 
 class CrownError(RuntimeError):
@@ -73,6 +74,7 @@ def load_library() -> C.CDLL:
     lib.crown_peak_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
     lib.crown_launch_count.argtypes = [vp, C.POINTER(C.c_uint64)]
     lib.crown_gemm_flops.argtypes = [vp, C.POINTER(C.c_double)]
+    lib.crown_h2d_bytes.argtypes = [vp, C.POINTER(C.c_double)]
     lib.crown_timing.argtypes = [vp, i32]
     lib.crown_timing_read.argtypes = [vp, i32, C.POINTER(C.c_double), C.POINTER(C.c_uint64),
                                       C.POINTER(C.c_double), C.POINTER(C.c_double)]
@@ -92,7 +94,8 @@ class CrownContext:
     in0, in1, W, b (numpy float32), stride, pad, shape (output shape)."""
 
     def __init__(self, net, B_max: int, S_max: int, device: str = "cuda:0", mem_cap_bytes: int = 0,
-                 mma_scheme: int = 0, slope_rule: int = 0, k_drain: int = 0, stream_weights: int = 0):
+                 mma_scheme: int = 0, slope_rule: int = 0, k_drain: int = 0, stream_weights: int = 0,
+                 stream_min_elems: int = 0, stream_stage_bytes: int = 0):
         if not torch.cuda.is_available():
             raise CrownError("no CUDA device: the crownb200 hot path has no CPU fallback")
         self.lib = load_library()
@@ -107,6 +110,7 @@ class CrownContext:
         self.relu_ids = [i for i, n in enumerate(net.nodes) if n.op == "relu"]
         self.B_max, self.S_max = int(B_max), int(S_max)
         self._keep: List[torch.Tensor] = []
+        self.streamed_ids: List[int] = []
         arr = (CrownNode * self.n_nodes)()
         for i, n in enumerate(net.nodes):
             cn = arr[i]
@@ -118,12 +122,23 @@ class CrownContext:
                 cn.c_out, cn.c_in, cn.kh, cn.kw = n.W.shape
                 cn.stride, cn.pad, cn.h_in, cn.w_in = n.stride, n.pad, src[1], src[2]
             if n.op in ("linear", "conv"):
-                Wd = torch.from_numpy(np.ascontiguousarray(n.W, dtype=np.float32)).to(self.device)
                 bd = torch.from_numpy(np.ascontiguousarray(n.b, dtype=np.float32)).to(self.device)
-                self._keep += [Wd, bd]
-                cn.W_dev, cn.b_dev = Wd.data_ptr(), bd.data_ptr()
+                self._keep.append(bd)
+                cn.b_dev = bd.data_ptr()
+                min_elems = stream_min_elems or (1 << 28)
+                if stream_weights and n.op == "linear" and n.W.size >= min_elems:
+                    # streamed layer: no resident copy, only a pinned host buffer the library copies from
+                    Wh = torch.from_numpy(np.ascontiguousarray(n.W, dtype=np.float32)).pin_memory()
+                    self._keep.append(Wh)
+                    cn.W_dev, cn.W_host = None, Wh.data_ptr()
+                    self.streamed_ids.append(i)
+                else:
+                    Wd = torch.from_numpy(np.ascontiguousarray(n.W, dtype=np.float32)).to(self.device)
+                    self._keep.append(Wd)
+                    cn.W_dev = Wd.data_ptr()
         self._nodes = arr
-        self.opts = CrownOpts(mem_cap_bytes, stream_weights, mma_scheme, slope_rule, k_drain, 0)
+        self.opts = CrownOpts(mem_cap_bytes, stream_weights, mma_scheme, slope_rule, k_drain, stream_min_elems,
+                              stream_stage_bytes)
         need = C.c_size_t(0)
         self._check(self.lib.crown_workspace_bytes(arr, self.n_nodes, *self.in_chw, self.B_max, self.S_max,
                                                    C.byref(self.opts), C.byref(need)), None)
@@ -308,6 +323,12 @@ class CrownContext:
     def gemm_flops(self) -> float:
         v = C.c_double(0)
         self._check(self.lib.crown_gemm_flops(self.h, C.byref(v)), self.h)
+        return v.value
+
+    def h2d_bytes(self) -> float:
+        """Bytes of weights streamed host->device so far (0 unless stream_weights)."""
+        v = C.c_double(0)
+        self._check(self.lib.crown_h2d_bytes(self.h, C.byref(v)), self.h)
         return v.value
 
     def timing(self, enable: bool) -> None:

@@ -48,12 +48,27 @@ extern "C" int crown_init(crown_ctx** out, const crown_node* nodes, int n_nodes,
   ctx->ws_bytes = workspace_bytes;
   uint8_t* cur = reinterpret_cast<uint8_t*>(align_up(reinterpret_cast<size_t>(ctx->ws)));
   for (auto& ni : ctx->nodes) {
-    if (wants_prepack(ni, ctx->opts)) {
+    ni.streamed = is_streamed(ni.n, ctx->opts);
+    if (ni.n.op == CROWN_LINEAR && !ni.streamed && !ni.n.W_dev) {
+      delete ctx; return CROWN_EINVAL;     // a layer without a resident copy must qualify for streaming
+    }
+    if (ni.streamed) {
+      if (ctx->opts.mma_scheme != 0 || !gemm_tc_supported(128, ni.n.n_in, ni.n.n_out)) { delete ctx; return CROWN_EUNSUPPORTED; }
+      ni.tc_ok = true;
+    } else if (wants_prepack(ni, ctx->opts)) {
       size_t sz = align_up((size_t)ni.n.n_in * ni.n.n_out * 4);
       ni.Wt_hi = reinterpret_cast<float*>(cur); cur += sz;
       ni.Wt_lo = reinterpret_cast<float*>(cur); cur += sz;
       ni.tc_ok = true;
     }
+  }
+  if (ctx->plan.stage_bytes) {
+    ctx->stage[0] = cur; cur += ctx->plan.stage_bytes;
+    ctx->stage[1] = cur; cur += ctx->plan.stage_bytes;
+    if (cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking) != cudaSuccess) { delete ctx; return CROWN_ECUDA; }
+    for (int b = 0; b < 2; ++b)
+      if (cudaEventCreateWithFlags(&ctx->ev_copied[b], cudaEventDisableTiming) != cudaSuccess ||
+          cudaEventCreateWithFlags(&ctx->ev_free[b], cudaEventDisableTiming) != cudaSuccess) { delete ctx; return CROWN_ECUDA; }
   }
   ctx->coef_base = cur; ctx->coef_off.assign(n_nodes, 0);
   { size_t off = 0; for (int i = 0; i < n_nodes; ++i) if (ctx->nodes[i].n.op == CROWN_RELU) { ctx->coef_off[i] = off; off += align_up((size_t)B_max * ctx->nodes[i].size * 16); } cur += ctx->plan.coef_bytes; }
@@ -66,9 +81,34 @@ extern "C" int crown_init(crown_ctx** out, const crown_node* nodes, int n_nodes,
   ctx->peak = (size_t)(ctx->pool_base - ctx->ws);
   // prepack: transpose + TF32 split of every GEMM weight operand (one pass over W)
   for (auto& ni : ctx->nodes) {
-    if (!ni.tc_ok) continue;
+    if (!ni.tc_ok || ni.streamed) continue;
     Scope sc(ctx, CROWN_K_MISC);
     launch_split_tf32(ni.n.W_dev, ni.n.n_out, ni.n.n_in, 1, ni.Wt_hi, ni.Wt_lo, ctx->stream);
+  }
+  // streamed layers: the same prepack, N-slab by N-slab through the staging buffers, into pinned host memory
+  for (auto& ni : ctx->nodes) {
+    if (!ni.streamed) continue;
+    const int K = ni.n.n_out, N = ni.n.n_in;
+    const size_t bytes = (size_t)N * K * 4;
+    if (cudaHostAlloc(reinterpret_cast<void**>(&ni.hWt_hi), bytes, cudaHostAllocDefault) != cudaSuccess ||
+        cudaHostAlloc(reinterpret_cast<void**>(&ni.hWt_lo), bytes, cudaHostAllocDefault) != cudaSuccess) {
+      crown_destroy(ctx); return CROWN_ENOMEM;
+    }
+    // stage[1] holds the raw column slab W[:, n0:n0+ns] as [K, ns]; stage[0] its transposed hi/lo parts [ns, K]
+    const int ns_max = slab_rows(ctx->plan.stage_bytes, N, K, 2);
+    for (int n0 = 0; n0 < N; n0 += ns_max) {
+      const int ns = std::min(ns_max, N - n0);
+      float* raw = reinterpret_cast<float*>(ctx->stage[1]);
+      float* hi = reinterpret_cast<float*>(ctx->stage[0]);
+      float* lo = hi + (size_t)ns * K;
+      cudaError_t e1 = cudaMemcpy2DAsync(raw, (size_t)ns * 4, ni.n.W_host + n0, (size_t)N * 4, (size_t)ns * 4, K,
+                                         cudaMemcpyHostToDevice, ctx->stream);
+      { Scope sc(ctx, CROWN_K_MISC); launch_split_tf32(raw, K, ns, 1, hi, lo, ctx->stream); }
+      cudaError_t e2 = cudaMemcpyAsync(ni.hWt_hi + (size_t)n0 * K, hi, (size_t)ns * K * 4, cudaMemcpyDeviceToHost, ctx->stream);
+      cudaError_t e3 = cudaMemcpyAsync(ni.hWt_lo + (size_t)n0 * K, lo, (size_t)ns * K * 4, cudaMemcpyDeviceToHost, ctx->stream);
+      cudaError_t e4 = cudaStreamSynchronize(ctx->stream);
+      if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess || e4 != cudaSuccess) { crown_destroy(ctx); return CROWN_ECUDA; }
+    }
   }
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) { std::string m = cudaGetErrorString(e); delete ctx; (void)m; return CROWN_ECUDA; }
@@ -80,6 +120,9 @@ extern "C" int crown_destroy(crown_ctx* ctx) {
   if (!ctx) return CROWN_EINVAL;
   for (auto& r : ctx->recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
   for (auto e : ctx->free_events) cudaEventDestroy(e);
+  for (auto& ni : ctx->nodes) { if (ni.hWt_hi) cudaFreeHost(ni.hWt_hi); if (ni.hWt_lo) cudaFreeHost(ni.hWt_lo); }
+  for (int b = 0; b < 2; ++b) { if (ctx->ev_copied[b]) cudaEventDestroy(ctx->ev_copied[b]); if (ctx->ev_free[b]) cudaEventDestroy(ctx->ev_free[b]); }
+  if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
   delete ctx;
   return CROWN_OK;
 }
@@ -88,6 +131,7 @@ extern "C" const char* crown_version(void) { return "crownb200 0.1 (sm_100a)"; }
 extern "C" int crown_peak_bytes(crown_ctx* ctx, size_t* out) { if (!ctx || !out) return CROWN_EINVAL; *out = ctx->peak; return CROWN_OK; }
 extern "C" int crown_launch_count(crown_ctx* ctx, uint64_t* out) { if (!ctx || !out) return CROWN_EINVAL; *out = ctx->launches; return CROWN_OK; }
 extern "C" int crown_gemm_flops(crown_ctx* ctx, double* out) { if (!ctx || !out) return CROWN_EINVAL; *out = ctx->gemm_flops; return CROWN_OK; }
+extern "C" int crown_h2d_bytes(crown_ctx* ctx, double* out) { if (!ctx || !out) return CROWN_EINVAL; *out = ctx->h2d_bytes; return CROWN_OK; }
 extern "C" int crown_timing(crown_ctx* ctx, int enable) {
   if (!ctx) return CROWN_EINVAL;
   for (auto& r : ctx->recs) { ctx->free_events.push_back(r.a); ctx->free_events.push_back(r.b); }
@@ -155,8 +199,28 @@ int ibp_internal(crown_ctx* ctx, int B, const float* x_lo, const float* x_hi, fl
     switch (nd.op) {
       case CROWN_LINEAR: {
         if (!input_of(nd.in0, li, ui, relu_in)) return fail(ctx, CROWN_EINVAL, "ibp: producer interval missing");
+        if (ni.streamed) {
+          // raw row slabs of W from pinned host memory, double-buffered on the side stream (a7)
+          const int rs_max = slab_rows(ctx->plan.stage_bytes, nd.n_out, nd.n_in, 1);
+          const int nslabs = (nd.n_out + rs_max - 1) / rs_max;
+          int rc2 = stream_slabs(ctx, nslabs,
+            [&](int sl, uint8_t* dst, cudaStream_t cs) {
+              const int r0 = sl * rs_max, rs = std::min(rs_max, nd.n_out - r0);
+              ctx->h2d_bytes += (double)rs * nd.n_in * 4;
+              return cudaMemcpyAsync(dst, nd.W_host + (size_t)r0 * nd.n_in, (size_t)rs * nd.n_in * 4, cudaMemcpyHostToDevice, cs);
+            },
+            [&](int sl, uint8_t* src) {
+              const int r0 = sl * rs_max, rs = std::min(rs_max, nd.n_out - r0);
+              Scope sc(ctx, CROWN_K_IBP, 4.0 * rs * nd.n_in * ((B + 7) / 8), 4.0 * B * rs * (double)nd.n_in);
+              launch_ibp_linear(reinterpret_cast<const float*>(src), nd.b_dev ? nd.b_dev + r0 : nullptr, li, ui, relu_in,
+                                lo + r0, uo + r0, B, rs, nd.n_in, nd.n_out, s);
+              return 0;
+            });
+          if (rc2) return rc2;
+          break;
+        }
         Scope sc(ctx, CROWN_K_IBP, 4.0 * nd.n_out * nd.n_in * ((B + 7) / 8), 4.0 * B * nd.n_out * (double)nd.n_in);
-        launch_ibp_linear(nd.W_dev, nd.b_dev, li, ui, relu_in, lo, uo, B, nd.n_out, nd.n_in, s);
+        launch_ibp_linear(nd.W_dev, nd.b_dev, li, ui, relu_in, lo, uo, B, nd.n_out, nd.n_in, nd.n_out, s);
         break; }
       case CROWN_CONV2D: {
         if (!input_of(nd.in0, li, ui, relu_in)) return fail(ctx, CROWN_EINVAL, "ibp: producer interval missing");

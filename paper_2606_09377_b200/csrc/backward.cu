@@ -79,8 +79,18 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
     if (sn.n.op != CROWN_LINEAR) return fail(ctx, CROWN_EUNSUPPORTED, "crown_backward: identity start needs a Linear node");
     if (row0 < 0 || row0 + R > sn.size) return fail(ctx, CROWN_EINVAL, "crown_backward: row range outside the start node");
     { Scope sc(ctx, CROWN_K_MISC); launch_init_d(ctx->d_buf, sn.n.b_dev, row0, B, R, s); }
-    Pending p; p.v.p = sn.n.W_dev + (long long)row0 * sn.n.n_in; p.v.ld = sn.n.n_in; p.v.n = sn.n.n_in;
-    p.v.sB = 0; p.v.sBr = 0;
+    Pending p; p.v.ld = sn.n.n_in; p.v.n = sn.n.n_in; p.v.sB = 0; p.v.sBr = 0;
+    if (sn.streamed) {   // no resident copy: fetch the R rows from the caller's pinned host buffer into an A buffer
+      float* rowsbuf = nullptr;
+      p.buf = new_buf(ps, rowsbuf);
+      if (p.buf < 0) return fail(ctx, CROWN_ENOMEM, "backward: A-buffer pool exhausted");
+      CK(ctx, cudaMemcpyAsync(rowsbuf, sn.n.W_host + (size_t)row0 * sn.n.n_in, (size_t)R * sn.n.n_in * 4,
+                              cudaMemcpyHostToDevice, s));
+      ctx->h2d_bytes += (double)R * sn.n.n_in * 4;
+      p.v.p = rowsbuf;
+    } else {
+      p.v.p = sn.n.W_dev + (long long)row0 * sn.n.n_in;
+    }
     ps.pend[sn.n.in0] = p;
     first = start - 1;
   }
@@ -103,7 +113,7 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
         const int j = nd.in0;
         const bool lin_below = j >= 0 && (ctx->nodes[j].n.op == CROWN_LINEAR || ctx->nodes[j].n.op == CROWN_CONV2D);
         // the product that follows runs on the tensor cores when the producer is a prepacked Linear
-        const bool tc = lin_below && ctx->nodes[j].tc_ok && gemm_tc_supported(2 * B * R, ctx->nodes[j].n.n_in, ctx->nodes[j].n.n_out);
+        const bool tc = lin_below && ctx->nodes[j].tc_ok && (ctx->nodes[j].streamed || gemm_tc_supported(2 * B * R, ctx->nodes[j].n.n_in, ctx->nodes[j].n.n_out));
         RelaxArgs ra;
         ra.A = cur.v; ra.coef = coef_ptr(ctx, i);
         ra.alpha_lo = alpha_lo ? alpha_lo[i] : nullptr;
@@ -129,7 +139,7 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
         const int M_full = 2 * B * R;
         Pending out;
         float* D = nullptr;
-        if (ni.tc_ok && gemm_tc_supported(M_full, nd.n_in, nd.n_out)) {
+        if (ni.tc_ok && (ni.streamed || gemm_tc_supported(M_full, nd.n_in, nd.n_out))) {
           const float *hi = cur.v.p, *lo = cur.v.lo;
           Pending tmp;
           if (!lo) {   // operand not split yet (start matrix, fork sum): split pass, also makes it contiguous
@@ -144,15 +154,42 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
           out.buf = new_buf(ps, D);
           if (out.buf < 0) return fail(ctx, CROWN_ENOMEM, "backward: A-buffer pool exhausted");
           const char* e = nullptr;
-          { Scope sc(ctx, CROWN_K_GEMM_TC, 4.0 * ((double)M_full * nd.n_out + (double)nd.n_out * nd.n_in + (double)M_full * nd.n_in),
+          if (ni.streamed) {
+            // N-slabs of the prepacked operand Wt [n_in, n_out] from pinned host memory (a7); slab s+1 (or the
+            // next layer's first slab) is copied on the side stream while slab s is multiplied
+            const int K = nd.n_out, N = nd.n_in;
+            const int ns_max = slab_rows(ctx->plan.stage_bytes, N, K, 2);
+            const int nslabs = (N + ns_max - 1) / ns_max;
+            int rc2 = stream_slabs(ctx, nslabs,
+              [&](int sl, uint8_t* dst, cudaStream_t cs) {
+                const int n0 = sl * ns_max, ns = std::min(ns_max, N - n0);
+                float* dhi = reinterpret_cast<float*>(dst);
+                ctx->h2d_bytes += 2.0 * ns * K * 4;
+                cudaError_t e1 = cudaMemcpyAsync(dhi, ni.hWt_hi + (size_t)n0 * K, (size_t)ns * K * 4, cudaMemcpyHostToDevice, cs);
+                if (e1 != cudaSuccess) return e1;
+                return cudaMemcpyAsync(dhi + (size_t)ns * K, ni.hWt_lo + (size_t)n0 * K, (size_t)ns * K * 4, cudaMemcpyHostToDevice, cs);
+              },
+              [&](int sl, uint8_t* src) {
+                const int n0 = sl * ns_max, ns = std::min(ns_max, N - n0);
+                const float* whi = reinterpret_cast<const float*>(src);
+                Scope sc(ctx, CROWN_K_GEMM_TC, 4.0 * ((double)M_full * K + (double)K * ns + (double)M_full * ns), 2.0 * M_full * (double)ns * K);
+                if (launch_gemm_tc(hi, lo, whi, whi + (size_t)ns * K, D + n0, N, M_full, ns, K, ctx->opts.k_drain, ctx->num_sms, s, &e))
+                  return fail(ctx, CROWN_ECUDA, std::string("gemm_tc: ") + (e ? e : "?"));
+                return (int)CROWN_OK;
+              });
+            if (rc2) return rc2;
+          } else {
+            Scope sc(ctx, CROWN_K_GEMM_TC, 4.0 * ((double)M_full * nd.n_out + (double)nd.n_out * nd.n_in + (double)M_full * nd.n_in),
                      2.0 * M_full * (double)nd.n_in * nd.n_out);
             if (launch_gemm_tc(hi, lo, ni.Wt_hi, ni.Wt_lo, D, nd.n_in, M_full, nd.n_in, nd.n_out, ctx->opts.k_drain, ctx->num_sms, s, &e))
-              return fail(ctx, CROWN_ECUDA, std::string("gemm_tc: ") + (e ? e : "?")); }
+              return fail(ctx, CROWN_ECUDA, std::string("gemm_tc: ") + (e ? e : "?"));
+          }
           ctx->gemm_flops += 2.0 * M_full * (double)nd.n_in * nd.n_out;
           out.v = canon_view(D, B, R, nd.n_in);
         } else {
           // CUDA-core contraction; rows shared between branches / properties are multiplied once
           int m_eff = 0;
+          if (ni.streamed) return fail(ctx, CROWN_EUNSUPPORTED, "backward: a streamed layer needs M = 2*B*rows >= 128 (tensor-core path)");
           if (!view_uniform(cur.v, B, R, m_eff)) return fail(ctx, CROWN_EINVAL, "backward: non-uniform A view");
           out.buf = new_buf(ps, D);
           if (out.buf < 0) return fail(ctx, CROWN_ENOMEM, "backward: A-buffer pool exhausted");

@@ -24,11 +24,18 @@ struct NodeInfo {
   float* Wt_hi = nullptr;  // prepacked GEMM operand [n_in, n_out] (device)
   float* Wt_lo = nullptr;
   bool tc_ok = false;
+  // a7: weight streaming ("gather before / free after").  A streamed layer has no resident copy:
+  // raw W lives in the caller's pinned host buffer (n.W_host), the prepacked GEMM operand in pinned host memory
+  // owned by the library; both are copied H2D slab by slab through two staging buffers on a side stream.
+  bool streamed = false;
+  float* hWt_hi = nullptr;  // pinned host [n_in, n_out]
+  float* hWt_lo = nullptr;
 };
 
 struct Plan {
   size_t prepack_bytes = 0, coef_bytes = 0, ibp_bytes = 0, d_bytes = 0, io_bytes = 0;
   size_t buf_bytes = 0;
+  size_t stage_bytes = 0; // one of the two weight-streaming staging buffers (0: nothing is streamed)
   int nbuf = 0;
   int rc = 0;             // row chunk for identity passes
   int rows_cap = 0;       // max(rc, S_max)
@@ -64,6 +71,12 @@ struct crown_ctx {
   bool timing = false;
   std::vector<TimingRec> recs;
   std::vector<cudaEvent_t> free_events;
+  // weight streaming
+  cudaStream_t copy_stream = nullptr;
+  uint8_t* stage[2] = {nullptr, nullptr};
+  cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr};
+  uint64_t slab_seq = 0;      // slabs issued so far (parity = staging buffer)
+  double h2d_bytes = 0;
 };
 
 namespace {
@@ -100,7 +113,7 @@ int analyse(const crown_node* nodes, int n_nodes, int in_c, int in_h, int in_w,
     long long in_size = (long long)c * h * w;
     switch (n.op) {
       case CROWN_LINEAR:
-        if (n.n_out <= 0 || n.n_in != in_size || !n.W_dev) { err = "LINEAR: n_in does not match producer or W missing"; return CROWN_EINVAL; }
+        if (n.n_out <= 0 || n.n_in != in_size || (!n.W_dev && !n.W_host)) { err = "LINEAR: n_in does not match producer or W missing"; return CROWN_EINVAL; }
         ni.c = n.n_out; ni.h = 1; ni.w = 1;
         break;
       case CROWN_CONV2D: {
@@ -132,6 +145,22 @@ int analyse(const crown_node* nodes, int n_nodes, int in_c, int in_h, int in_w,
   return CROWN_OK;
 }
 
+bool is_streamed(const crown_node& n, const crown_opts& o) {
+  if (n.op != CROWN_LINEAR || !o.stream_weights || !n.W_host) return false;
+  const uint64_t min_elems = o.stream_min_elems ? o.stream_min_elems : (1ull << 28);
+  return (uint64_t)n.n_in * (uint64_t)n.n_out >= min_elems;
+}
+
+constexpr size_t kStageBytesMax = (size_t)1 << 30;   // 1 GiB per staging buffer
+
+// rows of a [rows_total, row_elems] fp32 matrix (x limbs) that fit one staging buffer, multiple of 128
+int slab_rows(size_t stage_bytes, int rows_total, int row_elems, int limbs) {
+  size_t r = stage_bytes / ((size_t)limbs * row_elems * 4);
+  if (r >= (size_t)rows_total) return rows_total;
+  r = r / 128 * 128;
+  return (int)(r < 128 ? 128 : r);
+}
+
 bool wants_prepack(const NodeInfo& ni, const crown_opts& o) {
   if (ni.n.op != CROWN_LINEAR || o.mma_scheme != 0) return false;
   // as GEMM operand: K = n_out, N = n_in; M is decided per pass
@@ -145,7 +174,12 @@ int make_plan(const std::vector<NodeInfo>& nodes, int n0, int B, int S, const cr
   for (const auto& ni : nodes) {
     nmax = std::max(nmax, ni.size);
     if (ni.n.op == CROWN_LINEAR && ni.n.in0 >= 0) max_start = std::max(max_start, ni.size);
-    if (wants_prepack(ni, o)) p.prepack_bytes += 2 * align_up((size_t)ni.n.n_in * ni.n.n_out * 4);
+    if (is_streamed(ni.n, o)) {
+      // staging must hold 128 rows of the prepacked operand (2 limbs x n_out) and 128 raw rows (n_in)
+      size_t need = std::max((size_t)2 * 128 * ni.n.n_out * 4, (size_t)128 * ni.n.n_in * 4);
+      size_t full = (size_t)2 * ni.n.n_in * ni.n.n_out * 4;
+      p.stage_bytes = std::max(p.stage_bytes, std::max(need, std::min(full, o.stream_stage_bytes ? (size_t)o.stream_stage_bytes : kStageBytesMax)));
+    } else if (wants_prepack(ni, o)) p.prepack_bytes += 2 * align_up((size_t)ni.n.n_in * ni.n.n_out * 4);
     if (ni.n.op == CROWN_RELU) p.coef_bytes += align_up((size_t)B * ni.size * 16);
     p.ibp_bytes += 2 * align_up((size_t)B * ni.size * 4);
     if (ni.n.op == CROWN_RELU) p.io_bytes += align_up((size_t)B * S * ni.size * 4) + 2 * align_up((size_t)B * ni.size * 4);
@@ -154,7 +188,8 @@ int make_plan(const std::vector<NodeInfo>& nodes, int n0, int B, int S, const cr
                 2 * align_up((size_t)B * S * 4) + align_up((size_t)B);
   p.nbuf = has_add ? 8 : 3;
   size_t per_row = (size_t)2 * B * nmax * 4;            // bytes of one start-spec row in one buffer
-  size_t fixed = p.prepack_bytes + p.coef_bytes + p.ibp_bytes + p.io_bytes;
+  p.stage_bytes = align_up(p.stage_bytes);
+  size_t fixed = p.prepack_bytes + p.coef_bytes + p.ibp_bytes + p.io_bytes + 2 * p.stage_bytes;
   int rc = max_start;
   if (o.mem_cap_bytes) {
     size_t d_est = align_up((size_t)2 * B * std::max(max_start, S) * 4);
@@ -191,6 +226,33 @@ struct Scope {
     }
   }
 };
+
+// ---- a7: weight streaming through the two staging buffers ------------------------------------------
+// copy(slab, dst, copy_stream) enqueues the H2D copies of one slab; use(slab, src) launches the kernels that
+// read it on the main stream.  Slab s+1 is copied while slab s is consumed ("gather before / free after",
+// PAPER.md:146); because every call is only an enqueue, the copy of the NEXT layer's first slab also starts
+// as soon as a staging buffer is free, i.e. while the current layer still computes.
+template <class Copy, class Use>
+int stream_slabs(crown_ctx* ctx, int nslabs, Copy copy, Use use) {
+  auto issue = [&](int s) -> int {
+    const int buf = (int)((ctx->slab_seq + s) & 1);
+    CK(ctx, cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_free[buf], 0));
+    CK(ctx, copy(s, ctx->stage[buf], ctx->copy_stream));
+    CK(ctx, cudaEventRecord(ctx->ev_copied[buf], ctx->copy_stream));
+    return CROWN_OK;
+  };
+  int rc = issue(0);
+  if (rc) return rc;
+  for (int s = 0; s < nslabs; ++s) {
+    const int buf = (int)((ctx->slab_seq + s) & 1);
+    if (s + 1 < nslabs && (rc = issue(s + 1))) return rc;
+    CK(ctx, cudaStreamWaitEvent(ctx->stream, ctx->ev_copied[buf], 0));
+    if ((rc = use(s, ctx->stage[buf]))) return rc;
+    CK(ctx, cudaEventRecord(ctx->ev_free[buf], ctx->stream));
+  }
+  ctx->slab_seq += nslabs;
+  return CROWN_OK;
+}
 
 // ---- A-buffer pool ----------------------------------------------------------------------------
 int pool_get(crown_ctx* ctx) {

@@ -451,9 +451,9 @@ static int launch_bn(const float* A_hi, const float* A_lo, const float* Wt_hi, c
 }  // namespace tc
 
 int gemm_tc_supported(int M, int N, int K) {
-  // TMA needs 16-byte row pitches (K % 4) and the epilogue stores float4 (N % 4); tiles smaller than one
-  // 128 x 128 block are left to the CUDA-core kernel.
-  return M >= 128 && N >= 128 && K >= 32 && (K % 4 == 0) && (N % 4 == 0);
+  // TMA needs 16-byte row pitches (K % 4) and the epilogue stores float4 (N % 4).  M below one tile is fine (TMA
+  // zero-fills the missing rows) and still beats the CUDA-core kernel; N < 128 or K < 32 is left to that kernel.
+  return M >= 1 && N >= 128 && K >= 32 && (K % 4 == 0) && (N % 4 == 0);
 }
 
 int launch_gemm_tc(const float* A_hi, const float* A_lo, const float* Wt_hi, const float* Wt_lo, float* D,

@@ -18,7 +18,7 @@ template <int BT, int RW>
 __global__ void __launch_bounds__(kIbpWarps * 32, 2)
 ibp_linear_kernel(const float* __restrict__ W, const float* __restrict__ bias,
                   const float* __restrict__ l_in, const float* __restrict__ u_in, int relu_in,
-                  float* __restrict__ l_out, float* __restrict__ u_out, int B, int n_out, int n_in) {
+                  float* __restrict__ l_out, float* __restrict__ u_out, int B, int n_out, int n_in, int ldo) {
   __shared__ __align__(16) float sc[BT][kIbpKC];
   __shared__ __align__(16) float sr[BT][kIbpKC];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -98,28 +98,28 @@ ibp_linear_kernel(const float* __restrict__ W, const float* __restrict__ bias,
       float r = warp_sum(accR[i][b]);
       if (lane == 0 && row < n_out && b0 + b < B) {
         c += bias ? bias[row] : 0.f;
-        l_out[(long long)(b0 + b) * n_out + row] = c - r;
-        u_out[(long long)(b0 + b) * n_out + row] = c + r;
+        l_out[(long long)(b0 + b) * ldo + row] = c - r;
+        u_out[(long long)(b0 + b) * ldo + row] = c + r;
       }
     }
   }
 }
 
 void launch_ibp_linear(const float* W, const float* bias, const float* l_in, const float* u_in,
-                       int relu_in, float* l_out, float* u_out, int B, int n_out, int n_in,
+                       int relu_in, float* l_out, float* u_out, int B, int n_out, int n_in, int ldo,
                        cudaStream_t s) {
   if (B <= 0 || n_out <= 0) return;
   constexpr int RW = 4;
   dim3 block(kIbpWarps * 32);
   int gx = ceil_div(n_out, kIbpWarps * RW);
   if (B <= 1) {
-    ibp_linear_kernel<1, RW><<<dim3(gx, 1), block, 0, s>>>(W, bias, l_in, u_in, relu_in, l_out, u_out, B, n_out, n_in);
+    ibp_linear_kernel<1, RW><<<dim3(gx, 1), block, 0, s>>>(W, bias, l_in, u_in, relu_in, l_out, u_out, B, n_out, n_in, ldo);
   } else if (B <= 2) {
-    ibp_linear_kernel<2, RW><<<dim3(gx, 1), block, 0, s>>>(W, bias, l_in, u_in, relu_in, l_out, u_out, B, n_out, n_in);
+    ibp_linear_kernel<2, RW><<<dim3(gx, 1), block, 0, s>>>(W, bias, l_in, u_in, relu_in, l_out, u_out, B, n_out, n_in, ldo);
   } else if (B <= 4) {
-    ibp_linear_kernel<4, RW><<<dim3(gx, 1), block, 0, s>>>(W, bias, l_in, u_in, relu_in, l_out, u_out, B, n_out, n_in);
+    ibp_linear_kernel<4, RW><<<dim3(gx, 1), block, 0, s>>>(W, bias, l_in, u_in, relu_in, l_out, u_out, B, n_out, n_in, ldo);
   } else {
-    ibp_linear_kernel<8, RW><<<dim3(gx, ceil_div(B, 8)), block, 0, s>>>(W, bias, l_in, u_in, relu_in, l_out, u_out, B, n_out, n_in);
+    ibp_linear_kernel<8, RW><<<dim3(gx, ceil_div(B, 8)), block, 0, s>>>(W, bias, l_in, u_in, relu_in, l_out, u_out, B, n_out, n_in, ldo);
   }
 }
 

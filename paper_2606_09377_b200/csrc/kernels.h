@@ -44,8 +44,9 @@ void launch_concretize(const AView& A, const float* d, const float* x_lo, const 
 
 // a1 -- IBP through a Linear layer in centre/radius form:
 // c' = W c + b, r' = |W| r; l' = c' - r', u' = c' + r'.  relu_in: clamp the input interval at 0 first.
+// ldo: row pitch of l_out/u_out (= n_out, or the full layer width when W is a streamed row slab).
 void launch_ibp_linear(const float* W, const float* bias, const float* l_in, const float* u_in,
-                       int relu_in, float* l_out, float* u_out, int B, int n_out, int n_in,
+                       int relu_in, float* l_out, float* u_out, int B, int n_out, int n_in, int ldo,
                        cudaStream_t s);
 
 // IBP through ReLU / Add (elementwise).

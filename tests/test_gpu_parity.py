@@ -151,3 +151,22 @@ def test_cfg4_scaled():
 def test_cfg5_scaled():
     wl = W.make(5, scale=4, B=2)
     _check_workload(wl)
+
+
+def test_streamed_weights_equal_resident_bitwise():
+    """a7: layer-wise weight streaming from pinned host memory (PAPER.md:146 hook points) must not change a bit
+    (the paper's FSDP argument)."""
+    import torch
+    wl3 = W.make(3, scale=16, B=2)    # 256-1024-1024-1024-10: tensor-core GEMMs on the streamed layers
+    lo, hi = wl3.box()
+    r_res = _ctx(wl3.net, wl3.B, wl3.S).run(lo, hi, wl3.C, None, "crown")
+    # all hidden layers streamed; a 1 MiB staging cap forces several slabs per layer (W2: 8 MiB prepacked)
+    for stage in (0, 1 << 20):
+        c2 = _ctx(wl3.net, wl3.B, wl3.S, stream_weights=1, stream_min_elems=1 << 18, stream_stage_bytes=stage)
+        assert len(c2.streamed_ids) == 3
+        r_str = c2.run(lo, hi, wl3.C, None, "crown")
+        assert c2.h2d_bytes() > 0
+        for k in ("lb", "ub"):
+            assert torch.equal(r_res[k], r_str[k]), k
+        for i in r_res["pre"]:
+            assert torch.equal(r_res["pre"][i][0], r_str["pre"][i][0]) and torch.equal(r_res["pre"][i][1], r_str["pre"][i][1])
