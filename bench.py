@@ -185,7 +185,7 @@ class ClockSampler:
 def run_b200(args):
     import torch
     import torch.distributed as dist
-    from paper_2606_09377_b200 import CrownContext
+    from paper_2606_09377_b200 import CrownContext, multi
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -266,10 +266,7 @@ def run_b200(args):
                 b.synchronize()
                 ms.append(a.elapsed_time(b))
         barrier()
-        tot = torch.tensor([sum(ms)], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(tot, op=dist.ReduceOp.MAX)
-        return float(tot.item()) / steps
+        return multi.max_over_ranks(sum(ms)) / steps       # the job is as slow as its slowest replica
 
     clk = ClockSampler(local)
     l0 = ctx.launch_count()
