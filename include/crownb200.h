@@ -85,6 +85,11 @@ typedef struct {
                                CUDA-core running sum takes over (0 = library default)            */
   uint64_t stream_min_elems;/* see stream_weights (0 = library default 2^28 elements)            */
   uint64_t stream_stage_bytes; /* size cap of each of the two staging buffers (0 = default 1 GiB) */
+  int32_t enable_fusion;    /* 1: where it applies (resident or streamed Linear below a ReLU, fixed-rule slopes)
+                               run a4 + a5 as ONE kernel (gemm_fused.cu): relaxation, bias accumulation and
+                               TF32 split happen in shared memory between TMA and the MMAs, Abar is never
+                               materialised.  0 (default): relax kernel + contraction kernel, which measured
+                               faster on B200 for every BASELINE config                  */
 } crown_opts;
 
 typedef struct crown_ctx crown_ctx;   /* opaque; owned by the library; freed by crown_destroy */
@@ -161,7 +166,8 @@ int crown_run_host(crown_ctx* ctx, int B, const float* x_lo_host, const float* x
                    float* lb_host, float* ub_host, uint8_t* verified_host);
 
 /* D[M,N] = A[M,K] . W[K,N] (row-major fp32) through the same contraction kernel the backward
- * pass uses (scheme: 0 = 3xTF32 tcgen05, 2 = FFMA); exposed for parity tests and roofline
+ * pass uses (scheme: 0 = 3xTF32 tcgen05 on prepared limbs, 1 = the fused kernel in split-only mode: A_hi_dev is
+ * the raw fp32 A and is split inside the kernel, 2 = FFMA); exposed for parity tests and roofline
  * measurement of kernel 1.  Wt_hi/Wt_lo [N,K] and A_hi/A_lo [M,K] are produced by
  * crown_split_tf32 (transpose=1 for W). */
 int crown_gemm(crown_ctx* ctx, int scheme, int M, int N, int K,

@@ -71,7 +71,7 @@ extern "C" int crown_init(crown_ctx** out, const crown_node* nodes, int n_nodes,
           cudaEventCreateWithFlags(&ctx->ev_free[b], cudaEventDisableTiming) != cudaSuccess) { delete ctx; return CROWN_ECUDA; }
   }
   ctx->coef_base = cur; ctx->coef_off.assign(n_nodes, 0);
-  { size_t off = 0; for (int i = 0; i < n_nodes; ++i) if (ctx->nodes[i].n.op == CROWN_RELU) { ctx->coef_off[i] = off; off += align_up((size_t)B_max * ctx->nodes[i].size * 16); } cur += ctx->plan.coef_bytes; }
+  { size_t off = 0; for (int i = 0; i < n_nodes; ++i) if (ctx->nodes[i].n.op == CROWN_RELU) { ctx->coef_off[i] = off; off += align_up((size_t)B_max * ctx->nodes[i].size * 32); } cur += ctx->plan.coef_bytes; }
   ctx->ibp_base = cur; ctx->ibp_off.assign(n_nodes, 0);
   { size_t off = 0; for (int i = 0; i < n_nodes; ++i) { ctx->ibp_off[i] = off; off += 2 * align_up((size_t)B_max * ctx->nodes[i].size * 4); } cur += ctx->plan.ibp_bytes; }
   ctx->d_buf = reinterpret_cast<float*>(cur); cur += ctx->plan.d_bytes;

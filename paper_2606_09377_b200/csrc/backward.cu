@@ -54,6 +54,8 @@ int contribute(Pass& ps, int idx, Pending p) {
 
 
 float4* coef_ptr(crown_ctx* ctx, int i) { return reinterpret_cast<float4*>(ctx->coef_base + ctx->coef_off[i]); }
+long long plane_stride(crown_ctx* ctx, int i) { return (long long)ctx->B_max * ctx->nodes[i].size; }
+float* planes_ptr(crown_ctx* ctx, int i) { return reinterpret_cast<float*>(coef_ptr(ctx, i) + plane_stride(ctx, i)); }
 
 // One backward pass.  coef_ready: per node, 1 if coef_ptr(i) already holds the coefficients of ReLU i for the
 // bounds in l_dev/u_dev (crown_run computes each ReLU's coefficients once); may be nullptr.
@@ -107,13 +109,63 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
         if (!l_dev || !u_dev || !l_dev[i] || !u_dev[i]) return fail(ctx, CROWN_EINVAL, "crown_backward: bounds of a ReLU below start are missing");
         if (!coef_ready || !(*coef_ready)[i]) {
           Scope sc(ctx, CROWN_K_COEFF, 24.0 * B * ni.size);
-          launch_relax_coeffs(l_dev[i], u_dev[i], coef_ptr(ctx, i), (long long)B * ni.size, ctx->opts.slope_rule, s);
+          launch_relax_coeffs(l_dev[i], u_dev[i], coef_ptr(ctx, i), planes_ptr(ctx, i), plane_stride(ctx, i), (long long)B * ni.size,
+                              ctx->opts.slope_rule, s);
           if (coef_ready) (*coef_ready)[i] = 1;
         }
         const int j = nd.in0;
         const bool lin_below = j >= 0 && (ctx->nodes[j].n.op == CROWN_LINEAR || ctx->nodes[j].n.op == CROWN_CONV2D);
         // the product that follows runs on the tensor cores when the producer is a prepacked Linear
         const bool tc = lin_below && ctx->nodes[j].tc_ok && (ctx->nodes[j].streamed || gemm_tc_supported(2 * B * R, ctx->nodes[j].n.n_in, ctx->nodes[j].n.n_out));
+        // fused path: relaxation + bias accumulation + split + contraction in one kernel (gemm_fused.cu); needs a
+        // resident prepacked Linear below with this ReLU as its only consumer and fixed-rule slopes (no alpha)
+        if (tc && ctx->opts.enable_fusion && ctx->nodes[j].n.op == CROWN_LINEAR &&
+            ctx->nodes[j].n_consumers == 1 && ps.pend.find(j) == ps.pend.end() &&
+            !(alpha_lo && alpha_lo[i]) && !(alpha_up && alpha_up[i]) &&
+            gemm_fused_supported(cur.v, B, R, ctx->nodes[j].n.n_in, ctx->nodes[j].n.n_out)) {
+          const NodeInfo& nj = ctx->nodes[j];
+          const int Kf = nj.n.n_out, Nf = nj.n.n_in;
+          const int M_full = 2 * B * R;
+          Pending outp;
+          float* D = nullptr;
+          outp.buf = new_buf(ps, D);
+          if (outp.buf < 0) return fail(ctx, CROWN_ENOMEM, "backward: A-buffer pool exhausted");
+          const char* e = nullptr;
+          if (nj.streamed) {
+            // N-slabs of the prepacked operand from pinned host memory (a7); d is accumulated by the first slab only
+            const int ns_max = slab_rows(ctx->plan.stage_bytes, Nf, Kf, 2);
+            const int nslabs = (Nf + ns_max - 1) / ns_max;
+            int rc2 = stream_slabs(ctx, nslabs,
+              [&](int sl, uint8_t* dst, cudaStream_t cs) {
+                const int n0 = sl * ns_max, ns = std::min(ns_max, Nf - n0);
+                float* dhi = reinterpret_cast<float*>(dst);
+                ctx->h2d_bytes += 2.0 * ns * Kf * 4;
+                cudaError_t e1 = cudaMemcpyAsync(dhi, nj.hWt_hi + (size_t)n0 * Kf, (size_t)ns * Kf * 4, cudaMemcpyHostToDevice, cs);
+                if (e1 != cudaSuccess) return e1;
+                return cudaMemcpyAsync(dhi + (size_t)ns * Kf, nj.hWt_lo + (size_t)n0 * Kf, (size_t)ns * Kf * 4, cudaMemcpyHostToDevice, cs);
+              },
+              [&](int sl, uint8_t* src) {
+                const int n0 = sl * ns_max, ns = std::min(ns_max, Nf - n0);
+                const float* whi = reinterpret_cast<const float*>(src);
+                Scope sc(ctx, CROWN_K_GEMM_TC, 4.0 * ((double)M_full * Kf + 2.0 * Kf * ns + (double)M_full * ns), 2.0 * M_full * (double)ns * Kf);
+                if (launch_gemm_fused(cur.v, B, R, planes_ptr(ctx, i), plane_stride(ctx, i), nj.n.b_dev, sl == 0 ? ctx->d_buf : nullptr, whi,
+                                      whi + (size_t)ns * Kf, D + n0, Nf, ns, Kf, ctx->opts.k_drain, ctx->num_sms, s, &e))
+                  return fail(ctx, CROWN_ECUDA, std::string("gemm_fused: ") + (e ? e : "?"));
+                return (int)CROWN_OK;
+              });
+            if (rc2) return rc2;
+          } else {
+            Scope sc(ctx, CROWN_K_GEMM_TC, 4.0 * ((double)M_full * Kf + 2.0 * Kf * Nf + (double)M_full * Nf), 2.0 * M_full * (double)Nf * Kf);
+            if (launch_gemm_fused(cur.v, B, R, planes_ptr(ctx, i), plane_stride(ctx, i), nj.n.b_dev, ctx->d_buf, nj.Wt_hi, nj.Wt_lo, D, Nf, Nf, Kf,
+                                  ctx->opts.k_drain, ctx->num_sms, s, &e))
+              return fail(ctx, CROWN_ECUDA, std::string("gemm_fused: ") + (e ? e : "?"));
+          }
+          ctx->gemm_flops += 2.0 * M_full * (double)Nf * Kf;
+          outp.v = canon_view(D, B, R, Nf);
+          release(ctx, cur);
+          rc = contribute(ps, nj.n.in0, outp);
+          break;
+        }
         RelaxArgs ra;
         ra.A = cur.v; ra.coef = coef_ptr(ctx, i);
         ra.alpha_lo = alpha_lo ? alpha_lo[i] : nullptr;
@@ -396,6 +448,15 @@ extern "C" int crown_gemm(crown_ctx* ctx, int scheme, int M, int N, int K, const
     const char* e = nullptr;
     Scope sc(ctx, CROWN_K_GEMM_TC, 4.0 * ((double)M * K + (double)K * N + (double)M * N), 2.0 * M * (double)N * K);
     if (launch_gemm_tc(A_hi_dev, A_lo_dev, Wt_hi_dev, Wt_lo_dev, D_dev, N, M, N, K, ctx->opts.k_drain, ctx->num_sms, ctx->stream, &e))
+      return fail(ctx, CROWN_EINVAL, std::string("crown_gemm: ") + (e ? e : "?"));
+  } else if (scheme == 1) {
+    // fused kernel in split-only mode: A_hi_dev is the RAW fp32 A [M,K]; the TF32 split happens inside the kernel
+    const char* e = nullptr;
+    AView v = canon_view(A_hi_dev, 1, M / 2, K);
+    if (M % 2) return fail(ctx, CROWN_EINVAL, "crown_gemm: scheme 1 needs an even M");
+    Scope sc(ctx, CROWN_K_GEMM_TC, 4.0 * ((double)M * K + 2.0 * K * N + (double)M * N), 2.0 * M * (double)N * K);
+    if (launch_gemm_fused(v, 1, M / 2, nullptr, 0, nullptr, nullptr, Wt_hi_dev, Wt_lo_dev, D_dev, N, N, K, ctx->opts.k_drain,
+                          ctx->num_sms, ctx->stream, &e))
       return fail(ctx, CROWN_EINVAL, std::string("crown_gemm: ") + (e ? e : "?"));
   } else if (scheme == 2) {
     // FFMA path takes W [K,N] row-major in Wt_hi_dev (NOT transposed) and fp32 A in A_hi_dev

@@ -180,7 +180,7 @@ int make_plan(const std::vector<NodeInfo>& nodes, int n0, int B, int S, const cr
       size_t full = (size_t)2 * ni.n.n_in * ni.n.n_out * 4;
       p.stage_bytes = std::max(p.stage_bytes, std::max(need, std::min(full, o.stream_stage_bytes ? (size_t)o.stream_stage_bytes : kStageBytesMax)));
     } else if (wants_prepack(ni, o)) p.prepack_bytes += 2 * align_up((size_t)ni.n.n_in * ni.n.n_out * 4);
-    if (ni.n.op == CROWN_RELU) p.coef_bytes += align_up((size_t)B * ni.size * 16);
+    if (ni.n.op == CROWN_RELU) p.coef_bytes += align_up((size_t)B * ni.size * 32);   // float4 records + 3 SoA planes
     p.ibp_bytes += 2 * align_up((size_t)B * ni.size * 4);
     if (ni.n.op == CROWN_RELU) p.io_bytes += align_up((size_t)B * S * ni.size * 4) + 2 * align_up((size_t)B * ni.size * 4);
   }

@@ -11,7 +11,8 @@ namespace crownb200 {
 // (reading G3); adaptive rule lambda = 1 iff u > -l (reading G4).
 // ------------------------------------------------------------------------------------------------
 __global__ void relax_coeffs_kernel(const float* __restrict__ l, const float* __restrict__ u,
-                                    float4* __restrict__ coef, long long count, int rule) {
+                                    float4* __restrict__ coef, float* __restrict__ planes, long long plane_stride,
+                                    long long count, int rule) {
   long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= count) return;
   float lo = l[i], hi = u[i];
@@ -28,13 +29,17 @@ __global__ void relax_coeffs_kernel(const float* __restrict__ l, const float* __
     c = make_float4(dU, bU, dL, 1.f);
   }
   coef[i] = c;
+  // the same coefficients as planes {dU, bU, dL} for 128-bit loads along the neuron axis (gemm_fused.cu)
+  planes[i] = c.x;
+  planes[plane_stride + i] = c.y;
+  planes[2 * plane_stride + i] = c.z;
 }
 
-void launch_relax_coeffs(const float* l, const float* u, float4* coef, long long count, int rule,
-                         cudaStream_t s) {
+void launch_relax_coeffs(const float* l, const float* u, float4* coef, float* planes, long long plane_stride,
+                         long long count, int rule, cudaStream_t s) {
   if (count <= 0) return;
   int threads = 256;
-  relax_coeffs_kernel<<<ceil_div(count, threads), threads, 0, s>>>(l, u, coef, count, rule);
+  relax_coeffs_kernel<<<ceil_div(count, threads), threads, 0, s>>>(l, u, coef, planes, plane_stride, count, rule);
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -26,15 +26,12 @@
 
 #include "common.cuh"
 #include "kernels.h"
+#include "tc_common.cuh"
 
 namespace crownb200 {
 
 namespace tc {
 
-constexpr int BM = 128;
-constexpr int BK = 32;               // 32 fp32 = 128 B = one swizzle row
-constexpr int UMMA_K = 8;            // kind::tf32: 32 bytes of K per instruction
-constexpr int GROUP_M = 8;           // m-blocks per raster group
 
 template <int BN>
 struct Cfg {
@@ -46,158 +43,22 @@ struct Cfg {
   static constexpr int EPI_COLS = BN / 2;            // columns drained by one epilogue warp
   static constexpr int THREADS = 128 + EPI_WARPS * 32;
   static constexpr int TMEM_COLS = 4 * BN;           // {big, small} accumulators, each double-buffered
-  static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align slack*/ + 256 /*barriers*/;
+  static constexpr int EPI_STAGE_BYTES = EPI_WARPS * 4096;   // one 32 x 32 fp32 slab per epilogue warp (TMA store)
+  static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + EPI_STAGE_BYTES + 1024 /*align slack*/ + 256 /*barriers*/;
 };
-
-// ---------------------------------------------------------------- PTX wrappers
-__device__ __forceinline__ uint32_t smem_u32(const void* p) {
-  return static_cast<uint32_t>(__cvta_generic_to_shared(p));
-}
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(bar), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(bar) : "memory");
-}
-__device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
-  uint32_t ok;
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-      "selp.u32 %0, 1, 0, p;\n\t}"
-      : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
-  return ok != 0;
-}
-__device__ __forceinline__ uint64_t globaltimer_ns() {
-  uint64_t t;
-  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-  return t;
-}
-// Bounded wait: a protocol bug must trap, not hang the GPU.
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  if (mbar_try_wait(bar, parity)) return;
-  uint64_t t0 = globaltimer_ns();
-  uint32_t spins = 0;
-  while (!mbar_try_wait(bar, parity)) {
-    if ((++spins & 1023u) == 0 && globaltimer_ns() - t0 > 4000000000ull) {
-      printf("crownb200 gemm_tc: mbarrier wait timed out (block %d thread %d bar %u parity %u)\n",
-             blockIdx.x, threadIdx.x, bar, parity);
-      __trap();
-    }
-  }
-}
-__device__ __forceinline__ void fence_barrier_init() {
-  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-}
-__device__ __forceinline__ void fence_proxy_async() {
-  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-}
-__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int x, int y, uint32_t bar) {
-  asm volatile(
-      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
-      :: "r"(dst), "l"(map), "r"(x), "r"(y), "r"(bar) : "memory");
-}
-__device__ __forceinline__ void prefetch_tmap(const CUtensorMap* map) {
-  asm volatile("prefetch.tensormap [%0];" :: "l"(map) : "memory");
-}
-__device__ __forceinline__ void tcgen05_fence_after() {
-  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-}
-__device__ __forceinline__ void tcgen05_fence_before() {
-  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-}
-__device__ __forceinline__ void tmem_alloc(uint32_t dst_smem, uint32_t ncols) {
-  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(dst_smem), "r"(ncols) : "memory");
-}
-__device__ __forceinline__ void tmem_relinquish() {
-  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-}
-__device__ __forceinline__ void tmem_dealloc(uint32_t addr, uint32_t ncols) {
-  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(addr), "r"(ncols) : "memory");
-}
-__device__ __forceinline__ void umma_tf32(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t idesc,
-                                          uint32_t accumulate) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "setp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
-      :: "r"(tmem_d), "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(accumulate) : "memory");
-}
-__device__ __forceinline__ void umma_commit(uint32_t bar) {
-  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(bar) : "memory");
-}
-__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
-  asm volatile(
-      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
-      "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,"
-      "%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
-      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-        "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
-        "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
-        "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
-      : "r"(taddr) : "memory");
-}
-__device__ __forceinline__ void tmem_ld64(uint32_t taddr, uint32_t (&v)[64]) {
-  asm volatile(
-      "tcgen05.ld.sync.aligned.32x32b.x64.b32 "
-      "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,"
-      "%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,"
-      "%32,%33,%34,%35,%36,%37,%38,%39,%40,%41,%42,%43,%44,%45,%46,%47,"
-      "%48,%49,%50,%51,%52,%53,%54,%55,%56,%57,%58,%59,%60,%61,%62,%63}, [%64];"
-      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-        "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
-        "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
-        "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31]),
-        "=r"(v[32]), "=r"(v[33]), "=r"(v[34]), "=r"(v[35]), "=r"(v[36]), "=r"(v[37]), "=r"(v[38]), "=r"(v[39]),
-        "=r"(v[40]), "=r"(v[41]), "=r"(v[42]), "=r"(v[43]), "=r"(v[44]), "=r"(v[45]), "=r"(v[46]), "=r"(v[47]),
-        "=r"(v[48]), "=r"(v[49]), "=r"(v[50]), "=r"(v[51]), "=r"(v[52]), "=r"(v[53]), "=r"(v[54]), "=r"(v[55]),
-        "=r"(v[56]), "=r"(v[57]), "=r"(v[58]), "=r"(v[59]), "=r"(v[60]), "=r"(v[61]), "=r"(v[62]), "=r"(v[63])
-      : "r"(taddr) : "memory");
-}
-__device__ __forceinline__ void tmem_ld_wait() {
-  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-}
-
-// Shared-memory matrix descriptor, K-major operand tile with 128-byte swizzle (rows of 128 B, 8-row groups
-// 1024 B apart): start address (>>4) | SBO = 1024 B (>>4) at bit 32 | version 1 at bit 46 | SWIZZLE_128B (2) at bit 61.
-__device__ __forceinline__ uint64_t make_kmajor_sw128_desc(uint32_t smem_addr) {
-  uint64_t d = 0;
-  d |= (uint64_t)((smem_addr & 0x3FFFFu) >> 4);
-  d |= (uint64_t)(1024u >> 4) << 32;
-  d |= (uint64_t)1 << 46;
-  d |= (uint64_t)2 << 61;
-  return d;
-}
-// Instruction descriptor for kind::tf32, fp32 accumulate, both operands K-major, M = 128, N = BN.
-__host__ __device__ constexpr uint32_t make_idesc_tf32(int m, int n) {
-  return (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(m >> 4) << 24);
-}
-
-__device__ __forceinline__ void tile_coords(int t, int m_tiles, int n_tiles, int& mb, int& nb) {
-  // groups of GROUP_M m-blocks sweep all n-blocks: concurrently running CTAs share W tiles in L2
-  int per_group = GROUP_M * n_tiles;
-  int g = t / per_group;
-  int first_m = g * GROUP_M;
-  int gm = min(GROUP_M, m_tiles - first_m);
-  int in_g = t - g * per_group;
-  mb = first_m + in_g % gm;
-  nb = in_g / gm;
-}
 
 template <int BN>
 __global__ void __launch_bounds__(Cfg<BN>::THREADS, 1)
 gemm_tf32x3_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant__ CUtensorMap tmA_lo,
                    const __grid_constant__ CUtensorMap tmB_hi, const __grid_constant__ CUtensorMap tmB_lo,
-                   float* __restrict__ D, long long ldd, int M, int N, int K, int kb_per_chunk,
+                   const __grid_constant__ CUtensorMap tmD, int M, int N, int K, int kb_per_chunk,
                    int chunks_per_small) {
   using C = Cfg<BN>;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t raw = smem_u32(smem_raw);
   const uint32_t base = (raw + 1023u) & ~1023u;
-  const uint32_t bar_base = base + C::STAGES * C::STAGE_BYTES;
+  const uint32_t epi_base = base + C::STAGES * C::STAGE_BYTES;           // 1024-aligned: swizzled store slabs
+  const uint32_t bar_base = epi_base + C::EPI_STAGE_BYTES;
   // barriers: full[STAGES], empty[STAGES], bfull[2], bempty[2] (big accumulator), sfull[2], sempty[2] (small
   // accumulator); then the TMEM base address slot
   auto full_bar = [&](int s) { return bar_base + 8u * s; };
@@ -357,22 +218,29 @@ gemm_tf32x3_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_cons
           ++small_cnt;
         }
       }
-      const int row = mb * BM + quad * 32 + lane;
-      const int col0 = nb * BN + chalf * EC;
-      if (row < M) {
-        float* drow = D + (long long)row * ldd + col0;
+      // tile -> global through shared memory and the TMA: lane = row writes its 32 columns (128 B) of a slab in the
+      // 128B-swizzled layout (conflict-free), one lane issues the bulk tensor store, which also clips the M / N edges
+      const uint32_t slab = epi_base + (uint32_t)ew * 4096u + (uint32_t)lane * 128u;
+      const uint32_t sw = (uint32_t)(lane & 7);
 #pragma unroll
-        for (int i = 0; i < EC; i += 4) {
-          if (col0 + i + 3 < N) {
-            *reinterpret_cast<float4*>(drow + i) = make_float4(acc[i], acc[i + 1], acc[i + 2], acc[i + 3]);
-          } else {
+      for (int sl = 0; sl < EC / 32; ++sl) {
+        if (lane == 0) bulk_wait_read0();          // the previous store has finished reading this warp's slab
+        __syncwarp();
 #pragma unroll
-            for (int e = 0; e < 4; ++e)
-              if (col0 + i + e < N) drow[i + e] = acc[i + e];
-          }
+        for (int c = 0; c < 8; ++c) {
+          const int i = sl * 32 + c * 4;
+          asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};"
+                       :: "r"(slab + (((uint32_t)c ^ sw) << 4)), "f"(acc[i]), "f"(acc[i + 1]), "f"(acc[i + 2]), "f"(acc[i + 3]) : "memory");
+        }
+        fence_proxy_async();
+        __syncwarp();
+        if (lane == 0) {
+          tma_store_2d(&tmD, epi_base + (uint32_t)ew * 4096u, nb * BN + chalf * EC + sl * 32, mb * BM + quad * 32);
+          bulk_commit();
         }
       }
     }
+    if (lane == 0) bulk_wait0();
   }
 
   tcgen05_fence_before();
@@ -384,45 +252,14 @@ gemm_tf32x3_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_cons
 }
 
 // ---------------------------------------------------------------- host side
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
-                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
-                                  CUtensorMapFloatOOBfill);
-
-static EncodeTiledFn get_encode_fn() {
-  static EncodeTiledFn fn = nullptr;
-  if (fn) return fn;
-  void* p = nullptr;
-  cudaDriverEntryPointQueryResult q;
-  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
-      q != cudaDriverEntryPointSuccess)
-    return nullptr;
-  fn = reinterpret_cast<EncodeTiledFn>(p);
-  return fn;
-}
-
-// [rows, K] fp32 row-major, box = 32 (K) x box_rows, 128B swizzle, zero fill out of bounds.
-static bool make_tmap(CUtensorMap* m, const float* ptr, int rows, int K, int box_rows) {
-  EncodeTiledFn fn = get_encode_fn();
-  if (!fn) return false;
-  cuuint64_t dims[2] = {(cuuint64_t)K, (cuuint64_t)rows};
-  cuuint64_t strides[1] = {(cuuint64_t)K * 4};
-  cuuint32_t box[2] = {(cuuint32_t)BK, (cuuint32_t)box_rows};
-  cuuint32_t estr[2] = {1, 1};
-  CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(ptr), dims, strides, box, estr,
-                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
-                  CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  return r == CUDA_SUCCESS;
-}
-
 template <int BN>
 static int launch_bn(const float* A_hi, const float* A_lo, const float* Wt_hi, const float* Wt_lo, float* D,
                      long long ldd, int M, int N, int K, int k_drain, int num_sms, cudaStream_t s,
                      const char** err) {
   using C = Cfg<BN>;
-  CUtensorMap ta, tb, tc_, td;
+  CUtensorMap ta, tb, tc_, td, tout;
   if (!make_tmap(&ta, A_hi, M, K, BM) || !make_tmap(&tb, A_lo, M, K, BM) ||
-      !make_tmap(&tc_, Wt_hi, N, K, BN) || !make_tmap(&td, Wt_lo, N, K, BN)) {
+      !make_tmap(&tc_, Wt_hi, N, K, BN) || !make_tmap(&td, Wt_lo, N, K, BN) || !make_tmap_out(&tout, D, M, N, ldd)) {
     if (err) *err = "cuTensorMapEncodeTiled failed";
     return -1;
   }
@@ -441,7 +278,7 @@ static int launch_bn(const float* A_hi, const float* A_lo, const float* Wt_hi, c
   if (kb_per_chunk < 1) kb_per_chunk = 1;
   int chunks_per_small = 16384 / (kb_per_chunk * BK);   // small accumulator drained every 16384 elements of K
   if (chunks_per_small < 1) chunks_per_small = 1;
-  gemm_tf32x3_kernel<BN><<<grid, C::THREADS, C::SMEM_BYTES, s>>>(ta, tb, tc_, td, D, ldd, M, N, K, kb_per_chunk,
+  gemm_tf32x3_kernel<BN><<<grid, C::THREADS, C::SMEM_BYTES, s>>>(ta, tb, tc_, td, tout, M, N, K, kb_per_chunk,
                                                                  chunks_per_small);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) { if (err) *err = cudaGetErrorString(e); return -1; }

@@ -17,9 +17,10 @@ struct AView {
 };
 
 // a3 -- relaxation coefficients of a ReLU from its pre-activation bounds.
-// coef[b*n+j] = {dU, bU, dL_fixed, unstable?1:0}.  rule: 0 adaptive, 1 zero, 2 one.
-void launch_relax_coeffs(const float* l, const float* u, float4* coef, long long count, int rule,
-                         cudaStream_t s);
+// coef[b*n+j] = {dU, bU, dL_fixed, unstable?1:0}; planes[p*plane_stride + b*n+j], p = 0 dU, 1 bU, 2 dL (the same
+// values as planes, for 128-bit loads along the neuron axis).  rule: 0 adaptive, 1 zero, 2 one.
+void launch_relax_coeffs(const float* l, const float* u, float4* coef, float* planes, long long plane_stride,
+                         long long count, int rule, cudaStream_t s);
 
 // a4 -- fused relaxation of A through a ReLU, both branches, with the bias
 // accumulation of the ReLU (bU through the sign-selected part of A) and of the linear layer below
@@ -80,6 +81,16 @@ int gemm_tc_supported(int M, int N, int K);
 int launch_gemm_tc(const float* A_hi, const float* A_lo, const float* Wt_hi, const float* Wt_lo,
                    float* D, long long ldd, int M, int N, int K, int k_drain, int num_sms,
                    cudaStream_t s, const char** err);
+
+// a4 + a5 fused -- relaxation of A through a ReLU (planes != nullptr; fixed-rule slopes only), d += A-/+ . bU,
+// d += Abar . bias, TF32 split and the 3xTF32 contraction with the prepacked operand in one kernel
+// (gemm_fused.cu).  A is a raw fp32 view ([2,B,R,K], strides multiples of K); D [2*B*R, N] with row pitch ldd
+// (an N-slab of a wider output when the operand is streamed; pass d = nullptr for all slabs but the first).
+int gemm_fused_supported(const AView& A, int B, int R, int N, int K);
+int launch_gemm_fused(const AView& A, int B, int R, const float* planes, long long plane_stride, const float* bias,
+                      float* d,
+                      const float* Wt_hi, const float* Wt_lo, float* D, long long ldd, int N, int K, int k_drain,
+                      int num_sms, cudaStream_t s, const char** err);
 
 // a2 / a6 -- Conv2d IBP (centre/radius) and conv-transpose backward of A.
 void launch_ibp_conv(const float* W, const float* bias, const float* l_in, const float* u_in,
