@@ -49,6 +49,7 @@ def parse_args():
     ap.add_argument("--mem-cap-gb", type=float, default=0.0)
     ap.add_argument("--stream-weights", action="store_true",
                     help="layers with >= 2^28 weights are streamed from pinned host memory (a7), not resident")
+    ap.add_argument("--fusion", action="store_true", help="use the fused relax+contraction kernel where it applies")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     return ap.parse_args()
@@ -66,18 +67,14 @@ def peaks():
 
 def workload_desc(wl, cfgname):
     return {"workload": f"{cfgname}:{wl.name}", "B": int(wl.B), "S": int(wl.S),
-            "eps_set": [float(e) for e in wl.eps_set], "properties_per_step": int(wl.B * len(wl.eps_set)),
+            "eps_set": sorted({round(float(e), 6) for e in wl.eps}), "properties_per_step": int(wl.B),
             "intermediate": wl.intermediate, "alpha": wl.alpha is not None}
 
 
 def boxes(wl):
-    """One (x_lo, x_hi) pair per eps of the workload (reading G13: each eps is its own batch)."""
-    out = []
-    for e in wl.eps_set:
-        e32 = np.float32(e).astype(np.float64)
-        x = wl.x0.astype(np.float64)
-        out.append(((x - e32).astype(np.float32), (x + e32).astype(np.float32)))
-    return out
+    """The (x_lo, x_hi) batches of a step.  Workloads with several eps (cfg2: 64 points x 3 eps) are stacked by
+    workloads.stack_eps into ONE batch of per-property radii before this is called (reading G13)."""
+    return [wl.box()]
 
 
 # ------------------------------------------------------------------------------------------------
@@ -93,7 +90,9 @@ def oracle_sample(wl, bxs, budget_s, max_props=None):
     except Exception:
         thr = os.cpu_count() or 1
     done, t0 = 0, time.perf_counter()
-    order = [(p, e) for p in range(wl.B) for e in range(len(bxs))]
+    k = max(1, len({float(e) for e in wl.eps}))          # stacked eps groups: visit them round robin
+    per = max(1, wl.B // k)
+    order = [(p, 0) for p in sorted(range(wl.B), key=lambda q: (q % per, q // per))]
     for p, e in order:
         lo, hi = bxs[e]
         al = None if wl.alpha is None else [a[p] for a in wl.alpha]
@@ -109,7 +108,7 @@ def run_reference(args):
     if rank != 0:
         return
     cfg = int(args.workload[3:])
-    wl = W.make(cfg, scale=args.scale, B=args.batch or None)
+    wl = W.stack_eps(W.make(cfg, scale=args.scale, B=args.batch or None))
     bxs = boxes(wl)
     # each step = a bounded sample (first `per_step` properties) so K+W steps end within minutes
     n1, t1, thr = oracle_sample(wl, bxs, 0.0, max_props=1)
@@ -198,7 +197,7 @@ def run_b200(args):
         dist.init_process_group("nccl", device_id=dev)
 
     cfg = int(args.workload[3:])
-    wl = W.make(cfg, scale=args.scale, B=args.batch or None)
+    wl = W.stack_eps(W.make(cfg, scale=args.scale, B=args.batch or None))
     bxs = boxes(wl)
     B, S, nE = wl.B, wl.S, len(bxs)
     props_per_step = B * nE
@@ -206,7 +205,7 @@ def run_b200(args):
     if cap == 0 and cfg in (3, 4):
         cap = 64 << 30
     ctx = CrownContext(wl.net, B, S, device=f"cuda:{local}", mem_cap_bytes=cap,
-                       stream_weights=int(args.stream_weights))
+                       stream_weights=int(args.stream_weights), enable_fusion=int(args.fusion))
     inter = 1 if wl.intermediate == "ibp" else 0
 
     # ---- inputs resident in HBM -------------------------------------------------------------------
@@ -332,7 +331,7 @@ def run_b200(args):
             "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32 (3xTF32 products, fp32 accumulate)", "data": "synthetic",
             "config": dict(workload_desc(wl, args.workload), l2="flushed between timed steps (256 MB write)",
-                           mem_cap_bytes=cap, stream_weights=bool(args.stream_weights),
+                           mem_cap_bytes=cap, stream_weights=bool(args.stream_weights), fusion=bool(args.fusion),
                            streamed_layers=len(ctx.streamed_ids), weight_h2d_bytes_per_step=w_h2d_step),
             "verified_last_batch": verified, "aw_tflops": aw_tflops, "aw_flops_per_step": flops_step,
             "peak_hbm_gb": {"workspace_high_water": peak_ws / 1e9, "torch_max_allocated": peak_torch / 1e9},

@@ -65,17 +65,16 @@ def _check_props(wl, res, lo, hi, props, rows_per_layer=None, seed=0):
 
 
 def test_cfg2_full_all_eps():
-    wl = W.make(2)                                   # 784-(256x6)-10, B = 64, alpha
-    for eps in wl.eps_set:
-        _, res, lo, hi = _run(wl, eps)
-        props = range(wl.B) if eps == wl.eps_set[1] else [0, 21, 42, 63]
-        _check_props(wl, res, lo, hi, props)
-        # soundness on samples for two properties (O6; slack = parity tolerance, reading G17)
-        lb, ub = _np64(res["lb"]), _np64(res["ub"])
-        for p in (0, 63):
-            X = W.sample_points(2, lo[p], hi[p], 2048, 512)
-            ok, vlo, vhi, _, _ = O.sample_check(wl.net, wl.C[p], X, lb[p], ub[p], slack_rel=RTOL, slack_abs=ATOL)
-            assert ok, (vlo, vhi)
+    wl = W.stack_eps(W.make(2))                      # 784-(256x6)-10, 64 points x 3 eps = ONE batch of 192, alpha
+    assert wl.B == 192
+    _, res, lo, hi = _run(wl)
+    _check_props(wl, res, lo, hi, list(range(64, 128)) + [0, 21, 42, 63, 128, 149, 170, 191])
+    # soundness on samples for a property of each eps (O6; slack = parity tolerance, reading G17)
+    lb, ub = _np64(res["lb"]), _np64(res["ub"])
+    for p in (0, 100, 191):
+        X = W.sample_points(2, lo[p], hi[p], 2048, 512)
+        ok, vlo, vhi, _, _ = O.sample_check(wl.net, wl.C[p], X, lb[p], ub[p], slack_rel=RTOL, slack_abs=ATOL)
+        assert ok, (vlo, vhi)
 
 
 def test_cfg5_full():

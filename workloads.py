@@ -300,6 +300,20 @@ def make(cfg: int, scale: int = 1, B: Optional[int] = None, eps: Optional[float]
                     intermediate=inter, eps_set=(0.015, 0.026, 0.05) if cfg == 2 else (eps_,))
 
 
+def stack_eps(wl: Workload) -> Workload:
+    """All eps values of a workload as ONE batch: property p of the result is point p % B with radius
+    eps_set[p // B] (eps is a per-property input of the boundary, so the three batches of cfg2 are one
+    call of 3*B properties, reading G13).  C, labels and alpha repeat per eps."""
+    k = len(wl.eps_set)
+    if k <= 1:
+        return wl
+    eps = np.concatenate([np.full((wl.B,), e, dtype=np.float32) for e in wl.eps_set])
+    al = None if wl.alpha is None else [np.concatenate([a] * k, axis=0) for a in wl.alpha]
+    return Workload(cfg=wl.cfg, name=wl.name + f"_x{k}eps", net=wl.net, x0=np.concatenate([wl.x0] * k, axis=0),
+                    eps=eps, C=np.concatenate([wl.C] * k, axis=0), labels=np.concatenate([wl.labels] * k),
+                    alpha=al, intermediate=wl.intermediate, eps_set=(float("nan"),))
+
+
 def small_mlp(widths, seed: int, B: int = 2, eps: float = 0.1, S: Optional[int] = None,
               with_alpha: bool = True, bias_shift: float = 0.0, weight_scale: float = 1.0) -> Workload:
     """Tiny seeded MLP workload for unit tests / brute force. bias_shift is added to the hidden
