@@ -294,6 +294,12 @@ def run_b200(args):
     pk = peaks()
     long_step = ms_step > 1000.0
     shares = {k: round(c["ms"] / tot_class_ms, 4) for k, c in classes.items() if c["launches"]}
+    # per kernel class: launches per step, mean device time, achieved algorithmic GB/s and TFLOP/s (bytes / flops are the
+    # library's own per-launch algorithmic counts)
+    per_class = {k: {"launches_per_step": c["launches"] / args.steps, "ms_per_step": c["ms"] / args.steps,
+                     "gbs": (c["bytes"] / (c["ms"] * 1e-3) / 1e9) if c["ms"] > 0 and c["bytes"] > 0 else None,
+                     "tflops": (c["flops"] / (c["ms"] * 1e-3) / 1e12) if c["ms"] > 0 and c["flops"] > 0 else None}
+                 for k, c in classes.items() if c["launches"]}
     d = classes[dom]
     avg_ms = d["ms"] / max(d["launches"], 1)
     if dom == "gemm_tc":
@@ -335,7 +341,7 @@ def run_b200(args):
                            streamed_layers=len(ctx.streamed_ids), weight_h2d_bytes_per_step=w_h2d_step),
             "verified_last_batch": verified, "aw_tflops": aw_tflops, "aw_flops_per_step": flops_step,
             "peak_hbm_gb": {"workspace_high_water": peak_ws / 1e9, "torch_max_allocated": peak_torch / 1e9},
-            "kernel_time_shares": shares,
+            "kernel_time_shares": shares, "kernel_classes": per_class,
             "roofline": roof, "cpu_baseline": cpu,
             "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                     "ms_per_step": ms_e2e},

@@ -211,7 +211,7 @@ int ibp_internal(crown_ctx* ctx, int B, const float* x_lo, const float* x_hi, fl
             },
             [&](int sl, uint8_t* src) {
               const int r0 = sl * rs_max, rs = std::min(rs_max, nd.n_out - r0);
-              Scope sc(ctx, CROWN_K_IBP, 4.0 * rs * nd.n_in * ((B + 7) / 8), 4.0 * B * rs * (double)nd.n_in);
+              Scope sc(ctx, CROWN_K_IBP, 4.0 * rs * nd.n_in * ((B + 3) / 4), 4.0 * B * rs * (double)nd.n_in);
               launch_ibp_linear(reinterpret_cast<const float*>(src), nd.b_dev ? nd.b_dev + r0 : nullptr, li, ui, relu_in,
                                 lo + r0, uo + r0, B, rs, nd.n_in, nd.n_out, s);
               return 0;
@@ -219,7 +219,7 @@ int ibp_internal(crown_ctx* ctx, int B, const float* x_lo, const float* x_hi, fl
           if (rc2) return rc2;
           break;
         }
-        Scope sc(ctx, CROWN_K_IBP, 4.0 * nd.n_out * nd.n_in * ((B + 7) / 8), 4.0 * B * nd.n_out * (double)nd.n_in);
+        Scope sc(ctx, CROWN_K_IBP, 4.0 * nd.n_out * nd.n_in * ((B + 3) / 4), 4.0 * B * nd.n_out * (double)nd.n_in);
         launch_ibp_linear(nd.W_dev, nd.b_dev, li, ui, relu_in, lo, uo, B, nd.n_out, nd.n_in, nd.n_out, s);
         break; }
       case CROWN_CONV2D: {
