@@ -200,7 +200,6 @@ gemm_fused_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
       int g, r0, nb; tile_info(t, g, r0, nb);
       const bool row_ok = r0 + row < p.Rg;
       const long long m = (long long)g * p.Rg + (row_ok ? r0 + row : 0);
-      const int b = (int)((m / p.R) % p.B);
       const bool upper = m >= (long long)p.B * p.R;
       // per-stage coefficient slots {dU, bU, dL, bias}; the lower branch multiplies a>0 by dL and a<0 by dU, the
       // upper branch swaps them

@@ -52,7 +52,7 @@ __global__ void __launch_bounds__(Cfg<BN>::THREADS, 1)
 gemm_tf32x3_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant__ CUtensorMap tmA_lo,
                    const __grid_constant__ CUtensorMap tmB_hi, const __grid_constant__ CUtensorMap tmB_lo,
                    const __grid_constant__ CUtensorMap tmD, int M, int N, int K, int kb_per_chunk,
-                   int chunks_per_small) {
+                   int chunks_per_small, int accumulate) {
   using C = Cfg<BN>;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t raw = smem_u32(smem_raw);
@@ -235,7 +235,8 @@ gemm_tf32x3_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_cons
         fence_proxy_async();
         __syncwarp();
         if (lane == 0) {
-          tma_store_2d(&tmD, epi_base + (uint32_t)ew * 4096u, nb * BN + chalf * EC + sl * 32, mb * BM + quad * 32);
+          if (accumulate) tma_reduce_add_2d(&tmD, epi_base + (uint32_t)ew * 4096u, nb * BN + chalf * EC + sl * 32, mb * BM + quad * 32);
+          else tma_store_2d(&tmD, epi_base + (uint32_t)ew * 4096u, nb * BN + chalf * EC + sl * 32, mb * BM + quad * 32);
           bulk_commit();
         }
       }
@@ -257,12 +258,8 @@ static int launch_bn(const float* A_hi, const float* A_lo, const float* Wt_hi, c
                      long long ldd, int M, int N, int K, int k_drain, int num_sms, cudaStream_t s,
                      const char** err) {
   using C = Cfg<BN>;
-  CUtensorMap ta, tb, tc_, td, tout;
-  if (!make_tmap(&ta, A_hi, M, K, BM) || !make_tmap(&tb, A_lo, M, K, BM) ||
-      !make_tmap(&tc_, Wt_hi, N, K, BN) || !make_tmap(&td, Wt_lo, N, K, BN) || !make_tmap_out(&tout, D, M, N, ldd)) {
-    if (err) *err = "cuTensorMapEncodeTiled failed";
-    return -1;
-  }
+  CUtensorMap tout;
+  if (!make_tmap_out(&tout, D, M, N, ldd)) { if (err) *err = "cuTensorMapEncodeTiled failed"; return -1; }
   static bool attr_set = false;
   if (!attr_set) {
     cudaError_t e = cudaFuncSetAttribute(gemm_tf32x3_kernel<BN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -278,10 +275,32 @@ static int launch_bn(const float* A_hi, const float* A_lo, const float* Wt_hi, c
   if (kb_per_chunk < 1) kb_per_chunk = 1;
   int chunks_per_small = 16384 / (kb_per_chunk * BK);   // small accumulator drained every 16384 elements of K
   if (chunks_per_small < 1) chunks_per_small = 1;
-  gemm_tf32x3_kernel<BN><<<grid, C::THREADS, C::SMEM_BYTES, s>>>(ta, tb, tc_, td, tout, M, N, K, kb_per_chunk,
-                                                                 chunks_per_small);
-  cudaError_t e = cudaGetLastError();
-  if (e != cudaSuccess) { if (err) *err = cudaGetErrorString(e); return -1; }
+  // K panels.  One wave of 148 tiles shares ~8 m-blocks of A and ~19 n-blocks of W; streamed over the whole K their
+  // hi/lo limbs are (8 + 19) * 128 rows * K * 8 B, which for K = 16384 is 450 MB: far beyond the 126 MB L2, and
+  // measured (profiles/r1_gemm_tf32x3_cfg3.md) as DRAM traffic above the kernel's own request volume.  Cutting K
+  // into panels whose per-wave working set fits L2 makes operand re-use independent of how far CTAs drift apart;
+  // panels after the first add into D with the TMA's fp32 reduce-add (fixed order: deterministic).
+  const long long share_blocks = (long long)(m_tiles < GROUP_M ? m_tiles : GROUP_M) +
+                                 (long long)(n_tiles < 19 ? n_tiles : 19);
+  const long long bytes_per_k = share_blocks * 128 * 8;
+  int kp = K;
+  if (bytes_per_k * K > (96LL << 20)) {
+    kp = (int)((64LL << 20) / bytes_per_k) / 512 * 512;
+    if (kp < 1024) kp = 1024;
+  }
+  for (int k0 = 0; k0 < K; k0 += kp) {
+    const int kk = K - k0 < kp ? K - k0 : kp;
+    CUtensorMap ta, tb, tc_, td;
+    if (!make_tmap(&ta, A_hi + k0, M, kk, BM, K) || !make_tmap(&tb, A_lo + k0, M, kk, BM, K) ||
+        !make_tmap(&tc_, Wt_hi + k0, N, kk, BN, K) || !make_tmap(&td, Wt_lo + k0, N, kk, BN, K)) {
+      if (err) *err = "cuTensorMapEncodeTiled failed";
+      return -1;
+    }
+    gemm_tf32x3_kernel<BN><<<grid, C::THREADS, C::SMEM_BYTES, s>>>(ta, tb, tc_, td, tout, M, N, kk, kb_per_chunk,
+                                                                   chunks_per_small, k0 > 0 ? 1 : 0);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) { if (err) *err = cudaGetErrorString(e); return -1; }
+  }
   return 0;
 }
 

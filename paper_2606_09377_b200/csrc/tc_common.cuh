@@ -70,6 +70,11 @@ __device__ __forceinline__ void tma_store_2d(const CUtensorMap* map, uint32_t sr
   asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];"
                :: "l"(map), "r"(src), "r"(x), "r"(y) : "memory");
 }
+// same, but D += tile (fp32 add performed by the TMA unit in L2): used by the K-panel passes after the first
+__device__ __forceinline__ void tma_reduce_add_2d(const CUtensorMap* map, uint32_t src, int x, int y) {
+  asm volatile("cp.reduce.async.bulk.tensor.2d.global.shared::cta.add.tile.bulk_group [%0, {%2, %3}], [%1];"
+               :: "l"(map), "r"(src), "r"(x), "r"(y) : "memory");
+}
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
@@ -186,12 +191,13 @@ inline EncodeTiledFn get_encode_fn() {
   return fn;
 }
 
-// [rows, K] fp32 row-major, box = 32 (K) x box_rows, 128B swizzle, zero fill out of bounds.
-inline bool make_tmap(CUtensorMap* m, const float* ptr, int rows, int K, int box_rows) {
+// [rows, K] fp32 with row pitch `pitch` elements (a K-panel of a wider matrix when pitch > K), box = 32 (K) x box_rows,
+// 128B swizzle, zero fill out of bounds.
+inline bool make_tmap(CUtensorMap* m, const float* ptr, int rows, int K, int box_rows, long long pitch = 0) {
   EncodeTiledFn fn = get_encode_fn();
   if (!fn) return false;
   cuuint64_t dims[2] = {(cuuint64_t)K, (cuuint64_t)rows};
-  cuuint64_t strides[1] = {(cuuint64_t)K * 4};
+  cuuint64_t strides[1] = {(cuuint64_t)(pitch ? pitch : K) * 4};
   cuuint32_t box[2] = {(cuuint32_t)BK, (cuuint32_t)box_rows};
   cuuint32_t estr[2] = {1, 1};
   CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(ptr), dims, strides, box, estr,
