@@ -90,6 +90,8 @@ typedef struct {
                                TF32 split happen in shared memory between TMA and the MMAs, Abar is never
                                materialised.  0 (default): relax kernel + contraction kernel, which measured
                                faster on B200 for every BASELINE config                  */
+  int32_t disable_conc_fusion; /* 1: always materialise A_0 and run the concretise kernel (default 0: when the
+                               last contraction of a pass has a single K panel, concretise in its epilogue) */
 } crown_opts;
 
 typedef struct crown_ctx crown_ctx;   /* opaque; owned by the library; freed by crown_destroy */

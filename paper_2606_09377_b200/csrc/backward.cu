@@ -70,6 +70,7 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
   if (lb && (!ub || !x_lo || !x_hi)) return fail(ctx, CROWN_EINVAL, "crown_backward: concretisation needs ub, x_lo, x_hi");
   std::fill(ctx->pool_ref.begin(), ctx->pool_ref.end(), 0);
   Pass ps; ps.ctx = ctx; ps.B = B; ps.R = R;
+  float* conc_part = nullptr; int conc_parts = 0, conc_buf = -1;
   const NodeInfo& sn = ctx->nodes[start];
   int first = start;   // first node to visit in the reverse sweep
   if (C_dev) {
@@ -212,6 +213,10 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
             const int K = nd.n_out, N = nd.n_in;
             const int ns_max = slab_rows(ctx->plan.stage_bytes, N, K, 2);
             const int nslabs = (N + ns_max - 1) / ns_max;
+            // same rule as the resident path (bitwise equality of the two modes): concretise in the epilogue
+            const bool fc = nd.in0 < 0 && lb && !A_dev && ps.pend.find(-1) == ps.pend.end() && !ctx->opts.disable_conc_fusion &&
+                            gemm_tc_conc_supported(M_full, N, K) && (size_t)M_full * gemm_tc_conc_parts(N) * 8 <= ctx->plan.buf_bytes &&
+                            (ns_max % 128 == 0 || nslabs == 1);
             int rc2 = stream_slabs(ctx, nslabs,
               [&](int sl, uint8_t* dst, cudaStream_t cs) {
                 const int n0 = sl * ns_max, ns = std::min(ns_max, N - n0);
@@ -225,11 +230,34 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
                 const int n0 = sl * ns_max, ns = std::min(ns_max, N - n0);
                 const float* whi = reinterpret_cast<const float*>(src);
                 Scope sc(ctx, CROWN_K_GEMM_TC, 4.0 * ((double)M_full * K + (double)K * ns + (double)M_full * ns), 2.0 * M_full * (double)ns * K);
-                if (launch_gemm_tc(hi, lo, whi, whi + (size_t)ns * K, D + n0, N, M_full, ns, K, ctx->opts.k_drain, ctx->num_sms, s, &e))
+                ConcArgs ca;
+                if (fc) { ca.x_lo = x_lo; ca.x_hi = x_hi; ca.part = D; ca.B = B; ca.R = R; ca.parts = gemm_tc_conc_parts(N);
+                          ca.ldx = N; ca.col_off = n0; ca.piece0 = 2 * (n0 / 128); }
+                if (launch_gemm_tc(hi, lo, whi, whi + (size_t)ns * K, fc ? nullptr : D + n0, N, M_full, ns, K, ctx->opts.k_drain,
+                                   ctx->num_sms, s, &e, fc ? &ca : nullptr))
                   return fail(ctx, CROWN_ECUDA, std::string("gemm_tc: ") + (e ? e : "?"));
                 return (int)CROWN_OK;
               });
             if (rc2) return rc2;
+            if (fc) {
+              conc_part = D; conc_parts = gemm_tc_conc_parts(N); conc_buf = out.buf;
+              ctx->gemm_flops += 2.0 * M_full * (double)N * K;
+              release(ctx, cur);
+              break;
+            }
+          } else if (nd.in0 < 0 && lb && !A_dev && ps.pend.find(-1) == ps.pend.end() && !ctx->opts.disable_conc_fusion &&
+                     gemm_tc_conc_supported(M_full, nd.n_in, nd.n_out) &&
+                     (size_t)M_full * gemm_tc_conc_parts(nd.n_in) * 8 <= ctx->plan.buf_bytes) {
+            // last contraction of the pass: concretise in its epilogue (a8 fused), A_0 never reaches HBM
+            ConcArgs ca;
+            ca.x_lo = x_lo; ca.x_hi = x_hi; ca.part = D; ca.B = B; ca.R = R; ca.parts = gemm_tc_conc_parts(nd.n_in); ca.ldx = nd.n_in;
+            Scope sc(ctx, CROWN_K_GEMM_TC, 4.0 * (2.0 * M_full * nd.n_out + 2.0 * nd.n_out * nd.n_in), 2.0 * M_full * (double)nd.n_in * nd.n_out);
+            if (launch_gemm_tc(hi, lo, ni.Wt_hi, ni.Wt_lo, nullptr, nd.n_in, M_full, nd.n_in, nd.n_out, ctx->opts.k_drain, ctx->num_sms, s, &e, &ca))
+              return fail(ctx, CROWN_ECUDA, std::string("gemm_tc: ") + (e ? e : "?"));
+            conc_part = D; conc_parts = ca.parts; conc_buf = out.buf;
+            ctx->gemm_flops += 2.0 * M_full * (double)nd.n_in * nd.n_out;
+            release(ctx, cur);
+            break;                      // nothing is contributed to the input node: the bound is finished below
           } else {
             Scope sc(ctx, CROWN_K_GEMM_TC, 4.0 * ((double)M_full * nd.n_out + (double)nd.n_out * nd.n_in + (double)M_full * nd.n_in),
                      2.0 * M_full * (double)nd.n_in * nd.n_out);
@@ -284,6 +312,14 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
         return fail(ctx, CROWN_EUNSUPPORTED, "crown_backward: unsupported op");
     }
     if (rc) return rc;
+  }
+  if (conc_part) {   // the bound was concretised inside the last contraction
+    if (d_dev) CK(ctx, cudaMemcpyAsync(d_dev, ctx->d_buf, (size_t)2 * B * R * 4, cudaMemcpyDeviceToDevice, s));
+    { Scope sc(ctx, CROWN_K_CONCRETIZE, 8.0 * 2 * B * R * conc_parts);
+      launch_concretize_parts(conc_part, conc_parts, ctx->d_buf, lb, ub, out_stride, B, R, s); }
+    pool_release(ctx, conc_buf);
+    CK(ctx, cudaGetLastError());
+    return CROWN_OK;
   }
   // A w.r.t. the network input
   auto it = ps.pend.find(-1);

@@ -259,6 +259,30 @@ void launch_concretize(const AView& A, const float* d, const float* x_lo, const 
   else concretize_kernel<1><<<blocks, 256, 0, s>>>(A.p, A.sBr, A.sB, A.ld, A.n, d, x_lo, x_hi, lb, ub, out_stride, B, R);
 }
 
+// a8, second half of the fused form: add the per-piece (dot, |.|) pairs written by the contraction epilogue in
+// index order and finish lb = dot - ab + d (branch 0), ub = dot + ab + d (branch 1).
+__global__ void concretize_parts_kernel(const float2* __restrict__ part, int parts, const float* __restrict__ d,
+                                        float* __restrict__ lb, float* __restrict__ ub, int out_stride, int B, int R) {
+  const long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long BR = (long long)B * R;
+  if (m >= 2 * BR) return;
+  float dot = 0.f, ab = 0.f;
+  for (int i = 0; i < parts; ++i) { const float2 v = part[m * parts + i]; dot += v.x; ab += v.y; }
+  const int br = (int)(m / BR);
+  const long long pair = m % BR;
+  const int b = (int)(pair / R), r = (int)(pair % R);
+  const float dd = d ? d[m] : 0.f;
+  if (br == 0) lb[(long long)b * out_stride + r] = (dot - ab) + dd;
+  else ub[(long long)b * out_stride + r] = (dot + ab) + dd;
+}
+void launch_concretize_parts(const float* part, int parts, const float* d, float* lb, float* ub, int out_stride,
+                             int B, int R, cudaStream_t s) {
+  const long long rows = 2LL * B * R;
+  if (rows <= 0) return;
+  concretize_parts_kernel<<<ceil_div(rows, 256), 256, 0, s>>>(reinterpret_cast<const float2*>(part), parts, d, lb, ub,
+                                                             out_stride, B, R);
+}
+
 // ------------------------------------------------------------------------------------------------
 // helpers
 // ------------------------------------------------------------------------------------------------

@@ -52,7 +52,7 @@ __global__ void __launch_bounds__(Cfg<BN>::THREADS, 1)
 gemm_tf32x3_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant__ CUtensorMap tmA_lo,
                    const __grid_constant__ CUtensorMap tmB_hi, const __grid_constant__ CUtensorMap tmB_lo,
                    const __grid_constant__ CUtensorMap tmD, int M, int N, int K, int kb_per_chunk,
-                   int chunks_per_small, int accumulate) {
+                   int chunks_per_small, int accumulate, const ConcArgs conc) {
   using C = Cfg<BN>;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t raw = smem_u32(smem_raw);
@@ -218,6 +218,31 @@ gemm_tf32x3_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_cons
           ++small_cnt;
         }
       }
+      if (conc.part != nullptr) {
+        // a8 fused: this warp's 64 columns of row `row` against the box of the row's property; A_0 is never stored
+        const int row = mb * BM + quad * 32 + lane;
+        const int col0 = nb * BN + chalf * EC;
+        if (row < M) {
+          const int b = (row / conc.R) % conc.B;
+          const float* xl = conc.x_lo + (long long)b * conc.ldx + conc.col_off + col0;
+          const float* xh = conc.x_hi + (long long)b * conc.ldx + conc.col_off + col0;
+          float dot = 0.f, ab = 0.f;
+#pragma unroll
+          for (int i = 0; i < EC; i += 4) {
+            if (col0 + i < N) {                      // N % 4 == 0: whole float4 in range
+              const float4 lo = __ldg(reinterpret_cast<const float4*>(xl + i));
+              const float4 hi = __ldg(reinterpret_cast<const float4*>(xh + i));
+              dot = fmaf(acc[i], 0.5f * (lo.x + hi.x), dot);     ab = fmaf(fabsf(acc[i]), 0.5f * (hi.x - lo.x), ab);
+              dot = fmaf(acc[i + 1], 0.5f * (lo.y + hi.y), dot); ab = fmaf(fabsf(acc[i + 1]), 0.5f * (hi.y - lo.y), ab);
+              dot = fmaf(acc[i + 2], 0.5f * (lo.z + hi.z), dot); ab = fmaf(fabsf(acc[i + 2]), 0.5f * (hi.z - lo.z), ab);
+              dot = fmaf(acc[i + 3], 0.5f * (lo.w + hi.w), dot); ab = fmaf(fabsf(acc[i + 3]), 0.5f * (hi.w - lo.w), ab);
+            }
+          }
+          float2* dst = reinterpret_cast<float2*>(conc.part) + (long long)row * conc.parts + (conc.piece0 + nb * 2 + chalf);
+          *dst = make_float2(dot, ab);
+        }
+        continue;
+      }
       // tile -> global through shared memory and the TMA: lane = row writes its 32 columns (128 B) of a slab in the
       // 128B-swizzled layout (conflict-free), one lane issues the bulk tensor store, which also clips the M / N edges
       const uint32_t slab = epi_base + (uint32_t)ew * 4096u + (uint32_t)lane * 128u;
@@ -256,10 +281,15 @@ gemm_tf32x3_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_cons
 template <int BN>
 static int launch_bn(const float* A_hi, const float* A_lo, const float* Wt_hi, const float* Wt_lo, float* D,
                      long long ldd, int M, int N, int K, int k_drain, int num_sms, cudaStream_t s,
-                     const char** err) {
+                     const char** err, const ConcArgs* conc) {
   using C = Cfg<BN>;
   CUtensorMap tout;
-  if (!make_tmap_out(&tout, D, M, N, ldd)) { if (err) *err = "cuTensorMapEncodeTiled failed"; return -1; }
+  const bool fused_conc = conc && conc->part;
+  // fused concretisation stores no D: the output map is a placeholder over the partial-sum buffer
+  if (!(fused_conc ? make_tmap_out(&tout, conc->part, M, 4, 4) : make_tmap_out(&tout, D, M, N, ldd))) {
+    if (err) *err = "cuTensorMapEncodeTiled failed";
+    return -1;
+  }
   static bool attr_set = false;
   if (!attr_set) {
     cudaError_t e = cudaFuncSetAttribute(gemm_tf32x3_kernel<BN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -288,6 +318,8 @@ static int launch_bn(const float* A_hi, const float* A_lo, const float* Wt_hi, c
     kp = (int)((64LL << 20) / bytes_per_k) / 512 * 512;
     if (kp < 1024) kp = 1024;
   }
+  if (fused_conc && kp != K) { if (err) *err = "gemm_tc: fused concretisation needs a single K panel"; return -1; }
+  const ConcArgs cargs = fused_conc ? *conc : ConcArgs();
   for (int k0 = 0; k0 < K; k0 += kp) {
     const int kk = K - k0 < kp ? K - k0 : kp;
     CUtensorMap ta, tb, tc_, td;
@@ -297,7 +329,7 @@ static int launch_bn(const float* A_hi, const float* A_lo, const float* Wt_hi, c
       return -1;
     }
     gemm_tf32x3_kernel<BN><<<grid, C::THREADS, C::SMEM_BYTES, s>>>(ta, tb, tc_, td, tout, M, N, kk, kb_per_chunk,
-                                                                   chunks_per_small, k0 > 0 ? 1 : 0);
+                                                                   chunks_per_small, k0 > 0 ? 1 : 0, cargs);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) { if (err) *err = cudaGetErrorString(e); return -1; }
   }
@@ -312,16 +344,24 @@ int gemm_tc_supported(int M, int N, int K) {
   return M >= 1 && N >= 128 && K >= 32 && (K % 4 == 0) && (N % 4 == 0);
 }
 
+int gemm_tc_conc_parts(int N) { return 2 * ((N + 127) / 128); }
+
+int gemm_tc_conc_supported(int M, int N, int K) {
+  // single K panel (see launch_bn): the working-set rule only cuts K above ~3000 for >= 27 shared blocks
+  return gemm_tc_supported(M, N, K) && K <= 2048;
+}
+
 int launch_gemm_tc(const float* A_hi, const float* A_lo, const float* Wt_hi, const float* Wt_lo, float* D,
                    long long ldd, int M, int N, int K, int k_drain, int num_sms, cudaStream_t s,
-                   const char** err) {
+                   const char** err, const ConcArgs* conc) {
   auto mis = [](const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) != 0; };
-  if (!gemm_tc_supported(M, N, K) || mis(A_hi) || mis(A_lo) || mis(Wt_hi) || mis(Wt_lo) || mis(D) ||
-      (ldd % 4) != 0) {
+  const bool fc = conc && conc->part;
+  if (!gemm_tc_supported(M, N, K) || mis(A_hi) || mis(A_lo) || mis(Wt_hi) || mis(Wt_lo) || (!fc && (mis(D) || (ldd % 4) != 0)) ||
+      (fc && (mis(conc->x_lo) || mis(conc->x_hi) || mis(conc->part)))) {
     if (err) *err = "gemm_tc: unsupported shape or misaligned operand";
     return -1;
   }
-  return tc::launch_bn<128>(A_hi, A_lo, Wt_hi, Wt_lo, D, ldd, M, N, K, k_drain, num_sms, s, err);
+  return tc::launch_bn<128>(A_hi, A_lo, Wt_hi, Wt_lo, D, ldd, M, N, K, k_drain, num_sms, s, err, conc);
 }
 
 }  // namespace crownb200

@@ -76,11 +76,26 @@ void launch_gemm_ffma(const float* A, long long lda, const float* W, long long l
 // a5 -- 3xTF32 contraction on tcgen05 tensor cores: D[M,N] = (A_hi + A_lo)[M,K] . (Wt_hi + Wt_lo)[N,K]^T
 // with the three products hi.hi + hi.lo + lo.hi accumulated in fp32 (TMEM), drained to an fp32
 // CUDA-core running sum every k_drain elements of K.
-struct TmapSet;  // opaque TMA descriptors of one (A, W) operand pair, built on the host
+// a8 fused into the last contraction: when `part` != nullptr the epilogue does not store D; every epilogue warp
+// reduces its 64 columns of the tile against the box instead (dot = sum A.x_c, ab = sum |A|.x_r) and writes the pair
+// to part[(row * parts + piece) * 2 + {0,1}], piece = 2 * n_block + column half.  launch_concretize_parts then adds
+// the pieces in index order (deterministic).  Only valid when K is a single panel (|.| is not linear in K).
+struct ConcArgs {
+  const float* x_lo = nullptr; const float* x_hi = nullptr;   // [B, ldx]
+  float* part = nullptr;                                       // [M, parts, 2]
+  int B = 0, R = 0, parts = 0;
+  int ldx = 0;        // row pitch of x_lo / x_hi (the full input width)
+  int col_off = 0;    // first input column of this launch (N-slab of a streamed operand), multiple of 128
+  int piece0 = 0;     // first piece index of this launch = 2 * col_off / 128
+};
+int gemm_tc_conc_parts(int N);                 // pieces per row for an N-wide output
+int gemm_tc_conc_supported(int M, int N, int K);
+void launch_concretize_parts(const float* part, int parts, const float* d, float* lb, float* ub, int out_stride,
+                             int B, int R, cudaStream_t s);
 int gemm_tc_supported(int M, int N, int K);
 int launch_gemm_tc(const float* A_hi, const float* A_lo, const float* Wt_hi, const float* Wt_lo,
                    float* D, long long ldd, int M, int N, int K, int k_drain, int num_sms,
-                   cudaStream_t s, const char** err);
+                   cudaStream_t s, const char** err, const ConcArgs* conc = nullptr);
 
 // a4 + a5 fused -- relaxation of A through a ReLU (planes != nullptr; fixed-rule slopes only), d += A-/+ . bU,
 // d += Abar . bias, TF32 split and the 3xTF32 contraction with the prepacked operand in one kernel
