@@ -307,7 +307,8 @@ def run_b200(args):
         peak = bf16 * TF32_OVER_BF16 / 3.0           # fp32-equivalent: 3 TF32 MMAs per useful product
         ach = d["flops"] / d["launches"] / (avg_ms * 1e-3) / 1e12
         # DRAM bytes per launch from the committed ncu --set full capture of this command (profiles/r1_gemm_tf32x3_cfg2.md:
-        # 202 MB read + 70 MB written per N = 256 launch at B = 192); null for workloads without a committed capture
+        # 202 MB read + 70 MB written per N = 256 launch at B = 192; algorithmic 4(2MK + 2KN + MN) = 302 MB, the
+        # difference is L2 hits on limbs the relax kernel just wrote); null for workloads without a committed capture
         traffic = 2.72e8 if (cfg == 2 and args.scale == 1 and not args.batch and not args.fusion) else None
         roof = {"kernel": "gemm_tf32x3_kernel", "bound": "tensor", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
                 "frac": ach / peak, "traffic": traffic,
