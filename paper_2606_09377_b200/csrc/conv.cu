@@ -129,7 +129,7 @@ template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" :: "n"(N) : "memory"); }
 
 template <int KH, int KW, int S, int CT>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 2)
 conv_bwd_tiled_kernel(const float* __restrict__ A, long long sBr, long long sB, long long ld, int B, int R,
                       const float* __restrict__ W, const float* __restrict__ addend, float* __restrict__ out,
                       ConvBwdGeom g) {
