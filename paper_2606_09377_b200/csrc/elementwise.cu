@@ -324,27 +324,50 @@ void launch_rowdot_bias(const AView& A, const float* bias, int bias_div, float* 
                                                              bias_div > 0 ? bias_div : 1, d, B, R);
 }
 
-__global__ void view_add_kernel(const float* __restrict__ a, long long aBr, long long aB, long long ald,
-                                const float* __restrict__ b2, long long bBr, long long bB, long long bld,
-                                float* __restrict__ out, int B, int R, int n) {
-  long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  long long tot = 2LL * B * R * n;
-  if (i >= tot) return;
-  int j = (int)(i % n);
-  long long m = i / n;
-  int r = (int)(m % R);
-  long long t = m / R;
-  int b = (int)(t % B), br = (int)(t / B);
-  float v = a[br * aBr + b * aB + r * ald + j];
-  if (b2) v += b2[br * bBr + b * bB + r * bld + j];
-  out[i] = v;
+// out[m, :] = a[m, :] (+ b[m, :]) for the 2*B*R rows of two strided views; blockIdx.y = row, threads walk the row
+// with 128-bit accesses when everything is 16-byte aligned (no per-element index arithmetic).
+template <int VEC>
+__global__ void __launch_bounds__(256) view_add_kernel(const float* __restrict__ a, long long aBr, long long aB, long long ald,
+                                                       const float* __restrict__ b2, long long bBr, long long bB, long long bld,
+                                                       float* __restrict__ out, int B, int R, int n, long long row_base) {
+  const long long m = row_base + blockIdx.y;
+  const int r = (int)(m % R);
+  const long long t = m / R;
+  const int b = (int)(t % B), br = (int)(t / B);
+  const float* pa = a + br * aBr + b * aB + (long long)r * ald;
+  const float* pb = b2 ? b2 + br * bBr + b * bB + (long long)r * bld : nullptr;
+  float* po = out + m * (long long)n;
+  if (VEC == 4) {
+    for (int j = (blockIdx.x * blockDim.x + threadIdx.x) * 4; j < n; j += gridDim.x * blockDim.x * 4) {
+      float4 v = ldg_stream4(pa + j);
+      if (pb) { const float4 w = ldg_stream4(pb + j); v.x += w.x; v.y += w.y; v.z += w.z; v.w += w.w; }
+      stg_stream4(po + j, v);
+    }
+  } else {
+    for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += gridDim.x * blockDim.x) {
+      float v = pa[j];
+      if (pb) v += pb[j];
+      po[j] = v;
+    }
+  }
 }
 void launch_view_add(const AView& a, const AView* b, float* out, int B, int R, cudaStream_t s) {
-  long long tot = 2LL * B * R * a.n;
-  if (tot <= 0) return;
-  view_add_kernel<<<ceil_div(tot, 256), 256, 0, s>>>(a.p, a.sBr, a.sB, a.ld, b ? b->p : nullptr,
-                                                    b ? b->sBr : 0, b ? b->sB : 0, b ? b->ld : 0, out,
-                                                    B, R, a.n);
+  const long long rows = 2LL * B * R;
+  if (rows <= 0 || a.n <= 0) return;
+  auto al16 = [](const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; };
+  auto view_ok = [&](const AView& v) { return al16(v.p) && v.ld % 4 == 0 && v.sB % 4 == 0 && v.sBr % 4 == 0; };
+  const bool vec = a.n % 4 == 0 && al16(out) && view_ok(a) && (!b || view_ok(*b));
+  const int per = vec ? 1024 : 256;                       // elements per block pass
+  int gx = ceil_div(a.n, per);
+  if (gx > 16) gx = 16;
+  for (long long r0 = 0; r0 < rows; r0 += 65535) {        // gridDim.y limit
+    const int ny = (int)(rows - r0 < 65535 ? rows - r0 : 65535);
+    dim3 grid(gx, ny);
+    if (vec) view_add_kernel<4><<<grid, 256, 0, s>>>(a.p, a.sBr, a.sB, a.ld, b ? b->p : nullptr, b ? b->sBr : 0, b ? b->sB : 0,
+                                                   b ? b->ld : 0, out, B, R, a.n, r0);
+    else view_add_kernel<1><<<grid, 256, 0, s>>>(a.p, a.sBr, a.sB, a.ld, b ? b->p : nullptr, b ? b->sBr : 0, b ? b->sB : 0,
+                                                b ? b->ld : 0, out, B, R, a.n, r0);
+  }
 }
 
 __global__ void verdict_kernel(const float* __restrict__ lb, uint8_t* __restrict__ v, int B, int S) {

@@ -195,3 +195,41 @@ def test_streamed_weights_equal_resident_bitwise():
             assert torch.equal(r_res[k], r_str[k]), k
         for i in r_res["pre"]:
             assert torch.equal(r_res["pre"][i][0], r_str["pre"][i][0]) and torch.equal(r_res["pre"][i][1], r_str["pre"][i][1])
+
+
+def test_boundary_calls_one_by_one():
+    """ibp_forward / crown_backward / concretize called separately through the C-ABI (not via crown_run): O1 against
+    the oracle's IBP for every node and the fused spec, O3's A and d against the oracle's linear bounds, and the
+    stand-alone concretisation against the fused one."""
+    wl = W.make(2, B=4)
+    lo, hi = wl.box()
+    ctx = _ctx(wl.net, wl.B, wl.S)
+    # O1
+    ivals, (ilb, iub) = ctx.ibp_forward(lo, hi, wl.C)
+    for p in range(wl.B):
+        ref = O.ibp(wl.net, lo[p], hi[p])
+        for i, (l, u) in enumerate(ref):
+            _close(_np(ivals[i][0])[p], l.reshape(-1), f"ibp node {i} l")
+            _close(_np(ivals[i][1])[p], u.reshape(-1), f"ibp node {i} u")
+        slb, sub = O.ibp_spec(wl.net, lo[p], hi[p], wl.C[p])
+        _close(_np(ilb)[p], slb, "ibp spec lb", atol=1e-4)      # wide IBP intervals: cancellation of O(100) terms
+        _close(_np(iub)[p], sub, "ibp spec ub", atol=1e-4)
+    # O3 with A and d returned, then a8 on its own
+    res = ctx.run(lo, hi, wl.C, wl.alpha, wl.intermediate)
+    al = {i: a for i, a in zip(wl.net.relu_ids(), wl.alpha)}
+    out = ctx.crown_backward(wl.B, len(wl.net.nodes) - 1, res["pre"], Cmat=wl.C, alpha_lo=al, alpha_up=al,
+                             box=(lo, hi), want_A=True)
+    lb2, ub2 = ctx.concretize(out["A"], out["d"], lo, hi)
+    A, d = _np(out["A"]), _np(out["d"])
+    for p in range(wl.B):
+        forced = {i: (_np(l)[p].astype(np.float64), _np(u)[p].astype(np.float64)) for i, (l, u) in res["pre"].items()}
+        alp = {i: a[p] for i, a in al.items()}
+        olb, oub, (A_lo, A_up, d_lo, d_up) = O.final_bounds(wl.net, lo[p], hi[p], wl.C[p], forced, alp, alp)
+        scale = 1e-4 * max(np.abs(A_lo).max(), np.abs(A_up).max())
+        assert np.max(np.abs(A[0, p] - A_lo)) <= scale and np.max(np.abs(A[1, p] - A_up)) <= scale
+        _close(d[0, p], d_lo, "d_lo", atol=1e-4 * np.abs(d_lo).max())
+        _close(d[1, p], d_up, "d_up", atol=1e-4 * np.abs(d_up).max())
+        for g in (_np(out["lb"])[p], _np(lb2)[p], _np(res["lb"])[p]):
+            _close(g, olb, "lb")
+        for g in (_np(out["ub"])[p], _np(ub2)[p], _np(res["ub"])[p]):
+            _close(g, oub, "ub")
