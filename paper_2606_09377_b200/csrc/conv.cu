@@ -9,23 +9,30 @@
 namespace crownb200 {
 
 // ---- a2: IBP through Conv2d.  c' = conv(c, W) + b, r' = conv(r, |W|);  l' = c' - r', u' = c' + r'.
-// grid: (spatial tiles, c_out, B); one thread per output pixel of one output channel.
+// grid: (spatial tiles, c_out / 4, B); one thread per output pixel of FOUR output channels, so every (l, u) pair
+// read from global memory feeds 8 FMAs; the filters of the 4 channels sit in shared memory.
+constexpr int kIbpConvCO = 4;
 __global__ void __launch_bounds__(256)
 ibp_conv_kernel(const float* __restrict__ W, const float* __restrict__ bias, const float* __restrict__ l_in,
                 const float* __restrict__ u_in, int relu_in, float* __restrict__ l_out,
                 float* __restrict__ u_out, int c_in, int h, int w, int c_out, int kh, int kw, int stride,
                 int pad, int ho, int wo) {
-  extern __shared__ float sw[];   // [c_in*kh*kw] filter of this output channel
-  const int co = blockIdx.y, b = blockIdx.z;
+  extern __shared__ float sw[];   // [kIbpConvCO][c_in*kh*kw]
+  const int co0 = blockIdx.y * kIbpConvCO, b = blockIdx.z;
   const int fsz = c_in * kh * kw;
-  for (int i = threadIdx.x; i < fsz; i += blockDim.x) sw[i] = W[(long long)co * fsz + i];
+  for (int i = threadIdx.x; i < kIbpConvCO * fsz; i += blockDim.x) {
+    const int o = i / fsz, k = i % fsz;
+    sw[i] = (co0 + o < c_out) ? W[(long long)(co0 + o) * fsz + k] : 0.f;
+  }
   __syncthreads();
   const int pix = blockIdx.x * blockDim.x + threadIdx.x;
   if (pix >= ho * wo) return;
   const int p = pix / wo, q = pix % wo;
   const float* lb = l_in + (long long)b * c_in * h * w;
   const float* ub = u_in + (long long)b * c_in * h * w;
-  float c = 0.f, r = 0.f;
+  float c[kIbpConvCO], r[kIbpConvCO];
+#pragma unroll
+  for (int o = 0; o < kIbpConvCO; ++o) { c[o] = 0.f; r[o] = 0.f; }
   for (int ci = 0; ci < c_in; ++ci)
     for (int i = 0; i < kh; ++i) {
       const int y = p * stride + i - pad;
@@ -35,15 +42,25 @@ ibp_conv_kernel(const float* __restrict__ W, const float* __restrict__ bias, con
         if (x < 0 || x >= w) continue;
         float lo = lb[(ci * h + y) * w + x], hi = ub[(ci * h + y) * w + x];
         if (relu_in) { lo = fmaxf(lo, 0.f); hi = fmaxf(hi, 0.f); }
-        const float wv = sw[(ci * kh + i) * kw + j];
-        c = fmaf(wv, 0.5f * (lo + hi), c);
-        r = fmaf(fabsf(wv), 0.5f * (hi - lo), r);
+        const float xc = 0.5f * (lo + hi), xr = 0.5f * (hi - lo);
+        const int k = (ci * kh + i) * kw + j;
+#pragma unroll
+        for (int o = 0; o < kIbpConvCO; ++o) {
+          const float wv = sw[o * fsz + k];
+          c[o] = fmaf(wv, xc, c[o]);
+          r[o] = fmaf(fabsf(wv), xr, r[o]);
+        }
       }
     }
-  c += bias ? bias[co] : 0.f;
-  const long long o = ((long long)b * c_out + co) * ho * wo + pix;
-  l_out[o] = c - r;
-  u_out[o] = c + r;
+#pragma unroll
+  for (int o = 0; o < kIbpConvCO; ++o) {
+    const int co = co0 + o;
+    if (co >= c_out) break;
+    const float cc = c[o] + (bias ? bias[co] : 0.f);
+    const long long idx = ((long long)b * c_out + co) * ho * wo + pix;
+    l_out[idx] = cc - r[o];
+    u_out[idx] = cc + r[o];
+  }
 }
 
 void launch_ibp_conv(const float* W, const float* bias, const float* l_in, const float* u_in, int relu_in,
@@ -52,8 +69,8 @@ void launch_ibp_conv(const float* W, const float* bias, const float* l_in, const
   if (B <= 0) return;
   int threads = 256;
   while (threads > 32 && threads / 2 >= ho * wo) threads /= 2;
-  dim3 grid(ceil_div(ho * wo, threads), c_out, B);
-  size_t smem = (size_t)c_in * kh * kw * sizeof(float);
+  dim3 grid(ceil_div(ho * wo, threads), ceil_div(c_out, kIbpConvCO), B);
+  size_t smem = (size_t)kIbpConvCO * c_in * kh * kw * sizeof(float);
   ibp_conv_kernel<<<grid, threads, smem, s>>>(W, bias, l_in, u_in, relu_in, l_out, u_out, c_in, h, w, c_out,
                                               kh, kw, stride, pad, ho, wo);
 }
