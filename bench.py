@@ -49,7 +49,7 @@ def parse_args():
     ap.add_argument("--mem-cap-gb", type=float, default=0.0)
     ap.add_argument("--stream-weights", action="store_true",
                     help="layers with >= 2^28 weights are streamed from pinned host memory (a7), not resident")
-    ap.add_argument("--fusion", action="store_true", help="use the fused relax+contraction kernel where it applies")
+    ap.add_argument("--no-epi-fusion", action="store_true", help="run the relaxation as its own kernel (debug)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     return ap.parse_args()
@@ -205,7 +205,7 @@ def run_b200(args):
     if cap == 0 and cfg in (3, 4):
         cap = 64 << 30
     ctx = CrownContext(wl.net, B, S, device=f"cuda:{local}", mem_cap_bytes=cap,
-                       stream_weights=int(args.stream_weights), enable_fusion=int(args.fusion))
+                       stream_weights=int(args.stream_weights), disable_epi_fusion=int(args.no_epi_fusion))
     inter = 1 if wl.intermediate == "ibp" else 0
 
     # ---- inputs resident in HBM -------------------------------------------------------------------
@@ -309,7 +309,7 @@ def run_b200(args):
         # DRAM bytes per launch from the committed ncu --set full capture of this command (profiles/r1_gemm_tf32x3_cfg2.md:
         # 202 MB read + 70 MB written per N = 256 launch at B = 192; algorithmic 4(2MK + 2KN + MN) = 302 MB, the
         # difference is L2 hits on limbs the relax kernel just wrote); null for workloads without a committed capture
-        traffic = 2.72e8 if (cfg == 2 and args.scale == 1 and not args.batch and not args.fusion) else None
+        traffic = 2.72e8 if (cfg == 2 and args.scale == 1 and not args.batch and not args.no_epi_fusion) else None
         roof = {"kernel": "gemm_tf32x3_kernel", "bound": "tensor", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
                 "frac": ach / peak, "traffic": traffic,
                 "peak_source": f"{pk['src']} bf16 {'sustained' if long_step else 'burst'} x nominal tf32/bf16 ratio / 3"}
@@ -341,7 +341,7 @@ def run_b200(args):
             "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32 (3xTF32 products, fp32 accumulate)", "data": "synthetic",
             "config": dict(workload_desc(wl, args.workload), l2="flushed between timed steps (256 MB write)",
-                           mem_cap_bytes=cap, stream_weights=bool(args.stream_weights), fusion=bool(args.fusion),
+                           mem_cap_bytes=cap, stream_weights=bool(args.stream_weights), epi_fusion=not args.no_epi_fusion,
                            streamed_layers=len(ctx.streamed_ids), weight_h2d_bytes_per_step=w_h2d_step),
             "verified_last_batch": verified, "aw_tflops": aw_tflops, "aw_flops_per_step": flops_step,
             "peak_hbm_gb": {"workspace_high_water": peak_ws / 1e9, "torch_max_allocated": peak_torch / 1e9},

@@ -85,11 +85,10 @@ typedef struct {
                                CUDA-core running sum takes over (0 = library default)            */
   uint64_t stream_min_elems;/* see stream_weights (0 = library default 2^28 elements)            */
   uint64_t stream_stage_bytes; /* size cap of each of the two staging buffers (0 = default 1 GiB) */
-  int32_t enable_fusion;    /* 1: where it applies (resident or streamed Linear below a ReLU, fixed-rule slopes)
-                               run a4 + a5 as ONE kernel (gemm_fused.cu): relaxation, bias accumulation and
-                               TF32 split happen in shared memory between TMA and the MMAs, Abar is never
-                               materialised.  0 (default): relax kernel + contraction kernel, which measured
-                               faster on B200 for every BASELINE config                  */
+  int32_t disable_epi_fusion; /* 0 (default): where a contraction has a single K panel and is followed by a ReLU over a
+                               tensor-core Linear with fixed-rule slopes, its epilogue applies that relaxation, both
+                               bias accumulations and the TF32 split (a4 fused into a5: A <- A.Lambda_i W_i is ONE
+                               kernel).  1: always run the separate relaxation kernel               */
   int32_t disable_conc_fusion; /* 1: always materialise A_0 and run the concretise kernel (default 0: when the
                                last contraction of a pass has a single K panel, concretise in its epilogue) */
 } crown_opts;
@@ -121,7 +120,8 @@ int ibp_forward(crown_ctx* ctx, int B, const float* x_lo_dev, const float* x_hi_
 /* O3 -- one CROWN backward pass (PAPER.md:64-68 Eq. 1, :128 A <- A.Lambda_i W_i) from node
  * `start` down to the input, for `rows` start-spec rows per property.
  *   C_dev == NULL : start matrix = rows [row0, row0+rows) of the identity on node `start`'s
- *                   output (intermediate bounds); `start` must be Linear or Conv2d.
+ *                   output (intermediate bounds); `start` must be a Linear node
+ *                   (CROWN_EUNSUPPORTED otherwise: identity starts on conv maps are NEXT-3).
  *   C_dev != NULL : [B, rows, size_start] start matrix (row0 ignored).
  *   l_dev/u_dev   : arrays of n_nodes pointers; for every ReLU node i below `start`, the
  *                   pre-activation bounds of its INPUT, [B, size_i].
@@ -168,8 +168,8 @@ int crown_run_host(crown_ctx* ctx, int B, const float* x_lo_host, const float* x
                    float* lb_host, float* ub_host, uint8_t* verified_host);
 
 /* D[M,N] = A[M,K] . W[K,N] (row-major fp32) through the same contraction kernel the backward
- * pass uses (scheme: 0 = 3xTF32 tcgen05 on prepared limbs, 1 = the fused kernel in split-only mode: A_hi_dev is
- * the raw fp32 A and is split inside the kernel, 2 = FFMA); exposed for parity tests and roofline
+ * pass uses (scheme: 0 = 3xTF32 tcgen05 on prepared limbs, 2 = FFMA; 1 -- reserved in SURVEY.md for a split-bf16
+ * scheme -- is intentionally absent); exposed for parity tests and roofline
  * measurement of kernel 1.  Wt_hi/Wt_lo [N,K] and A_hi/A_lo [M,K] are produced by
  * crown_split_tf32 (transpose=1 for W). */
 int crown_gemm(crown_ctx* ctx, int scheme, int M, int N, int K,

@@ -34,7 +34,7 @@ class CrownNode(C.Structure):
 class CrownOpts(C.Structure):
     _fields_ = [("mem_cap_bytes", C.c_uint64), ("stream_weights", C.c_int32), ("mma_scheme", C.c_int32),
                 ("slope_rule", C.c_int32), ("k_drain", C.c_int32), ("stream_min_elems", C.c_uint64),
-                ("stream_stage_bytes", C.c_uint64), ("enable_fusion", C.c_int32),
+                ("stream_stage_bytes", C.c_uint64), ("disable_epi_fusion", C.c_int32),
                 ("disable_conc_fusion", C.c_int32)]
 
 
@@ -96,7 +96,7 @@ class CrownContext:
 
     def __init__(self, net, B_max: int, S_max: int, device: str = "cuda:0", mem_cap_bytes: int = 0,
                  mma_scheme: int = 0, slope_rule: int = 0, k_drain: int = 0, stream_weights: int = 0,
-                 stream_min_elems: int = 0, stream_stage_bytes: int = 0, enable_fusion: int = 0,
+                 stream_min_elems: int = 0, stream_stage_bytes: int = 0, disable_epi_fusion: int = 0,
                  disable_conc_fusion: int = 0):
         if not torch.cuda.is_available():
             raise CrownError("no CUDA device: the crownb200 hot path has no CPU fallback")
@@ -140,7 +140,7 @@ class CrownContext:
                     cn.W_dev = Wd.data_ptr()
         self._nodes = arr
         self.opts = CrownOpts(mem_cap_bytes, stream_weights, mma_scheme, slope_rule, k_drain, stream_min_elems,
-                              stream_stage_bytes, enable_fusion, disable_conc_fusion)
+                              stream_stage_bytes, disable_epi_fusion, disable_conc_fusion)
         need = C.c_size_t(0)
         self._check(self.lib.crown_workspace_bytes(arr, self.n_nodes, *self.in_chw, self.B_max, self.S_max,
                                                    C.byref(self.opts), C.byref(need)), None)
@@ -300,7 +300,7 @@ class CrownContext:
                                         _ptr(Wt_lo), D.data_ptr()), self.h)
 
     def gemm(self, A: torch.Tensor, W: torch.Tensor, scheme: int = 0) -> torch.Tensor:
-        """D[M,N] = A[M,K] . W[K,N] through the contraction kernel (scheme 0 = 3xTF32 tcgen05, 2 = FFMA)."""
+        """D[M,N] = A[M,K] . W[K,N] through the contraction kernel (scheme 0 = 3xTF32 tcgen05 CTA-pair tiles, 2 = FFMA)."""
         A, W = self._dev(A), self._dev(W)
         D = torch.empty(A.shape[0], W.shape[1], device=self.device)
         if scheme == 0:

@@ -27,33 +27,34 @@ extern "C" int crown_init(crown_ctx** out, const crown_node* nodes, int n_nodes,
   if (!out || !opts || !workspace_dev || B_max <= 0 || S_max < 0) return CROWN_EINVAL;
   *out = nullptr;
   crown_ctx* ctx = new crown_ctx();
+  // every failure below releases whatever was created so far through crown_destroy (streams, events, pinned buffers)
+  auto bail = [&](int code) { crown_destroy(ctx); return code; };
   ctx->opts = *opts;
-  if (ctx->opts.mma_scheme != 0 && ctx->opts.mma_scheme != 2) { delete ctx; return CROWN_EINVAL; }
-  if (ctx->opts.slope_rule < 0 || ctx->opts.slope_rule > 2) { delete ctx; return CROWN_EINVAL; }
-  int rc = analyse(nodes, n_nodes, in_c, in_h, in_w, ctx->nodes, ctx->err, ctx->has_add);
-  if (rc) { delete ctx; return rc; }
+  if (ctx->opts.mma_scheme != 0 && ctx->opts.mma_scheme != 2) return bail(CROWN_EINVAL);
+  if (ctx->opts.slope_rule < 0 || ctx->opts.slope_rule > 2) return bail(CROWN_EINVAL);
+  int rc = analyse(nodes, n_nodes, in_c, in_h, in_w, ctx->nodes, ctx->err, ctx->has_add, &ctx->input_consumers);
+  if (rc) return bail(rc);
   ctx->in_c = in_c; ctx->in_h = in_h; ctx->in_w = in_w; ctx->n0 = in_c * in_h * in_w;
   ctx->B_max = B_max; ctx->S_max = std::max(S_max, 1);
   ctx->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
   rc = make_plan(ctx->nodes, ctx->n0, B_max, ctx->S_max, ctx->opts, ctx->has_add, ctx->plan, ctx->err);
-  if (rc) { delete ctx; return rc; }
-  if (workspace_bytes < ctx->plan.total) { delete ctx; return CROWN_ENOMEM; }
+  if (rc) return bail(rc);
+  if (workspace_bytes < ctx->plan.total) return bail(CROWN_ENOMEM);
   int dev = 0;
   if (cudaGetDevice(&dev) != cudaSuccess ||
-      cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
-    delete ctx; return CROWN_ECUDA;
-  }
+      cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+    return bail(CROWN_ECUDA);
+  // kernel attributes (opt-in dynamic shared memory) are per device: set them for the device of this context
+  if (kernels_init_device() != 0) return bail(CROWN_ECUDA);
   // carve the workspace
   ctx->ws = reinterpret_cast<uint8_t*>(workspace_dev);
   ctx->ws_bytes = workspace_bytes;
   uint8_t* cur = reinterpret_cast<uint8_t*>(align_up(reinterpret_cast<size_t>(ctx->ws)));
   for (auto& ni : ctx->nodes) {
     ni.streamed = is_streamed(ni.n, ctx->opts);
-    if (ni.n.op == CROWN_LINEAR && !ni.streamed && !ni.n.W_dev) {
-      delete ctx; return CROWN_EINVAL;     // a layer without a resident copy must qualify for streaming
-    }
+    if (ni.n.op == CROWN_LINEAR && !ni.streamed && !ni.n.W_dev) return bail(CROWN_EINVAL);   // no resident copy: must stream
     if (ni.streamed) {
-      if (ctx->opts.mma_scheme != 0 || !gemm_tc_supported(128, ni.n.n_in, ni.n.n_out)) { delete ctx; return CROWN_EUNSUPPORTED; }
+      if (ctx->opts.mma_scheme != 0 || !gemm_tc_supported(128, ni.n.n_in, ni.n.n_out)) return bail(CROWN_EUNSUPPORTED);
       ni.tc_ok = true;
     } else if (wants_prepack(ni, ctx->opts)) {
       size_t sz = align_up((size_t)ni.n.n_in * ni.n.n_out * 4);
@@ -65,16 +66,17 @@ extern "C" int crown_init(crown_ctx** out, const crown_node* nodes, int n_nodes,
   if (ctx->plan.stage_bytes) {
     ctx->stage[0] = cur; cur += ctx->plan.stage_bytes;
     ctx->stage[1] = cur; cur += ctx->plan.stage_bytes;
-    if (cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking) != cudaSuccess) { delete ctx; return CROWN_ECUDA; }
+    if (cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking) != cudaSuccess) return bail(CROWN_ECUDA);
     for (int b = 0; b < 2; ++b)
       if (cudaEventCreateWithFlags(&ctx->ev_copied[b], cudaEventDisableTiming) != cudaSuccess ||
-          cudaEventCreateWithFlags(&ctx->ev_free[b], cudaEventDisableTiming) != cudaSuccess) { delete ctx; return CROWN_ECUDA; }
+          cudaEventCreateWithFlags(&ctx->ev_free[b], cudaEventDisableTiming) != cudaSuccess) return bail(CROWN_ECUDA);
   }
   ctx->coef_base = cur; ctx->coef_off.assign(n_nodes, 0);
-  { size_t off = 0; for (int i = 0; i < n_nodes; ++i) if (ctx->nodes[i].n.op == CROWN_RELU) { ctx->coef_off[i] = off; off += align_up((size_t)B_max * ctx->nodes[i].size * 32); } cur += ctx->plan.coef_bytes; }
+  { size_t off = 0; for (int i = 0; i < n_nodes; ++i) if (ctx->nodes[i].n.op == CROWN_RELU) { ctx->coef_off[i] = off; off += align_up((size_t)B_max * ctx->nodes[i].size * 16); } cur += ctx->plan.coef_bytes; }
   ctx->ibp_base = cur; ctx->ibp_off.assign(n_nodes, 0);
   { size_t off = 0; for (int i = 0; i < n_nodes; ++i) { ctx->ibp_off[i] = off; off += 2 * align_up((size_t)B_max * ctx->nodes[i].size * 4); } cur += ctx->plan.ibp_bytes; }
   ctx->d_buf = reinterpret_cast<float*>(cur); cur += ctx->plan.d_bytes;
+  ctx->part_buf = reinterpret_cast<float*>(cur); cur += ctx->plan.part_bytes;
   ctx->io_base = cur; cur += ctx->plan.io_bytes;
   ctx->pool_base = cur;
   ctx->pool_ref.assign(ctx->plan.nbuf, 0);
@@ -92,7 +94,7 @@ extern "C" int crown_init(crown_ctx** out, const crown_node* nodes, int n_nodes,
     const size_t bytes = (size_t)N * K * 4;
     if (cudaHostAlloc(reinterpret_cast<void**>(&ni.hWt_hi), bytes, cudaHostAllocDefault) != cudaSuccess ||
         cudaHostAlloc(reinterpret_cast<void**>(&ni.hWt_lo), bytes, cudaHostAllocDefault) != cudaSuccess) {
-      crown_destroy(ctx); return CROWN_ENOMEM;
+      return bail(CROWN_ENOMEM);
     }
     // stage[1] holds the raw column slab W[:, n0:n0+ns] as [K, ns]; stage[0] its transposed hi/lo parts [ns, K]
     const int ns_max = slab_rows(ctx->plan.stage_bytes, N, K, 2);
@@ -107,11 +109,10 @@ extern "C" int crown_init(crown_ctx** out, const crown_node* nodes, int n_nodes,
       cudaError_t e2 = cudaMemcpyAsync(ni.hWt_hi + (size_t)n0 * K, hi, (size_t)ns * K * 4, cudaMemcpyDeviceToHost, ctx->stream);
       cudaError_t e3 = cudaMemcpyAsync(ni.hWt_lo + (size_t)n0 * K, lo, (size_t)ns * K * 4, cudaMemcpyDeviceToHost, ctx->stream);
       cudaError_t e4 = cudaStreamSynchronize(ctx->stream);
-      if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess || e4 != cudaSuccess) { crown_destroy(ctx); return CROWN_ECUDA; }
+      if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess || e4 != cudaSuccess) return bail(CROWN_ECUDA);
     }
   }
-  cudaError_t e = cudaGetLastError();
-  if (e != cudaSuccess) { std::string m = cudaGetErrorString(e); delete ctx; (void)m; return CROWN_ECUDA; }
+  if (cudaGetLastError() != cudaSuccess) return bail(CROWN_ECUDA);
   *out = ctx;
   return CROWN_OK;
 }
@@ -287,6 +288,7 @@ extern "C" int ibp_forward(crown_ctx* ctx, int B, const float* x_lo_dev, const f
   const NodeInfo& ln = ctx->nodes[last];
   if (ln.n.op != CROWN_LINEAR) return fail(ctx, CROWN_EUNSUPPORTED, "ibp_forward: spec needs a final Linear node");
   if (S <= 0 || S > ctx->plan.rows_cap || !lb_dev || !ub_dev) return fail(ctx, CROWN_EINVAL, "ibp_forward: bad spec arguments");
+  if (ln.streamed || !ln.n.W_dev) return fail(ctx, CROWN_EUNSUPPORTED, "ibp_forward: the spec bound needs a resident last Linear layer");
   cudaStream_t s = ctx->stream;
   std::fill(ctx->pool_ref.begin(), ctx->pool_ref.end(), 0);
   const float *li, *ui;

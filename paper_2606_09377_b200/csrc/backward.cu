@@ -54,8 +54,47 @@ int contribute(Pass& ps, int idx, Pending p) {
 
 
 float4* coef_ptr(crown_ctx* ctx, int i) { return reinterpret_cast<float4*>(ctx->coef_base + ctx->coef_off[i]); }
-long long plane_stride(crown_ctx* ctx, int i) { return (long long)ctx->B_max * ctx->nodes[i].size; }
-float* planes_ptr(crown_ctx* ctx, int i) { return reinterpret_cast<float*>(coef_ptr(ctx, i) + plane_stride(ctx, i)); }
+
+// One contraction A.W_i on the tensor cores, resident or streamed (N-slabs of the prepacked operand from pinned host
+// memory, a7: slab s+1 -- or the next layer's first slab -- is copied on the side stream while slab s is multiplied).
+// mode 0: D = product; 1: a8 fused (conc partials into part_buf); 2: a4 fused (D = hi limb, D_lo = lo limb of the
+// relaxed product, d partials into part_buf).  The same rule picks the mode in both residency modes: bitwise equality.
+int tc_contract(crown_ctx* ctx, const NodeInfo& ni, const float* hi, const float* lo, float* D, float* D_lo, int M_full,
+                int mode, const ConcArgs* conc, const RelaxEpiArgs* rel) {
+  const int K = ni.n.n_out, N = ni.n.n_in;
+  cudaStream_t s = ctx->stream;
+  const char* e = nullptr;
+  const double out_bytes = mode == 1 ? 0.0 : (mode == 2 ? 8.0 : 4.0) * (double)M_full;
+  if (!ni.streamed) {
+    Scope sc(ctx, CROWN_K_GEMM_TC, 8.0 * (double)M_full * K + 8.0 * (double)K * N + out_bytes * N, 2.0 * M_full * (double)N * K);
+    if (launch_gemm_tc(hi, lo, ni.Wt_hi, ni.Wt_lo, D, N, M_full, N, K, ctx->opts.k_drain, ctx->num_sms, s, &e, conc, rel))
+      return fail(ctx, CROWN_ECUDA, std::string("gemm_tc: ") + (e ? e : "?"));
+    return CROWN_OK;
+  }
+  const int ns_max = slab_rows(ctx->plan.stage_bytes, N, K, 2);
+  const int nslabs = (N + ns_max - 1) / ns_max;
+  return stream_slabs(ctx, nslabs,
+    [&](int sl, uint8_t* dst, cudaStream_t cs) {
+      const int n0 = sl * ns_max, ns = std::min(ns_max, N - n0);
+      float* dhi = reinterpret_cast<float*>(dst);
+      ctx->h2d_bytes += 2.0 * ns * K * 4;
+      cudaError_t e1 = cudaMemcpyAsync(dhi, ni.hWt_hi + (size_t)n0 * K, (size_t)ns * K * 4, cudaMemcpyHostToDevice, cs);
+      if (e1 != cudaSuccess) return e1;
+      return cudaMemcpyAsync(dhi + (size_t)ns * K, ni.hWt_lo + (size_t)n0 * K, (size_t)ns * K * 4, cudaMemcpyHostToDevice, cs);
+    },
+    [&](int sl, uint8_t* src) {
+      const int n0 = sl * ns_max, ns = std::min(ns_max, N - n0);
+      const float* whi = reinterpret_cast<const float*>(src);
+      Scope sc(ctx, CROWN_K_GEMM_TC, 8.0 * (double)M_full * K + 8.0 * (double)K * ns + out_bytes * ns, 2.0 * M_full * (double)ns * K);
+      ConcArgs ca; RelaxEpiArgs ra;
+      if (conc) { ca = *conc; ca.col_off = n0; }
+      if (rel) { ra = *rel; ra.col_off = n0; ra.out_lo = D_lo + n0; }
+      if (launch_gemm_tc(hi, lo, whi, whi + (size_t)ns * K, D ? D + n0 : nullptr, N, M_full, ns, K, ctx->opts.k_drain,
+                         ctx->num_sms, s, &e, conc ? &ca : nullptr, rel ? &ra : nullptr))
+        return fail(ctx, CROWN_ECUDA, std::string("gemm_tc: ") + (e ? e : "?"));
+      return (int)CROWN_OK;
+    });
+}
 
 // One backward pass.  coef_ready: per node, 1 if coef_ptr(i) already holds the coefficients of ReLU i for the
 // bounds in l_dev/u_dev (crown_run computes each ReLU's coefficients once); may be nullptr.
@@ -70,9 +109,18 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
   if (lb && (!ub || !x_lo || !x_hi)) return fail(ctx, CROWN_EINVAL, "crown_backward: concretisation needs ub, x_lo, x_hi");
   std::fill(ctx->pool_ref.begin(), ctx->pool_ref.end(), 0);
   Pass ps; ps.ctx = ctx; ps.B = B; ps.R = R;
-  float* conc_part = nullptr; int conc_parts = 0, conc_buf = -1;
+  bool conc_done = false; int conc_parts = 0;
   const NodeInfo& sn = ctx->nodes[start];
   int first = start;   // first node to visit in the reverse sweep
+  auto ensure_coef = [&](int i) -> int {
+    if (!l_dev || !u_dev || !l_dev[i] || !u_dev[i]) return fail(ctx, CROWN_EINVAL, "crown_backward: bounds of a ReLU below start are missing");
+    if (!coef_ready || !(*coef_ready)[i]) {
+      Scope sc(ctx, CROWN_K_COEFF, 24.0 * B * ctx->nodes[i].size);
+      launch_relax_coeffs(l_dev[i], u_dev[i], coef_ptr(ctx, i), (long long)B * ctx->nodes[i].size, ctx->opts.slope_rule, s);
+      if (coef_ready) (*coef_ready)[i] = 1;
+    }
+    return CROWN_OK;
+  };
   if (C_dev) {
     { Scope sc(ctx, CROWN_K_MISC); launch_init_d(ctx->d_buf, nullptr, 0, B, R, s); }
     Pending p; p.v.p = C_dev; p.v.ld = sn.size; p.v.n = sn.size; p.v.sB = (long long)R * sn.size; p.v.sBr = 0;
@@ -107,66 +155,11 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
     int rc = CROWN_OK;
     switch (nd.op) {
       case CROWN_RELU: {
-        if (!l_dev || !u_dev || !l_dev[i] || !u_dev[i]) return fail(ctx, CROWN_EINVAL, "crown_backward: bounds of a ReLU below start are missing");
-        if (!coef_ready || !(*coef_ready)[i]) {
-          Scope sc(ctx, CROWN_K_COEFF, 24.0 * B * ni.size);
-          launch_relax_coeffs(l_dev[i], u_dev[i], coef_ptr(ctx, i), planes_ptr(ctx, i), plane_stride(ctx, i), (long long)B * ni.size,
-                              ctx->opts.slope_rule, s);
-          if (coef_ready) (*coef_ready)[i] = 1;
-        }
+        if ((rc = ensure_coef(i))) return rc;
         const int j = nd.in0;
         const bool lin_below = j >= 0 && (ctx->nodes[j].n.op == CROWN_LINEAR || ctx->nodes[j].n.op == CROWN_CONV2D);
         // the product that follows runs on the tensor cores when the producer is a prepacked Linear
         const bool tc = lin_below && ctx->nodes[j].tc_ok && (ctx->nodes[j].streamed || gemm_tc_supported(2 * B * R, ctx->nodes[j].n.n_in, ctx->nodes[j].n.n_out));
-        // fused path: relaxation + bias accumulation + split + contraction in one kernel (gemm_fused.cu); needs a
-        // resident prepacked Linear below with this ReLU as its only consumer and fixed-rule slopes (no alpha)
-        if (tc && ctx->opts.enable_fusion && ctx->nodes[j].n.op == CROWN_LINEAR &&
-            ctx->nodes[j].n_consumers == 1 && ps.pend.find(j) == ps.pend.end() &&
-            !(alpha_lo && alpha_lo[i]) && !(alpha_up && alpha_up[i]) &&
-            gemm_fused_supported(cur.v, B, R, ctx->nodes[j].n.n_in, ctx->nodes[j].n.n_out)) {
-          const NodeInfo& nj = ctx->nodes[j];
-          const int Kf = nj.n.n_out, Nf = nj.n.n_in;
-          const int M_full = 2 * B * R;
-          Pending outp;
-          float* D = nullptr;
-          outp.buf = new_buf(ps, D);
-          if (outp.buf < 0) return fail(ctx, CROWN_ENOMEM, "backward: A-buffer pool exhausted");
-          const char* e = nullptr;
-          if (nj.streamed) {
-            // N-slabs of the prepacked operand from pinned host memory (a7); d is accumulated by the first slab only
-            const int ns_max = slab_rows(ctx->plan.stage_bytes, Nf, Kf, 2);
-            const int nslabs = (Nf + ns_max - 1) / ns_max;
-            int rc2 = stream_slabs(ctx, nslabs,
-              [&](int sl, uint8_t* dst, cudaStream_t cs) {
-                const int n0 = sl * ns_max, ns = std::min(ns_max, Nf - n0);
-                float* dhi = reinterpret_cast<float*>(dst);
-                ctx->h2d_bytes += 2.0 * ns * Kf * 4;
-                cudaError_t e1 = cudaMemcpyAsync(dhi, nj.hWt_hi + (size_t)n0 * Kf, (size_t)ns * Kf * 4, cudaMemcpyHostToDevice, cs);
-                if (e1 != cudaSuccess) return e1;
-                return cudaMemcpyAsync(dhi + (size_t)ns * Kf, nj.hWt_lo + (size_t)n0 * Kf, (size_t)ns * Kf * 4, cudaMemcpyHostToDevice, cs);
-              },
-              [&](int sl, uint8_t* src) {
-                const int n0 = sl * ns_max, ns = std::min(ns_max, Nf - n0);
-                const float* whi = reinterpret_cast<const float*>(src);
-                Scope sc(ctx, CROWN_K_GEMM_TC, 4.0 * ((double)M_full * Kf + 2.0 * Kf * ns + (double)M_full * ns), 2.0 * M_full * (double)ns * Kf);
-                if (launch_gemm_fused(cur.v, B, R, planes_ptr(ctx, i), plane_stride(ctx, i), nj.n.b_dev, sl == 0 ? ctx->d_buf : nullptr, whi,
-                                      whi + (size_t)ns * Kf, D + n0, Nf, ns, Kf, ctx->opts.k_drain, ctx->num_sms, s, &e))
-                  return fail(ctx, CROWN_ECUDA, std::string("gemm_fused: ") + (e ? e : "?"));
-                return (int)CROWN_OK;
-              });
-            if (rc2) return rc2;
-          } else {
-            Scope sc(ctx, CROWN_K_GEMM_TC, 4.0 * ((double)M_full * Kf + 2.0 * Kf * Nf + (double)M_full * Nf), 2.0 * M_full * (double)Nf * Kf);
-            if (launch_gemm_fused(cur.v, B, R, planes_ptr(ctx, i), plane_stride(ctx, i), nj.n.b_dev, ctx->d_buf, nj.Wt_hi, nj.Wt_lo, D, Nf, Nf, Kf,
-                                  ctx->opts.k_drain, ctx->num_sms, s, &e))
-              return fail(ctx, CROWN_ECUDA, std::string("gemm_fused: ") + (e ? e : "?"));
-          }
-          ctx->gemm_flops += 2.0 * M_full * (double)Nf * Kf;
-          outp.v = canon_view(D, B, R, Nf);
-          release(ctx, cur);
-          rc = contribute(ps, nj.n.in0, outp);
-          break;
-        }
         RelaxArgs ra;
         ra.A = cur.v; ra.coef = coef_ptr(ctx, i);
         ra.alpha_lo = alpha_lo ? alpha_lo[i] : nullptr;
@@ -179,8 +172,12 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
         if (out.buf < 0) return fail(ctx, CROWN_ENOMEM, "backward: A-buffer pool exhausted");
         ra.out_lo = nullptr;
         if (tc) { out.buf_lo = new_buf(ps, ra.out_lo); if (out.buf_lo < 0) return fail(ctx, CROWN_ENOMEM, "backward: A-buffer pool exhausted"); }
-        const double elems = 2.0 * B * R * ni.size;
-        { Scope sc(ctx, CROWN_K_RELAX, elems * (tc ? 12.0 : 8.0) + ((ra.alpha_lo || ra.alpha_up) ? 4.0 * B * R * ni.size : 0.0));
+        // algorithmic bytes: every DISTINCT input row is read once (at the start of a pass all branches / properties
+        // share the R rows of W_k), every output row is written once (+ the lo limb), alpha once per (row, neuron)
+        const double in_rows = (double)(cur.v.sBr ? 2 : 1) * (cur.v.sB ? B : 1) * R;
+        const double out_rows = 2.0 * B * R;
+        { Scope sc(ctx, CROWN_K_RELAX, 4.0 * ni.size * (in_rows + out_rows * (tc ? 2.0 : 1.0)) +
+                                       ((ra.alpha_lo || ra.alpha_up) ? 4.0 * B * R * ni.size : 0.0));
           launch_relax(ra, s); }
         out.v = canon_view(ra.out, B, R, ni.size); out.v.lo = ra.out_lo;
         out.bias_done_for = lin_below ? j : -2;
@@ -200,77 +197,65 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
             ra.d = nullptr; ra.B = B; ra.R = R; ra.n = ni.size;
             tmp.buf = new_buf(ps, ra.out); tmp.buf_lo = new_buf(ps, ra.out_lo);
             if (tmp.buf < 0 || tmp.buf_lo < 0) return fail(ctx, CROWN_ENOMEM, "backward: A-buffer pool exhausted");
-            { Scope sc(ctx, CROWN_K_RELAX, 12.0 * M_full * ni.size); launch_relax(ra, s); }
+            const double in_rows = (double)(cur.v.sBr ? 2 : 1) * (cur.v.sB ? B : 1) * R;
+            { Scope sc(ctx, CROWN_K_RELAX, 4.0 * ni.size * (in_rows + 2.0 * M_full)); launch_relax(ra, s); }
             hi = ra.out; lo = ra.out_lo;
             release(ctx, cur); cur = tmp;
           }
-          out.buf = new_buf(ps, D);
-          if (out.buf < 0) return fail(ctx, CROWN_ENOMEM, "backward: A-buffer pool exhausted");
-          const char* e = nullptr;
-          if (ni.streamed) {
-            // N-slabs of the prepacked operand Wt [n_in, n_out] from pinned host memory (a7); slab s+1 (or the
-            // next layer's first slab) is copied on the side stream while slab s is multiplied
-            const int K = nd.n_out, N = nd.n_in;
-            const int ns_max = slab_rows(ctx->plan.stage_bytes, N, K, 2);
-            const int nslabs = (N + ns_max - 1) / ns_max;
-            // same rule as the resident path (bitwise equality of the two modes): concretise in the epilogue
-            const bool fc = nd.in0 < 0 && lb && !A_dev && ps.pend.find(-1) == ps.pend.end() && !ctx->opts.disable_conc_fusion &&
-                            gemm_tc_conc_supported(M_full, N, K) && (size_t)M_full * gemm_tc_conc_parts(N) * 8 <= ctx->plan.buf_bytes &&
-                            (ns_max % 128 == 0 || nslabs == 1);
-            int rc2 = stream_slabs(ctx, nslabs,
-              [&](int sl, uint8_t* dst, cudaStream_t cs) {
-                const int n0 = sl * ns_max, ns = std::min(ns_max, N - n0);
-                float* dhi = reinterpret_cast<float*>(dst);
-                ctx->h2d_bytes += 2.0 * ns * K * 4;
-                cudaError_t e1 = cudaMemcpyAsync(dhi, ni.hWt_hi + (size_t)n0 * K, (size_t)ns * K * 4, cudaMemcpyHostToDevice, cs);
-                if (e1 != cudaSuccess) return e1;
-                return cudaMemcpyAsync(dhi + (size_t)ns * K, ni.hWt_lo + (size_t)n0 * K, (size_t)ns * K * 4, cudaMemcpyHostToDevice, cs);
-              },
-              [&](int sl, uint8_t* src) {
-                const int n0 = sl * ns_max, ns = std::min(ns_max, N - n0);
-                const float* whi = reinterpret_cast<const float*>(src);
-                Scope sc(ctx, CROWN_K_GEMM_TC, 4.0 * ((double)M_full * K + (double)K * ns + (double)M_full * ns), 2.0 * M_full * (double)ns * K);
-                ConcArgs ca;
-                if (fc) { ca.x_lo = x_lo; ca.x_hi = x_hi; ca.part = D; ca.B = B; ca.R = R; ca.parts = gemm_tc_conc_parts(N);
-                          ca.ldx = N; ca.col_off = n0; ca.piece0 = 2 * (n0 / 128); }
-                if (launch_gemm_tc(hi, lo, whi, whi + (size_t)ns * K, fc ? nullptr : D + n0, N, M_full, ns, K, ctx->opts.k_drain,
-                                   ctx->num_sms, s, &e, fc ? &ca : nullptr))
-                  return fail(ctx, CROWN_ECUDA, std::string("gemm_tc: ") + (e ? e : "?"));
-                return (int)CROWN_OK;
-              });
-            if (rc2) return rc2;
-            if (fc) {
-              conc_part = D; conc_parts = gemm_tc_conc_parts(N); conc_buf = out.buf;
-              ctx->gemm_flops += 2.0 * M_full * (double)N * K;
-              release(ctx, cur);
-              break;
-            }
-          } else if (nd.in0 < 0 && lb && !A_dev && ps.pend.find(-1) == ps.pend.end() && !ctx->opts.disable_conc_fusion &&
-                     gemm_tc_conc_supported(M_full, nd.n_in, nd.n_out) &&
-                     (size_t)M_full * gemm_tc_conc_parts(nd.n_in) * 8 <= ctx->plan.buf_bytes) {
-            // last contraction of the pass: concretise in its epilogue (a8 fused), A_0 never reaches HBM
+          const int K = nd.n_out, N = nd.n_in;
+          const int parts = gemm_tc_parts(N);
+          const bool single = gemm_tc_single_panel(K) != 0;
+          // a8 fused: the last contraction of the pass concretises in its epilogue, A_0 never reaches HBM
+          const bool fc = nd.in0 < 0 && lb && !A_dev && ctx->input_consumers == 1 && ps.pend.find(-1) == ps.pend.end() &&
+                          !ctx->opts.disable_conc_fusion && single && (size_t)M_full * parts * 8 <= ctx->plan.part_bytes;
+          // a4 fused: the product feeds a ReLU (only consumer: this layer) over a tensor-core Linear, fixed-rule slopes:
+          // the epilogue applies that relaxation and emits the next operand's limbs (A <- A.Lambda W as one kernel)
+          int r = nd.in0, j = -1;
+          bool fr = false;
+          if (!fc && r >= 0 && ctx->nodes[r].n.op == CROWN_RELU && ctx->nodes[r].n_consumers == 1 &&
+              ps.pend.find(r) == ps.pend.end() && !ctx->opts.disable_epi_fusion && single &&
+              !(alpha_lo && alpha_lo[r]) && !(alpha_up && alpha_up[r]) && (size_t)M_full * parts * 4 <= ctx->plan.part_bytes) {
+            j = ctx->nodes[r].n.in0;
+            fr = j >= 0 && ctx->nodes[j].n.op == CROWN_LINEAR && ctx->nodes[j].tc_ok &&
+                 (ctx->nodes[j].streamed || gemm_tc_supported(M_full, ctx->nodes[j].n.n_in, ctx->nodes[j].n.n_out));
+          }
+          if (fc) {
             ConcArgs ca;
-            ca.x_lo = x_lo; ca.x_hi = x_hi; ca.part = D; ca.B = B; ca.R = R; ca.parts = gemm_tc_conc_parts(nd.n_in); ca.ldx = nd.n_in;
-            Scope sc(ctx, CROWN_K_GEMM_TC, 4.0 * (2.0 * M_full * nd.n_out + 2.0 * nd.n_out * nd.n_in), 2.0 * M_full * (double)nd.n_in * nd.n_out);
-            if (launch_gemm_tc(hi, lo, ni.Wt_hi, ni.Wt_lo, nullptr, nd.n_in, M_full, nd.n_in, nd.n_out, ctx->opts.k_drain, ctx->num_sms, s, &e, &ca))
-              return fail(ctx, CROWN_ECUDA, std::string("gemm_tc: ") + (e ? e : "?"));
-            conc_part = D; conc_parts = ca.parts; conc_buf = out.buf;
-            ctx->gemm_flops += 2.0 * M_full * (double)nd.n_in * nd.n_out;
+            ca.x_lo = x_lo; ca.x_hi = x_hi; ca.part = ctx->part_buf; ca.B = B; ca.R = R; ca.parts = parts; ca.ldx = N;
+            if ((rc = tc_contract(ctx, ni, hi, lo, nullptr, nullptr, M_full, 1, &ca, nullptr))) return rc;
+            conc_done = true; conc_parts = parts;
+            ctx->gemm_flops += 2.0 * M_full * (double)N * K;
             release(ctx, cur);
             break;                      // nothing is contributed to the input node: the bound is finished below
-          } else {
-            Scope sc(ctx, CROWN_K_GEMM_TC, 4.0 * ((double)M_full * nd.n_out + (double)nd.n_out * nd.n_in + (double)M_full * nd.n_in),
-                     2.0 * M_full * (double)nd.n_in * nd.n_out);
-            if (launch_gemm_tc(hi, lo, ni.Wt_hi, ni.Wt_lo, D, nd.n_in, M_full, nd.n_in, nd.n_out, ctx->opts.k_drain, ctx->num_sms, s, &e))
-              return fail(ctx, CROWN_ECUDA, std::string("gemm_tc: ") + (e ? e : "?"));
           }
-          ctx->gemm_flops += 2.0 * M_full * (double)nd.n_in * nd.n_out;
-          out.v = canon_view(D, B, R, nd.n_in);
+          out.buf = new_buf(ps, D);
+          if (out.buf < 0) return fail(ctx, CROWN_ENOMEM, "backward: A-buffer pool exhausted");
+          if (fr) {
+            if ((rc = ensure_coef(r))) return rc;
+            float* D_lo = nullptr;
+            out.buf_lo = new_buf(ps, D_lo);
+            if (out.buf_lo < 0) return fail(ctx, CROWN_ENOMEM, "backward: A-buffer pool exhausted");
+            RelaxEpiArgs re;
+            re.coef = coef_ptr(ctx, r); re.coef_ld = N; re.bias = ctx->nodes[j].n.b_dev; re.out_lo = D_lo;
+            re.part = ctx->part_buf; re.B = B; re.R = R; re.parts = parts;
+            if ((rc = tc_contract(ctx, ni, hi, lo, D, D_lo, M_full, 2, nullptr, &re))) return rc;
+            { Scope sc(ctx, CROWN_K_MISC, 4.0 * M_full * parts); launch_reduce_parts(ctx->part_buf, parts, ctx->d_buf, M_full, s); }
+            ctx->gemm_flops += 2.0 * M_full * (double)N * K;
+            out.v = canon_view(D, B, R, N); out.v.lo = D_lo;
+            out.bias_done_for = j;
+            release(ctx, cur);
+            rc = contribute(ps, j, out);      // ReLU r is done: the relaxed product is A w.r.t. node j's output
+            break;
+          }
+          if ((rc = tc_contract(ctx, ni, hi, lo, D, nullptr, M_full, 0, nullptr, nullptr))) return rc;
+          ctx->gemm_flops += 2.0 * M_full * (double)N * K;
+          out.v = canon_view(D, B, R, N);
         } else {
           // CUDA-core contraction; rows shared between branches / properties are multiplied once
           int m_eff = 0;
-          if (ni.streamed) return fail(ctx, CROWN_EUNSUPPORTED, "backward: a streamed layer needs M = 2*B*rows >= 128 (tensor-core path)");
+          if (ni.streamed) return fail(ctx, CROWN_EUNSUPPORTED, "backward: a streamed layer needs the tensor-core path");
           if (!view_uniform(cur.v, B, R, m_eff)) return fail(ctx, CROWN_EINVAL, "backward: non-uniform A view");
+          if (cur.v.lo) return fail(ctx, CROWN_EINVAL, "backward: split operand on the CUDA-core path");
           out.buf = new_buf(ps, D);
           if (out.buf < 0) return fail(ctx, CROWN_ENOMEM, "backward: A-buffer pool exhausted");
           { Scope sc(ctx, CROWN_K_GEMM_FFMA, 4.0 * ((double)m_eff * nd.n_out + (double)nd.n_out * nd.n_in + (double)m_eff * nd.n_in),
@@ -313,11 +298,10 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
     }
     if (rc) return rc;
   }
-  if (conc_part) {   // the bound was concretised inside the last contraction
+  if (conc_done) {   // the bound was concretised inside the last contraction
     if (d_dev) CK(ctx, cudaMemcpyAsync(d_dev, ctx->d_buf, (size_t)2 * B * R * 4, cudaMemcpyDeviceToDevice, s));
     { Scope sc(ctx, CROWN_K_CONCRETIZE, 8.0 * 2 * B * R * conc_parts);
-      launch_concretize_parts(conc_part, conc_parts, ctx->d_buf, lb, ub, out_stride, B, R, s); }
-    pool_release(ctx, conc_buf);
+      launch_concretize_parts(ctx->part_buf, conc_parts, ctx->d_buf, lb, ub, out_stride, B, R, s); }
     CK(ctx, cudaGetLastError());
     return CROWN_OK;
   }
@@ -484,15 +468,6 @@ extern "C" int crown_gemm(crown_ctx* ctx, int scheme, int M, int N, int K, const
     const char* e = nullptr;
     Scope sc(ctx, CROWN_K_GEMM_TC, 4.0 * ((double)M * K + (double)K * N + (double)M * N), 2.0 * M * (double)N * K);
     if (launch_gemm_tc(A_hi_dev, A_lo_dev, Wt_hi_dev, Wt_lo_dev, D_dev, N, M, N, K, ctx->opts.k_drain, ctx->num_sms, ctx->stream, &e))
-      return fail(ctx, CROWN_EINVAL, std::string("crown_gemm: ") + (e ? e : "?"));
-  } else if (scheme == 1) {
-    // fused kernel in split-only mode: A_hi_dev is the RAW fp32 A [M,K]; the TF32 split happens inside the kernel
-    const char* e = nullptr;
-    AView v = canon_view(A_hi_dev, 1, M / 2, K);
-    if (M % 2) return fail(ctx, CROWN_EINVAL, "crown_gemm: scheme 1 needs an even M");
-    Scope sc(ctx, CROWN_K_GEMM_TC, 4.0 * ((double)M * K + 2.0 * K * N + (double)M * N), 2.0 * M * (double)N * K);
-    if (launch_gemm_fused(v, 1, M / 2, nullptr, 0, nullptr, nullptr, Wt_hi_dev, Wt_lo_dev, D_dev, N, N, K, ctx->opts.k_drain,
-                          ctx->num_sms, ctx->stream, &e))
       return fail(ctx, CROWN_EINVAL, std::string("crown_gemm: ") + (e ? e : "?"));
   } else if (scheme == 2) {
     // FFMA path takes W [K,N] row-major in Wt_hi_dev (NOT transposed) and fp32 A in A_hi_dev

@@ -135,7 +135,8 @@ struct ConvBwdGeom {
   int stage_floats;                     // floats per pipeline stage (filters + A tiles)
 };
 
-constexpr int kConvFillMax = 6;         // tile elements per thread (tile <= 6 * blockDim)
+constexpr int kConvFillMax = 6;
+constexpr size_t kConvBwdSmemBudget = 96 * 1024;         // tile elements per thread (tile <= 6 * blockDim)
 
 __device__ __forceinline__ void cp_async4(float* dst_smem, const float* src) {
   const uint32_t d = static_cast<uint32_t>(__cvta_generic_to_shared(dst_smem));
@@ -319,7 +320,7 @@ static bool launch_conv_bwd_tiled(const AView& A, const float* W, const float* a
   const int threads = ((g.PT * g.CG * g.RB + 31) / 32) * 32;
   if (g.PH * g.PW > kConvFillMax * threads) return false;
   const int cgct = g.CG * CT;
-  const size_t budget = 96 * 1024;                       // two stages; two blocks per SM still fit
+  const size_t budget = kConvBwdSmemBudget;              // two stages; two blocks per SM still fit
   const size_t per_co = ((size_t)KH * KW * cgct + (size_t)g.RB * g.PH * g.PW) * sizeof(float);
   int coc = (int)(budget / 2 / per_co);
   if (coc < 1) return false;
@@ -328,12 +329,6 @@ static bool launch_conv_bwd_tiled(const AView& A, const float* W, const float* a
   g.stage_floats = (int)(per_co * coc / sizeof(float));
   g.stage_floats = (g.stage_floats + 3) / 4 * 4;
   const size_t smem = (size_t)2 * g.stage_floats * sizeof(float);
-  static bool attr = false;
-  if (!attr) {
-    if (cudaFuncSetAttribute(conv_bwd_tiled_kernel<KH, KW, S, CT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)budget + 64) != cudaSuccess) return false;
-    attr = true;
-  }
   const long long rows = 2LL * B * R;
   dim3 grid((unsigned)((rows + g.RB - 1) / g.RB), (unsigned)((groups + g.CG - 1) / g.CG));
   conv_bwd_tiled_kernel<KH, KW, S, CT><<<grid, threads, smem, s>>>(A.p, A.sBr, A.sB, A.ld, B, R, W, addend, out, g);
@@ -346,6 +341,18 @@ static bool launch_conv_bwd_ct(const AView& A, const float* W, const float* adde
   if (c_in % 16 == 0) return launch_conv_bwd_tiled<KH, KW, S, 16>(A, W, addend, out, B, R, c_in, h, w, c_out, pad, ho, wo, s);
   if (c_in > 4) return launch_conv_bwd_tiled<KH, KW, S, 8>(A, W, addend, out, B, R, c_in, h, w, c_out, pad, ho, wo, s);
   return launch_conv_bwd_tiled<KH, KW, S, 4>(A, W, addend, out, B, R, c_in, h, w, c_out, pad, ho, wo, s);
+}
+
+template <int KH, int KW, int S>
+static bool conv_bwd_set_attr() {
+  const int bytes = (int)kConvBwdSmemBudget + 64;
+  return cudaFuncSetAttribute(conv_bwd_tiled_kernel<KH, KW, S, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) == cudaSuccess &&
+         cudaFuncSetAttribute(conv_bwd_tiled_kernel<KH, KW, S, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) == cudaSuccess &&
+         cudaFuncSetAttribute(conv_bwd_tiled_kernel<KH, KW, S, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) == cudaSuccess;
+}
+int conv_init_device() {
+  return (conv_bwd_set_attr<3, 3, 1>() && conv_bwd_set_attr<3, 3, 2>() && conv_bwd_set_attr<1, 1, 1>() &&
+          conv_bwd_set_attr<1, 1, 2>()) ? 0 : -1;
 }
 
 void launch_conv_transpose(const AView& A, const float* W, const float* addend, float* out, int B, int R,

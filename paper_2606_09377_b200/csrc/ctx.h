@@ -35,6 +35,7 @@ struct NodeInfo {
 struct Plan {
   size_t prepack_bytes = 0, coef_bytes = 0, ibp_bytes = 0, d_bytes = 0, io_bytes = 0;
   size_t buf_bytes = 0;
+  size_t part_bytes = 0;  // per-(row, 32-column piece) partial sums of the fused epilogues (a4 / a8 fused)
   size_t stage_bytes = 0; // one of the two weight-streaming staging buffers (0: nothing is streamed)
   int nbuf = 0;
   int rc = 0;             // row chunk for identity passes
@@ -49,6 +50,7 @@ struct TimingRec { cudaEvent_t a, b; int cls; double bytes, flops; };
 struct crown_ctx {
   std::vector<NodeInfo> nodes;
   int in_c = 0, in_h = 0, in_w = 0, n0 = 0;
+  int input_consumers = 0;   // nodes that read the network input; the fused concretisation needs exactly one
   int B_max = 0, S_max = 0;
   crown_opts opts{};
   cudaStream_t stream = nullptr;
@@ -60,6 +62,7 @@ struct crown_ctx {
   uint8_t* coef_base = nullptr; std::vector<size_t> coef_off;   // per node (ReLU only)
   uint8_t* ibp_base = nullptr;  std::vector<size_t> ibp_off;    // per node: l then u
   float* d_buf = nullptr;
+  float* part_buf = nullptr;
   uint8_t* io_base = nullptr;
   uint8_t* pool_base = nullptr;
   std::vector<int> pool_ref;
@@ -97,10 +100,11 @@ size_t align_up(size_t x, size_t a = 1024) { return (x + a - 1) / a * a; }
 
 // ---- graph analysis ---------------------------------------------------------------------------
 int analyse(const crown_node* nodes, int n_nodes, int in_c, int in_h, int in_w,
-            std::vector<NodeInfo>& out, std::string& err, bool& has_add) {
+            std::vector<NodeInfo>& out, std::string& err, bool& has_add, int* input_consumers = nullptr) {
   if (!nodes || n_nodes <= 0 || in_c <= 0 || in_h <= 0 || in_w <= 0) { err = "bad network description"; return CROWN_EINVAL; }
   out.assign(n_nodes, NodeInfo());
   has_add = false;
+  int in_cons = 0;     // consumers of the network input (node -1): a skip connection from x makes it > 1
   auto shape_of = [&](int idx, int& c, int& h, int& w) {
     if (idx < 0) { c = in_c; h = in_h; w = in_w; } else { c = out[idx].c; h = out[idx].h; w = out[idx].w; }
   };
@@ -139,9 +143,10 @@ int analyse(const crown_node* nodes, int n_nodes, int in_c, int in_h, int in_w,
         err = "unsupported op"; return CROWN_EUNSUPPORTED;
     }
     ni.size = ni.c * ni.h * ni.w;
-    if (n.in0 >= 0) out[n.in0].n_consumers++;
-    if (n.op == CROWN_ADD && n.in1 >= 0) out[n.in1].n_consumers++;
+    if (n.in0 >= 0) out[n.in0].n_consumers++; else ++in_cons;
+    if (n.op == CROWN_ADD) { if (n.in1 >= 0) out[n.in1].n_consumers++; else ++in_cons; }
   }
+  if (input_consumers) *input_consumers = in_cons;
   return CROWN_OK;
 }
 
@@ -171,7 +176,10 @@ int make_plan(const std::vector<NodeInfo>& nodes, int n0, int B, int S, const cr
               Plan& p, std::string& err) {
   p = Plan();
   int nmax = n0, max_start = 1;
+  bool any_epi = false;
   for (const auto& ni : nodes) {
+    if (ni.n.op == CROWN_LINEAR && o.mma_scheme == 0 && !o.disable_epi_fusion && gemm_tc_supported(128, ni.n.n_in, ni.n.n_out) &&
+        gemm_tc_single_panel(ni.n.n_out)) any_epi = true;
     nmax = std::max(nmax, ni.size);
     if (ni.n.op == CROWN_LINEAR && ni.n.in0 >= 0) max_start = std::max(max_start, ni.size);
     if (is_streamed(ni.n, o)) {
@@ -180,14 +188,17 @@ int make_plan(const std::vector<NodeInfo>& nodes, int n0, int B, int S, const cr
       size_t full = (size_t)2 * ni.n.n_in * ni.n.n_out * 4;
       p.stage_bytes = std::max(p.stage_bytes, std::max(need, std::min(full, o.stream_stage_bytes ? (size_t)o.stream_stage_bytes : kStageBytesMax)));
     } else if (wants_prepack(ni, o)) p.prepack_bytes += 2 * align_up((size_t)ni.n.n_in * ni.n.n_out * 4);
-    if (ni.n.op == CROWN_RELU) p.coef_bytes += align_up((size_t)B * ni.size * 32);   // float4 records + 3 SoA planes
+    if (ni.n.op == CROWN_RELU) p.coef_bytes += align_up((size_t)B * ni.size * 16);   // float4 records {dU, bU, dL, unstable}
     p.ibp_bytes += 2 * align_up((size_t)B * ni.size * 4);
     if (ni.n.op == CROWN_RELU) p.io_bytes += align_up((size_t)B * S * ni.size * 4) + 2 * align_up((size_t)B * ni.size * 4);
   }
   p.io_bytes += 2 * align_up((size_t)B * n0 * 4) + align_up((size_t)B * S * nodes.back().size * 4) +
                 2 * align_up((size_t)B * S * 4) + align_up((size_t)B);
-  p.nbuf = has_add ? 8 : 3;
+  // live A buffers of a chain: operand hi + lo and the product; when the product's epilogue also emits the next
+  // operand's hi + lo limbs (a4 fused, single-K-panel layers) one more
+  p.nbuf = has_add ? 8 : (any_epi ? 4 : 3);
   size_t per_row = (size_t)2 * B * nmax * 4;            // bytes of one start-spec row in one buffer
+  const size_t per_row_part = (size_t)2 * B * ((nmax + 31) / 32) * 8;
   p.stage_bytes = align_up(p.stage_bytes);
   size_t fixed = p.prepack_bytes + p.coef_bytes + p.ibp_bytes + p.io_bytes + 2 * p.stage_bytes;
   int rc = max_start;
@@ -195,7 +206,7 @@ int make_plan(const std::vector<NodeInfo>& nodes, int n0, int B, int S, const cr
     size_t d_est = align_up((size_t)2 * B * std::max(max_start, S) * 4);
     if (o.mem_cap_bytes <= fixed + d_est) { err = "mem_cap_bytes below the fixed footprint"; return CROWN_ENOMEM; }
     size_t avail = o.mem_cap_bytes - fixed - d_est;
-    size_t fit = avail / ((size_t)p.nbuf * per_row);
+    size_t fit = avail / ((size_t)p.nbuf * per_row + per_row_part);
     if (fit < (size_t)std::max(1, S)) { err = "mem_cap_bytes too small for one row chunk"; return CROWN_ENOMEM; }
     if (fit < (size_t)rc) rc = (int)fit;
     if (rc < max_start && rc > 64) rc = rc / 64 * 64;
@@ -204,7 +215,8 @@ int make_plan(const std::vector<NodeInfo>& nodes, int n0, int B, int S, const cr
   p.rows_cap = std::max(rc, S);
   p.d_bytes = align_up((size_t)2 * B * p.rows_cap * 4);
   p.buf_bytes = align_up((size_t)p.rows_cap * per_row);
-  p.total = fixed + p.d_bytes + (size_t)p.nbuf * p.buf_bytes;
+  p.part_bytes = align_up((size_t)p.rows_cap * per_row_part);
+  p.total = fixed + p.d_bytes + p.part_bytes + (size_t)p.nbuf * p.buf_bytes;
   return CROWN_OK;
 }
 

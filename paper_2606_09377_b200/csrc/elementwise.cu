@@ -11,8 +11,7 @@ namespace crownb200 {
 // (reading G3); adaptive rule lambda = 1 iff u > -l (reading G4).
 // ------------------------------------------------------------------------------------------------
 __global__ void relax_coeffs_kernel(const float* __restrict__ l, const float* __restrict__ u,
-                                    float4* __restrict__ coef, float* __restrict__ planes, long long plane_stride,
-                                    long long count, int rule) {
+                                    float4* __restrict__ coef, long long count, int rule) {
   long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= count) return;
   float lo = l[i], hi = u[i];
@@ -29,17 +28,12 @@ __global__ void relax_coeffs_kernel(const float* __restrict__ l, const float* __
     c = make_float4(dU, bU, dL, 1.f);
   }
   coef[i] = c;
-  // the same coefficients as planes {dU, bU, dL} for 128-bit loads along the neuron axis (gemm_fused.cu)
-  planes[i] = c.x;
-  planes[plane_stride + i] = c.y;
-  planes[2 * plane_stride + i] = c.z;
 }
 
-void launch_relax_coeffs(const float* l, const float* u, float4* coef, float* planes, long long plane_stride,
-                         long long count, int rule, cudaStream_t s) {
+void launch_relax_coeffs(const float* l, const float* u, float4* coef, long long count, int rule, cudaStream_t s) {
   if (count <= 0) return;
   int threads = 256;
-  relax_coeffs_kernel<<<ceil_div(count, threads), threads, 0, s>>>(l, u, coef, planes, plane_stride, count, rule);
+  relax_coeffs_kernel<<<ceil_div(count, threads), threads, 0, s>>>(l, u, coef, count, rule);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -283,6 +277,21 @@ void launch_concretize_parts(const float* part, int parts, const float* d, float
                                                              out_stride, B, R);
 }
 
+// d[m] += sum_i part[m*parts + i], i ascending: the per-piece d contributions written by the relaxing epilogue of the
+// contraction (a4 fused).  One thread per row; fixed order, so the result does not depend on the tiling.
+__global__ void reduce_parts_kernel(const float* __restrict__ part, int parts, float* __restrict__ d, long long rows) {
+  const long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (m >= rows) return;
+  const float* p = part + m * parts;
+  float acc = 0.f;
+  for (int i = 0; i < parts; ++i) acc += p[i];
+  d[m] += acc;
+}
+void launch_reduce_parts(const float* part, int parts, float* d, long long rows, cudaStream_t s) {
+  if (rows <= 0 || parts <= 0) return;
+  reduce_parts_kernel<<<ceil_div(rows, 128), 128, 0, s>>>(part, parts, d, rows);
+}
+
 // ------------------------------------------------------------------------------------------------
 // helpers
 // ------------------------------------------------------------------------------------------------
@@ -299,8 +308,8 @@ void launch_init_d(float* d, const float* bias, int row0, int B, int R, cudaStre
   init_d_kernel<<<ceil_div(tot, 256), 256, 0, s>>>(d, bias, row0, B, R);
 }
 
-__global__ void __launch_bounds__(256) rowdot_bias_kernel(const float* __restrict__ A, long long sBr,
-                                                          long long sB, long long ld, int n,
+__global__ void __launch_bounds__(256) rowdot_bias_kernel(const float* __restrict__ A, const float* __restrict__ Alo,
+                                                          long long sBr, long long sB, long long ld, int n,
                                                           const float* __restrict__ bias, int bias_div,
                                                           float* d, int B, int R) {
   const int lane = threadIdx.x & 31;
@@ -310,9 +319,15 @@ __global__ void __launch_bounds__(256) rowdot_bias_kernel(const float* __restric
   int br = (int)(m / BR);
   long long pair = m % BR;
   int b = (int)(pair / R), r = (int)(pair % R);
-  const float* a = A + br * sBr + (long long)b * sB + (long long)r * ld;
+  const long long off = br * sBr + (long long)b * sB + (long long)r * ld;
+  const float* a = A + off;
   float acc = 0.f;
-  for (int j = lane; j < n; j += 32) acc = fmaf(a[j], bias[j / bias_div], acc);
+  if (Alo) {            // view carries a TF32 lo limb: the value is hi + lo
+    const float* al = Alo + off;
+    for (int j = lane; j < n; j += 32) acc = fmaf(a[j] + al[j], bias[j / bias_div], acc);
+  } else {
+    for (int j = lane; j < n; j += 32) acc = fmaf(a[j], bias[j / bias_div], acc);
+  }
   acc = warp_sum(acc);
   if (lane == 0) d[m] += acc;
 }
@@ -320,33 +335,45 @@ void launch_rowdot_bias(const AView& A, const float* bias, int bias_div, float* 
                         cudaStream_t s) {
   long long rows = 2LL * B * R;
   if (rows <= 0 || !bias) return;
-  rowdot_bias_kernel<<<ceil_div(rows * 32, 256), 256, 0, s>>>(A.p, A.sBr, A.sB, A.ld, A.n, bias,
+  rowdot_bias_kernel<<<ceil_div(rows * 32, 256), 256, 0, s>>>(A.p, A.lo, A.sBr, A.sB, A.ld, A.n, bias,
                                                              bias_div > 0 ? bias_div : 1, d, B, R);
 }
 
 // out[m, :] = a[m, :] (+ b[m, :]) for the 2*B*R rows of two strided views; blockIdx.y = row, threads walk the row
 // with 128-bit accesses when everything is 16-byte aligned (no per-element index arithmetic).
 template <int VEC>
-__global__ void __launch_bounds__(256) view_add_kernel(const float* __restrict__ a, long long aBr, long long aB, long long ald,
-                                                       const float* __restrict__ b2, long long bBr, long long bB, long long bld,
+__global__ void __launch_bounds__(256) view_add_kernel(const float* __restrict__ a, const float* __restrict__ a_lo,
+                                                       long long aBr, long long aB, long long ald,
+                                                       const float* __restrict__ b2, const float* __restrict__ b_lo,
+                                                       long long bBr, long long bB, long long bld,
                                                        float* __restrict__ out, int B, int R, int n, long long row_base) {
   const long long m = row_base + blockIdx.y;
   const int r = (int)(m % R);
   const long long t = m / R;
   const int b = (int)(t % B), br = (int)(t / B);
-  const float* pa = a + br * aBr + b * aB + (long long)r * ald;
-  const float* pb = b2 ? b2 + br * bBr + b * bB + (long long)r * bld : nullptr;
+  const long long offa = br * aBr + b * aB + (long long)r * ald;
+  const long long offb = br * bBr + b * bB + (long long)r * bld;
+  const float* pa = a + offa;
+  const float* pal = a_lo ? a_lo + offa : nullptr;        // TF32 lo limbs: the value of a view is hi + lo
+  const float* pb = b2 ? b2 + offb : nullptr;
+  const float* pbl = (b2 && b_lo) ? b_lo + offb : nullptr;
   float* po = out + m * (long long)n;
   if (VEC == 4) {
     for (int j = (blockIdx.x * blockDim.x + threadIdx.x) * 4; j < n; j += gridDim.x * blockDim.x * 4) {
       float4 v = ldg_stream4(pa + j);
-      if (pb) { const float4 w = ldg_stream4(pb + j); v.x += w.x; v.y += w.y; v.z += w.z; v.w += w.w; }
+      if (pal) { const float4 w = ldg_stream4(pal + j); v.x += w.x; v.y += w.y; v.z += w.z; v.w += w.w; }
+      if (pb) {
+        float4 w = ldg_stream4(pb + j);
+        if (pbl) { const float4 w2 = ldg_stream4(pbl + j); w.x += w2.x; w.y += w2.y; w.z += w2.z; w.w += w2.w; }
+        v.x += w.x; v.y += w.y; v.z += w.z; v.w += w.w;
+      }
       stg_stream4(po + j, v);
     }
   } else {
     for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += gridDim.x * blockDim.x) {
       float v = pa[j];
-      if (pb) v += pb[j];
+      if (pal) v += pal[j];
+      if (pb) v += pbl ? pb[j] + pbl[j] : pb[j];
       po[j] = v;
     }
   }
@@ -355,7 +382,7 @@ void launch_view_add(const AView& a, const AView* b, float* out, int B, int R, c
   const long long rows = 2LL * B * R;
   if (rows <= 0 || a.n <= 0) return;
   auto al16 = [](const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; };
-  auto view_ok = [&](const AView& v) { return al16(v.p) && v.ld % 4 == 0 && v.sB % 4 == 0 && v.sBr % 4 == 0; };
+  auto view_ok = [&](const AView& v) { return al16(v.p) && (!v.lo || al16(v.lo)) && v.ld % 4 == 0 && v.sB % 4 == 0 && v.sBr % 4 == 0; };
   const bool vec = a.n % 4 == 0 && al16(out) && view_ok(a) && (!b || view_ok(*b));
   const int per = vec ? 1024 : 256;                       // elements per block pass
   int gx = ceil_div(a.n, per);
@@ -363,19 +390,20 @@ void launch_view_add(const AView& a, const AView* b, float* out, int B, int R, c
   for (long long r0 = 0; r0 < rows; r0 += 65535) {        // gridDim.y limit
     const int ny = (int)(rows - r0 < 65535 ? rows - r0 : 65535);
     dim3 grid(gx, ny);
-    if (vec) view_add_kernel<4><<<grid, 256, 0, s>>>(a.p, a.sBr, a.sB, a.ld, b ? b->p : nullptr, b ? b->sBr : 0, b ? b->sB : 0,
-                                                   b ? b->ld : 0, out, B, R, a.n, r0);
-    else view_add_kernel<1><<<grid, 256, 0, s>>>(a.p, a.sBr, a.sB, a.ld, b ? b->p : nullptr, b ? b->sBr : 0, b ? b->sB : 0,
-                                                b ? b->ld : 0, out, B, R, a.n, r0);
+    if (vec) view_add_kernel<4><<<grid, 256, 0, s>>>(a.p, a.lo, a.sBr, a.sB, a.ld, b ? b->p : nullptr, b ? b->lo : nullptr,
+                                                   b ? b->sBr : 0, b ? b->sB : 0, b ? b->ld : 0, out, B, R, a.n, r0);
+    else view_add_kernel<1><<<grid, 256, 0, s>>>(a.p, a.lo, a.sBr, a.sB, a.ld, b ? b->p : nullptr, b ? b->lo : nullptr,
+                                                b ? b->sBr : 0, b ? b->sB : 0, b ? b->ld : 0, out, B, R, a.n, r0);
   }
 }
 
 __global__ void verdict_kernel(const float* __restrict__ lb, uint8_t* __restrict__ v, int B, int S) {
   int b = blockIdx.x * blockDim.x + threadIdx.x;
   if (b >= B) return;
-  float m = INFINITY;
-  for (int s = 0; s < S; ++s) m = fminf(m, lb[(long long)b * S + s]);
-  v[b] = (m > 0.f) ? 1 : 0;
+  // fail closed: a NaN lower bound compares false, so the property is NOT verified (fminf would drop the NaN)
+  bool ok = S > 0;
+  for (int s = 0; s < S; ++s) ok = ok && (lb[(long long)b * S + s] > 0.f);
+  v[b] = ok ? 1 : 0;
 }
 void launch_verdict(const float* lb, uint8_t* verified, int B, int S, cudaStream_t s) {
   if (B <= 0) return;

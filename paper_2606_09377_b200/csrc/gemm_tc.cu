@@ -2,23 +2,31 @@
 // on the 5th-generation tensor cores, fp32-accurate via 3xTF32:
 //     D = A_hi.W_hi + A_hi.W_lo + A_lo.W_hi          (a = a_hi + a_lo, both exactly TF32-representable)
 // The dropped A_lo.W_lo term and the TF32 rounding of the lo parts are O(2^-22) relative per product.
+// The epilogue optionally applies the NEXT step of the recursion, so that `A <- A.Lambda_i W_i` is one kernel:
+//   a4 fused: relaxation of the product through the ReLU below (sign split, slopes, d += A-/+ . bU, d += Abar . b)
+//             and the TF32 hi/lo split of Abar, which is written as the next contraction's operand;
+//   a8 fused: concretisation of the product against the input box (the last contraction of a pass).
 //
-// Design (sm_100a):
-//   * operands K-major in global memory: A_hi/A_lo [M,K], Wt_hi/Wt_lo [N,K] (weights are transposed and
-//     split once at crown_init); TMA (cp.async.bulk.tensor, 128B swizzle) stages 4 operand tiles per
-//     pipeline stage into shared memory; one elected thread issues tcgen05.mma.kind::tf32 (UMMA 128 x BN x 8)
-//     with the accumulator in TMEM;
-//   * warp roles: warp 0 TMA producer, warp 1 MMA issuer, warp 2 TMEM allocator, warps 4-11 epilogue
-//     (two warps per TMEM lane quadrant, 64 columns each, one tcgen05.ld.32x32b.x64 per drain);
-//   * measured on B200: the tensor core's fp32 accumulation truncates, ~0.5 ulp of the running sum per MMA,
-//     so the error grows linearly with the length of an accumulation chain.  Two measures keep the result at
-//     CUDA-core FFMA accuracy: (1) two accumulators in TMEM, "big" for hi.hi and "small" for lo.hi + hi.lo
-//     (2^-11 of big), so big sees one MMA per k-step and small's truncation is 2^-11 smaller; (2) K is cut into
-//     drain chunks of k_drain elements (default 128 = 16 MMAs on big): each chunk of big is accumulated in
-//     TMEM, then added into an fp32 register running sum by the epilogue warps (round-to-nearest) while the
-//     tensor core fills the other buffer; small is drained every 16384 elements of K.  All four accumulators
-//     (big/small x double buffer) use the full 512 TMEM columns;
-//   * persistent grid (one CTA per SM), static tile order grouped along M for L2 reuse of W.
+// Design (sm_100a), round 2: a CTA PAIR per output tile (tcgen05 cta_group::2).
+//   * Round 1's 128x128 single-CTA tile moved 64 KB of operand limbs from L2 into shared memory per 768 tensor
+//     cycles (83 B/cycle/SM); its three measured operating points (cfg2 165, cfg3 192, cfg4 153 useful TFLOP/s)
+//     all sit at 10-12 TB/s of L2->SM traffic, the chip's L2 throughput.  A pair tile of
+//     256 x BN (BN <= 256): each CTA stages ITS 128 rows of A and HALF of the W tile (BN/2 rows), one UMMA
+//     256 x BN x 8 reads both halves, so the same 64 KB per stage feed twice the tensor work (32 flop/B).
+//   * operands K-major in global memory: A_hi/A_lo [M,K], Wt_hi/Wt_lo [N,K] (weights transposed and split once at
+//     crown_init); TMA (cp.async.bulk.tensor, 128B swizzle) stages 4 tiles per pipeline stage; both CTAs' loads
+//     signal the LEADER CTA's full barrier; one thread of the leader issues tcgen05.mma.cta_group::2.kind::tf32 and
+//     releases stages / publishes accumulators with multicast commits to both CTAs;
+//   * warp roles per CTA: warp 0 TMA producer, warp 1 MMA issuer (leader CTA only), warp 2 TMEM allocator, warps 4-11
+//     epilogue (two warps per TMEM lane quadrant, 128 columns each).  setmaxnreg moves registers from warps 0-3 to
+//     the epilogue warps, which keep a 128-column fp32 running sum per thread;
+//   * measured on B200 (round 1): the tensor core's fp32 accumulation truncates, ~0.5 ulp of the running sum per MMA,
+//     so the error grows linearly with the length of an accumulation chain.  K is therefore cut into drain chunks of
+//     k_drain elements (default 64 = 24 MMAs): each chunk is accumulated in TMEM (two 256-column buffers = all 512
+//     columns), then added into the fp32 register running sum by the epilogue warps (round-to-nearest) while the
+//     tensor core fills the other buffer;
+//   * persistent grid (one CTA pair per TPC), static tile order grouped along M for L2 reuse of W; K is cut into
+//     panels whose per-wave working set fits L2, later panels add into D with the TMA's fp32 reduce-add.
 #include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -32,237 +40,289 @@ namespace crownb200 {
 
 namespace tc {
 
+constexpr int PAIR_M = 2 * BM;                       // rows of a pair tile
+constexpr int BN_MAX = 256;
+constexpr int STAGES = 3;
+constexpr int A_BYTES = BM * BK * 4;                 // 16 KB: one limb of this CTA's 128 rows
+constexpr int B_BYTES = (BN_MAX / 2) * BK * 4;       // 16 KB: one limb of this CTA's half of the W tile
+constexpr int STAGE_BYTES = 2 * A_BYTES + 2 * B_BYTES;
+constexpr int EPI_WARPS = 8;                         // 4 lane quadrants x 2 column halves of 128
+constexpr int EC = 128;                              // columns owned by one epilogue warp
+constexpr int THREADS = 128 + EPI_WARPS * 32;
+constexpr int TMEM_COLS = 512;                       // two accumulator buffers of 256 columns
+constexpr int EPI_STAGE_BYTES = EPI_WARPS * 4096;    // one 32 x 32 fp32 slab per epilogue warp (TMA store)
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + EPI_STAGE_BYTES + 1024 /*align slack*/ + 256 /*barriers*/;
 
-template <int BN>
-struct Cfg {
-  static constexpr int STAGES = (BN == 128) ? 3 : 2;
-  static constexpr int A_BYTES = BM * BK * 4;
-  static constexpr int B_BYTES = BN * BK * 4;
-  static constexpr int STAGE_BYTES = 2 * A_BYTES + 2 * B_BYTES;
-  static constexpr int EPI_WARPS = 8;                // 4 lane quadrants x 2 column halves of BN/2
-  static constexpr int EPI_COLS = BN / 2;            // columns drained by one epilogue warp
-  static constexpr int THREADS = 128 + EPI_WARPS * 32;
-  static constexpr int TMEM_COLS = 4 * BN;           // {big, small} accumulators, each double-buffered
-  static constexpr int EPI_STAGE_BYTES = EPI_WARPS * 4096;   // one 32 x 32 fp32 slab per epilogue warp (TMA store)
-  static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + EPI_STAGE_BYTES + 1024 /*align slack*/ + 256 /*barriers*/;
+enum { EPI_STORE = 0, EPI_ADD = 1, EPI_RELAX = 2, EPI_CONC = 3 };
+
+struct EpiArgs {
+  int mode = EPI_STORE;
+  int B = 0, R = 0;              // row m -> branch m / (B*R), property (m / R) % B
+  int col_off = 0;               // first column of this launch inside the full row (N-slab of a streamed operand)
+  int parts = 0;                 // 32-column pieces per full row
+  float* part = nullptr;         // EPI_RELAX: [M, parts] floats; EPI_CONC: [M, parts] float2
+  // EPI_RELAX
+  const float4* coef = nullptr;  // [B, coef_ld] {dU, bU, dL, unstable}
+  long long coef_ld = 0;
+  const float* bias = nullptr;   // bias of the Linear below the ReLU, [coef_ld], or nullptr
+  // EPI_CONC
+  const float* x_lo = nullptr; const float* x_hi = nullptr; int ldx = 0;
 };
 
-template <int BN>
-__global__ void __launch_bounds__(Cfg<BN>::THREADS, 1)
-gemm_tf32x3_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant__ CUtensorMap tmA_lo,
-                   const __grid_constant__ CUtensorMap tmB_hi, const __grid_constant__ CUtensorMap tmB_lo,
-                   const __grid_constant__ CUtensorMap tmD, int M, int N, int K, int kb_per_chunk,
-                   int chunks_per_small, int accumulate, const ConcArgs conc) {
-  using C = Cfg<BN>;
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(THREADS, 1)
+gemm2_tf32x3_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant__ CUtensorMap tmA_lo,
+                    const __grid_constant__ CUtensorMap tmB_hi, const __grid_constant__ CUtensorMap tmB_lo,
+                    const __grid_constant__ CUtensorMap tmD, const __grid_constant__ CUtensorMap tmD_lo,
+                    int M, int N, int K, int BN, int kb_per_chunk, const EpiArgs ea) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t raw = smem_u32(smem_raw);
   const uint32_t base = (raw + 1023u) & ~1023u;
-  const uint32_t epi_base = base + C::STAGES * C::STAGE_BYTES;           // 1024-aligned: swizzled store slabs
-  const uint32_t bar_base = epi_base + C::EPI_STAGE_BYTES;
-  // barriers: full[STAGES], empty[STAGES], bfull[2], bempty[2] (big accumulator), sfull[2], sempty[2] (small
-  // accumulator); then the TMEM base address slot
+  const uint32_t epi_base = base + STAGES * STAGE_BYTES;           // 1024-aligned: swizzled store slabs
+  const uint32_t bar_base = epi_base + EPI_STAGE_BYTES;
+  // barriers (same offsets in both CTAs): full[STAGES] (leader's is used), empty[STAGES], accfull[2],
+  // accempty[2] (leader's is used); then the TMEM base address slot
   auto full_bar = [&](int s) { return bar_base + 8u * s; };
-  auto empty_bar = [&](int s) { return bar_base + 8u * (C::STAGES + s); };
-  auto bfull_bar = [&](int b) { return bar_base + 8u * (2 * C::STAGES + b); };
-  auto bempty_bar = [&](int b) { return bar_base + 8u * (2 * C::STAGES + 2 + b); };
-  auto sfull_bar = [&](int b) { return bar_base + 8u * (2 * C::STAGES + 4 + b); };
-  auto sempty_bar = [&](int b) { return bar_base + 8u * (2 * C::STAGES + 6 + b); };
-  const uint32_t tmem_slot = bar_base + 8u * (2 * C::STAGES + 8);
-  volatile uint32_t* tmem_slot_ptr =
-      reinterpret_cast<volatile uint32_t*>(smem_raw + (tmem_slot - raw));
+  auto empty_bar = [&](int s) { return bar_base + 8u * (STAGES + s); };
+  auto accfull_bar = [&](int b) { return bar_base + 8u * (2 * STAGES + b); };
+  auto accempty_bar = [&](int b) { return bar_base + 8u * (2 * STAGES + 2 + b); };
+  const uint32_t tmem_slot = bar_base + 8u * (2 * STAGES + 4);
+  volatile uint32_t* tmem_slot_ptr = reinterpret_cast<volatile uint32_t*>(smem_raw + (tmem_slot - raw));
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int m_tiles = (M + BM - 1) / BM, n_tiles = (N + BN - 1) / BN;
+  const uint32_t rank = cluster_ctarank();             // 0 = leader
+  const int cluster_id = blockIdx.x >> 1, num_clusters = gridDim.x >> 1;
+  const int m_tiles = (M + PAIR_M - 1) / PAIR_M, n_tiles = (N + BN - 1) / BN;
   const int num_tiles = m_tiles * n_tiles;
   const int num_kb = (K + BK - 1) / BK;
   const int num_chunks = (num_kb + kb_per_chunk - 1) / kb_per_chunk;
+  const int bh = BN >> 1;                              // rows of W this CTA stages
 
   if (warp == 0 && lane == 0) {
     prefetch_tmap(&tmA_hi); prefetch_tmap(&tmA_lo); prefetch_tmap(&tmB_hi); prefetch_tmap(&tmB_lo);
   }
   if (warp == 1 && lane == 0) {
-    for (int s = 0; s < C::STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-    for (int b = 0; b < 2; ++b) {
-      mbar_init(bfull_bar(b), 1); mbar_init(bempty_bar(b), C::EPI_WARPS);
-      mbar_init(sfull_bar(b), 1); mbar_init(sempty_bar(b), C::EPI_WARPS);
-    }
+    for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+    for (int b = 0; b < 2; ++b) { mbar_init(accfull_bar(b), 1); mbar_init(accempty_bar(b), 2 * EPI_WARPS); }
     fence_barrier_init();
   }
   if (warp == 2) {
-    tmem_alloc(tmem_slot, C::TMEM_COLS);
-    tmem_relinquish();
+    tmem_alloc_pair(tmem_slot, TMEM_COLS);
+    tmem_relinquish_pair();
   }
   tcgen05_fence_before();
   __syncthreads();
+  cluster_sync_all();          // both CTAs' barriers are initialised before any remote arrive / multicast commit
   tcgen05_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
-  // TMEM columns: big[b] at b*BN, small[b] at 2*BN + b*BN
 
-  if (warp == 0) {
-    // ===================== TMA producer =====================
-    if (lane == 0) {
-      int stage = 0; uint32_t parity = 0;
-      for (int t = blockIdx.x; t < num_tiles; t += gridDim.x) {
-        int mb, nb; tile_coords(t, m_tiles, n_tiles, mb, nb);
-        const int m0 = mb * BM, n0 = nb * BN;
-        for (int kb = 0; kb < num_kb; ++kb) {
-          mbar_wait(empty_bar(stage), parity ^ 1u);
-          const uint32_t sA_hi = base + stage * C::STAGE_BYTES;
-          const uint32_t sA_lo = sA_hi + C::A_BYTES;
-          const uint32_t sB_hi = sA_lo + C::A_BYTES;
-          const uint32_t sB_lo = sB_hi + C::B_BYTES;
-          mbar_expect_tx(full_bar(stage), C::STAGE_BYTES);
-          tma_load_2d(sA_hi, &tmA_hi, kb * BK, m0, full_bar(stage));
-          tma_load_2d(sA_lo, &tmA_lo, kb * BK, m0, full_bar(stage));
-          tma_load_2d(sB_hi, &tmB_hi, kb * BK, n0, full_bar(stage));
-          tma_load_2d(sB_lo, &tmB_lo, kb * BK, n0, full_bar(stage));
-          if (++stage == C::STAGES) { stage = 0; parity ^= 1u; }
+  if (warp < 4) {
+    setmaxnreg_dec<56>();
+    if (warp == 0) {
+      // ===================== TMA producer (both CTAs) =====================
+      if (lane == 0) {
+        int stage = 0; uint32_t parity = 0;
+        const uint32_t stage_tx = 2u * (2u * A_BYTES + 2u * (uint32_t)bh * BK * 4u);   // both CTAs' bytes
+        for (int t = cluster_id; t < num_tiles; t += num_clusters) {
+          int mb, nb; tile_coords(t, m_tiles, n_tiles, mb, nb);
+          const int m0 = mb * PAIR_M + (int)rank * BM, n0 = nb * BN + (int)rank * bh;
+          for (int kb = 0; kb < num_kb; ++kb) {
+            mbar_wait(empty_bar(stage), parity ^ 1u);
+            const uint32_t sA_hi = base + stage * STAGE_BYTES;
+            const uint32_t sA_lo = sA_hi + A_BYTES;
+            const uint32_t sB_hi = sA_lo + A_BYTES;
+            const uint32_t sB_lo = sB_hi + B_BYTES;
+            const uint32_t fb = mapa_cluster(full_bar(stage), 0);
+            if (rank == 0) mbar_expect_tx(full_bar(stage), stage_tx);
+            tma_load_2d_pair(sA_hi, &tmA_hi, kb * BK, m0, fb);
+            tma_load_2d_pair(sA_lo, &tmA_lo, kb * BK, m0, fb);
+            tma_load_2d_pair(sB_hi, &tmB_hi, kb * BK, n0, fb);
+            tma_load_2d_pair(sB_lo, &tmB_lo, kb * BK, n0, fb);
+            if (++stage == STAGES) { stage = 0; parity ^= 1u; }
+          }
         }
       }
-    }
-  } else if (warp == 1) {
-    // ===================== MMA issuer =====================
-    // Two accumulators of different magnitude: "big" takes hi.hi (one MMA per k-step, drained to the CUDA-core
-    // running sum every chunk), "small" takes lo.hi + hi.lo (2^-11 of big; drained every chunks_per_small chunks).
-    // The tensor core's fp32 accumulation truncates, ~0.5 ulp of the accumulator per MMA: keeping the two apart
-    // means big sees a third of the MMAs and small's truncation is 2^-11 smaller in absolute terms.
-    if (lane == 0) {
-      constexpr uint32_t idesc = make_idesc_tf32(BM, BN);
-      int stage = 0; uint32_t parity = 0;
-      uint32_t big_cnt = 0, small_cnt = 0;
-      for (int t = blockIdx.x; t < num_tiles; t += gridDim.x) {
-        uint32_t acc_small = 0;
-        for (int c = 0; c < num_chunks; ++c) {
-          const uint32_t bbuf = big_cnt & 1u, sbuf = small_cnt & 1u;
-          mbar_wait(bempty_bar(bbuf), ((big_cnt >> 1) & 1u) ^ 1u);
-          if (acc_small == 0) mbar_wait(sempty_bar(sbuf), ((small_cnt >> 1) & 1u) ^ 1u);
-          tcgen05_fence_after();
-          const uint32_t tmem_big = tmem_base + bbuf * BN;
-          const uint32_t tmem_small = tmem_base + 2 * BN + sbuf * BN;
-          const int kb_end = min(num_kb, (c + 1) * kb_per_chunk);
-          uint32_t acc_big = 0;
-          for (int kb = c * kb_per_chunk; kb < kb_end; ++kb) {
-            mbar_wait(full_bar(stage), parity);
+    } else if (warp == 1 && rank == 0) {
+      // ===================== MMA issuer (leader CTA) =====================
+      if (lane == 0) {
+        const uint32_t idesc = make_idesc_tf32(PAIR_M, BN);
+        int stage = 0; uint32_t parity = 0;
+        uint32_t cnt = 0;
+        for (int t = cluster_id; t < num_tiles; t += num_clusters) {
+          for (int c = 0; c < num_chunks; ++c) {
+            const uint32_t buf = cnt & 1u;
+            mbar_wait(accempty_bar(buf), ((cnt >> 1) & 1u) ^ 1u);
             tcgen05_fence_after();
-            const uint32_t sA_hi = base + stage * C::STAGE_BYTES;
-            const uint32_t sA_lo = sA_hi + C::A_BYTES;
-            const uint32_t sB_hi = sA_lo + C::A_BYTES;
-            const uint32_t sB_lo = sB_hi + C::B_BYTES;
+            const uint32_t tmem_d = tmem_base + buf * BN_MAX;
+            const int kb_end = min(num_kb, (c + 1) * kb_per_chunk);
+            uint32_t acc = 0;
+            for (int kb = c * kb_per_chunk; kb < kb_end; ++kb) {
+              mbar_wait(full_bar(stage), parity);
+              tcgen05_fence_after();
+              const uint32_t sA_hi = base + stage * STAGE_BYTES;
+              const uint32_t sA_lo = sA_hi + A_BYTES;
+              const uint32_t sB_hi = sA_lo + A_BYTES;
+              const uint32_t sB_lo = sB_hi + B_BYTES;
 #pragma unroll
-            for (int k = 0; k < BK / UMMA_K; ++k) {
-              const uint32_t koff = k * UMMA_K * 4;  // bytes inside the 128 B swizzle row
-              const uint64_t dA_hi = make_kmajor_sw128_desc(sA_hi + koff);
-              const uint64_t dA_lo = make_kmajor_sw128_desc(sA_lo + koff);
-              const uint64_t dB_hi = make_kmajor_sw128_desc(sB_hi + koff);
-              const uint64_t dB_lo = make_kmajor_sw128_desc(sB_lo + koff);
-              umma_tf32(tmem_small, dA_lo, dB_hi, idesc, acc_small);
-              umma_tf32(tmem_small, dA_hi, dB_lo, idesc, 1u);
-              umma_tf32(tmem_big, dA_hi, dB_hi, idesc, acc_big);
-              acc_small = 1u; acc_big = 1u;
+              for (int k = 0; k < BK / UMMA_K; ++k) {
+                const uint32_t koff = k * UMMA_K * 4;  // bytes inside the 128 B swizzle row
+                const uint64_t dA_hi = make_kmajor_sw128_desc(sA_hi + koff);
+                const uint64_t dA_lo = make_kmajor_sw128_desc(sA_lo + koff);
+                const uint64_t dB_hi = make_kmajor_sw128_desc(sB_hi + koff);
+                const uint64_t dB_lo = make_kmajor_sw128_desc(sB_lo + koff);
+                umma_tf32_pair(tmem_d, dA_lo, dB_hi, idesc, acc);      // the two small products first
+                umma_tf32_pair(tmem_d, dA_hi, dB_lo, idesc, 1u);
+                umma_tf32_pair(tmem_d, dA_hi, dB_hi, idesc, 1u);
+                acc = 1u;
+              }
+              umma_commit_pair(empty_bar(stage), 3);   // frees the stage in both CTAs once these MMAs have read it
+              if (++stage == STAGES) { stage = 0; parity ^= 1u; }
             }
-            umma_commit(empty_bar(stage));   // frees the smem stage once these MMAs have read it
-            if (++stage == C::STAGES) { stage = 0; parity ^= 1u; }
-          }
-          umma_commit(bfull_bar(bbuf));      // big chunk complete
-          ++big_cnt;
-          if ((c + 1) % chunks_per_small == 0 || c == num_chunks - 1) {
-            umma_commit(sfull_bar(sbuf));    // small accumulator complete
-            ++small_cnt; acc_small = 0;
+            umma_commit_pair(accfull_bar(buf), 3);     // chunk complete: both CTAs' epilogues may drain
+            ++cnt;
           }
         }
       }
     }
-  } else if (warp >= 4) {
-    // ===================== epilogue: TMEM -> fp32 running sum -> global =====================
+  } else {
+    // ===================== epilogue: TMEM -> fp32 running sum -> fused step -> global =====================
+    setmaxnreg_inc<224>();
     const int ew = warp - 4;
     const int quad = warp & 3;               // TMEM lane quadrant this warp may access
-    const int chalf = ew >> 2;               // which half of the BN columns
-    constexpr int EC = C::EPI_COLS;
-    uint32_t big_cnt = 0, small_cnt = 0;
-    for (int t = blockIdx.x; t < num_tiles; t += gridDim.x) {
+    const int chalf = ew >> 2;               // which 128 of the (up to) 256 tile columns
+    const uint32_t accempty_remote[2] = {mapa_cluster(accempty_bar(0), 0), mapa_cluster(accempty_bar(1), 0)};
+    const uint32_t slab_base = epi_base + (uint32_t)ew * 4096u;
+    const uint32_t slab = slab_base + (uint32_t)lane * 128u;
+    const uint32_t sw = (uint32_t)(lane & 7);
+    const long long BR = (long long)ea.B * ea.R;
+    uint32_t cnt = 0;
+    for (int t = cluster_id; t < num_tiles; t += num_clusters) {
       int mb, nb; tile_coords(t, m_tiles, n_tiles, mb, nb);
       float acc[EC];
 #pragma unroll
       for (int i = 0; i < EC; ++i) acc[i] = 0.f;
       for (int c = 0; c < num_chunks; ++c) {
-        {
-          const uint32_t buf = big_cnt & 1u;
-          mbar_wait(bfull_bar(buf), (big_cnt >> 1) & 1u);
-          tcgen05_fence_after();
-          const uint32_t taddr = tmem_base + ((uint32_t)(quad * 32) << 16) + buf * BN + chalf * EC;
-          static_assert(EC == 64, "epilogue drains 64 columns per warp");
-          uint32_t v[64];
-          tmem_ld64(taddr, v);
-          tmem_ld_wait();
+        const uint32_t buf = cnt & 1u;
+        mbar_wait(accfull_bar(buf), (cnt >> 1) & 1u);
+        tcgen05_fence_after();
+        const uint32_t taddr = tmem_base + ((uint32_t)(quad * 32) << 16) + buf * BN_MAX + chalf * EC;
 #pragma unroll
-          for (int i = 0; i < 64; ++i) acc[i] += __uint_as_float(v[i]);
-          tcgen05_fence_before();
-          __syncwarp();
-          if (lane == 0) mbar_arrive(bempty_bar(buf));
-          ++big_cnt;
-        }
-        if ((c + 1) % chunks_per_small == 0 || c == num_chunks - 1) {
-          const uint32_t buf = small_cnt & 1u;
-          mbar_wait(sfull_bar(buf), (small_cnt >> 1) & 1u);
-          tcgen05_fence_after();
-          const uint32_t taddr = tmem_base + ((uint32_t)(quad * 32) << 16) + 2 * BN + buf * BN + chalf * EC;
-          static_assert(EC == 64, "epilogue drains 64 columns per warp");
-          uint32_t v[64];
-          tmem_ld64(taddr, v);
-          tmem_ld_wait();
+        for (int h = 0; h < EC / 32; ++h) {
+          if (chalf * EC + h * 32 < BN) {      // warp-uniform
+            uint32_t v[32];
+            tmem_ld32(taddr + h * 32, v);
+            tmem_ld_wait();
 #pragma unroll
-          for (int i = 0; i < 64; ++i) acc[i] += __uint_as_float(v[i]);
-          tcgen05_fence_before();
-          __syncwarp();
-          if (lane == 0) mbar_arrive(sempty_bar(buf));
-          ++small_cnt;
+            for (int i = 0; i < 32; ++i) acc[h * 32 + i] += __uint_as_float(v[i]);
+          }
         }
+        tcgen05_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cluster(accempty_remote[buf]);
+        ++cnt;
       }
-      if (conc.part != nullptr) {
-        // a8 fused: this warp's 64 columns of row `row` against the box of the row's property; A_0 is never stored
-        const int row = mb * BM + quad * 32 + lane;
-        const int col0 = nb * BN + chalf * EC;
+      const int row = mb * PAIR_M + (int)rank * BM + quad * 32 + lane;       // this thread's output row
+      const int row0 = mb * PAIR_M + (int)rank * BM + quad * 32;             // first row of the warp's slab
+      const int tcol0 = nb * BN + chalf * EC;                                 // first column of the warp (in this launch)
+
+      if (ea.mode == EPI_CONC) {
+        // a8 fused: 32-column pieces of this row against the box of the row's property; A_0 is never stored
         if (row < M) {
-          const int b = (row / conc.R) % conc.B;
-          const float* xl = conc.x_lo + (long long)b * conc.ldx + conc.col_off + col0;
-          const float* xh = conc.x_hi + (long long)b * conc.ldx + conc.col_off + col0;
-          float dot = 0.f, ab = 0.f;
+          const int b = (row / ea.R) % ea.B;
+          const float* xl = ea.x_lo + (long long)b * ea.ldx + ea.col_off;
+          const float* xh = ea.x_hi + (long long)b * ea.ldx + ea.col_off;
+          float2* prow = reinterpret_cast<float2*>(ea.part) + (long long)row * ea.parts + (ea.col_off >> 5);
 #pragma unroll
-          for (int i = 0; i < EC; i += 4) {
-            if (col0 + i < N) {                      // N % 4 == 0: whole float4 in range
-              const float4 lo = __ldg(reinterpret_cast<const float4*>(xl + i));
-              const float4 hi = __ldg(reinterpret_cast<const float4*>(xh + i));
-              dot = fmaf(acc[i], 0.5f * (lo.x + hi.x), dot);     ab = fmaf(fabsf(acc[i]), 0.5f * (hi.x - lo.x), ab);
-              dot = fmaf(acc[i + 1], 0.5f * (lo.y + hi.y), dot); ab = fmaf(fabsf(acc[i + 1]), 0.5f * (hi.y - lo.y), ab);
-              dot = fmaf(acc[i + 2], 0.5f * (lo.z + hi.z), dot); ab = fmaf(fabsf(acc[i + 2]), 0.5f * (hi.z - lo.z), ab);
-              dot = fmaf(acc[i + 3], 0.5f * (lo.w + hi.w), dot); ab = fmaf(fabsf(acc[i + 3]), 0.5f * (hi.w - lo.w), ab);
+          for (int sl = 0; sl < EC / 32; ++sl) {
+            const int col = tcol0 + sl * 32;
+            if (chalf * EC + sl * 32 < BN && col < N) {
+              float dot = 0.f, ab = 0.f;
+#pragma unroll
+              for (int i = 0; i < 32; i += 4) {
+                if (col + i < N) {                     // N % 4 == 0: whole float4 in range
+                  const float4 lo = __ldg(reinterpret_cast<const float4*>(xl + col + i));
+                  const float4 hi = __ldg(reinterpret_cast<const float4*>(xh + col + i));
+                  const float a0 = acc[sl * 32 + i], a1 = acc[sl * 32 + i + 1], a2 = acc[sl * 32 + i + 2], a3 = acc[sl * 32 + i + 3];
+                  dot = fmaf(a0, 0.5f * (lo.x + hi.x), dot); ab = fmaf(fabsf(a0), 0.5f * (hi.x - lo.x), ab);
+                  dot = fmaf(a1, 0.5f * (lo.y + hi.y), dot); ab = fmaf(fabsf(a1), 0.5f * (hi.y - lo.y), ab);
+                  dot = fmaf(a2, 0.5f * (lo.z + hi.z), dot); ab = fmaf(fabsf(a2), 0.5f * (hi.z - lo.z), ab);
+                  dot = fmaf(a3, 0.5f * (lo.w + hi.w), dot); ab = fmaf(fabsf(a3), 0.5f * (hi.w - lo.w), ab);
+                }
+              }
+              prow[col >> 5] = make_float2(dot, ab);
             }
           }
-          float2* dst = reinterpret_cast<float2*>(conc.part) + (long long)row * conc.parts + (conc.piece0 + nb * 2 + chalf);
-          *dst = make_float2(dot, ab);
         }
         continue;
       }
-      // tile -> global through shared memory and the TMA: lane = row writes its 32 columns (128 B) of a slab in the
-      // 128B-swizzled layout (conflict-free), one lane issues the bulk tensor store, which also clips the M / N edges
-      const uint32_t slab = epi_base + (uint32_t)ew * 4096u + (uint32_t)lane * 128u;
-      const uint32_t sw = (uint32_t)(lane & 7);
+
+      // row -> (branch, property) for the relaxation coefficients
+      const bool rok = row < M;
+      const int rr = rok ? row : 0;
+      const bool upper = rr >= BR;
+      const float4* crow = nullptr;
+      if (ea.mode == EPI_RELAX) crow = ea.coef + (long long)((rr / ea.R) % ea.B) * ea.coef_ld + ea.col_off;
+
 #pragma unroll
       for (int sl = 0; sl < EC / 32; ++sl) {
-        if (lane == 0) bulk_wait_read0();          // the previous store has finished reading this warp's slab
-        __syncwarp();
+        const int col = tcol0 + sl * 32;
+        if (chalf * EC + sl * 32 >= BN || col >= N) continue;        // warp-uniform
+        if (ea.mode == EPI_RELAX) {
+          // a4 fused: lower: Abar = A+ dL + A- dU, d += A- . bU; upper: Abar = A+ dU + A- dL,
+          // d += A+ . bU; both: d += Abar . b.  One fp32 partial per (row, 32-column piece), summed in index order later.
+          float hi[32], dsum = 0.f;
 #pragma unroll
-        for (int c = 0; c < 8; ++c) {
-          const int i = sl * 32 + c * 4;
-          asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};"
-                       :: "r"(slab + (((uint32_t)c ^ sw) << 4)), "f"(acc[i]), "f"(acc[i + 1]), "f"(acc[i + 2]), "f"(acc[i + 3]) : "memory");
-        }
-        fence_proxy_async();
-        __syncwarp();
-        if (lane == 0) {
-          if (accumulate) tma_reduce_add_2d(&tmD, epi_base + (uint32_t)ew * 4096u, nb * BN + chalf * EC + sl * 32, mb * BM + quad * 32);
-          else tma_store_2d(&tmD, epi_base + (uint32_t)ew * 4096u, nb * BN + chalf * EC + sl * 32, mb * BM + quad * 32);
-          bulk_commit();
+          for (int i = 0; i < 32; ++i) {
+            float o = 0.f;
+            if (col + i < N) {
+              const float4 cf = __ldg(crow + col + i);
+              const float a = acc[sl * 32 + i];
+              const float pos = fmaxf(a, 0.f), neg = fminf(a, 0.f);
+              const float sp = upper ? cf.x : cf.z, sn = upper ? cf.z : cf.x;
+              o = pos * sp + neg * sn;
+              dsum = fmaf(upper ? pos : neg, cf.y, dsum);
+              if (ea.bias) dsum = fmaf(o, __ldg(ea.bias + ea.col_off + col + i), dsum);
+            }
+            hi[i] = tf32_rna(o);
+            acc[sl * 32 + i] = tf32_rna(o - hi[i]);       // lo limb, kept in the accumulator registers
+          }
+          if (rok) ea.part[(long long)row * ea.parts + ((ea.col_off + col) >> 5)] = dsum;
+          if (lane == 0) bulk_wait_read0();
+          __syncwarp();
+#pragma unroll
+          for (int c4 = 0; c4 < 8; ++c4)
+            asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};"
+                         :: "r"(slab + (((uint32_t)c4 ^ sw) << 4)), "f"(hi[c4 * 4]), "f"(hi[c4 * 4 + 1]), "f"(hi[c4 * 4 + 2]), "f"(hi[c4 * 4 + 3]) : "memory");
+          fence_proxy_async();
+          __syncwarp();
+          if (lane == 0) { tma_store_2d(&tmD, slab_base, col, row0); bulk_commit(); bulk_wait_read0(); }
+          __syncwarp();
+#pragma unroll
+          for (int c4 = 0; c4 < 8; ++c4) {
+            const int i = sl * 32 + c4 * 4;
+            asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};"
+                         :: "r"(slab + (((uint32_t)c4 ^ sw) << 4)), "f"(acc[i]), "f"(acc[i + 1]), "f"(acc[i + 2]), "f"(acc[i + 3]) : "memory");
+          }
+          fence_proxy_async();
+          __syncwarp();
+          if (lane == 0) { tma_store_2d(&tmD_lo, slab_base, col, row0); bulk_commit(); }
+        } else {
+          // tile -> global through shared memory and the TMA: lane = row writes its 32 columns (128 B) of a slab in the
+          // 128B-swizzled layout (conflict-free), one lane issues the bulk tensor store, which also clips the M / N edges
+          if (lane == 0) bulk_wait_read0();          // the previous store has finished reading this warp's slab
+          __syncwarp();
+#pragma unroll
+          for (int c4 = 0; c4 < 8; ++c4) {
+            const int i = sl * 32 + c4 * 4;
+            asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};"
+                         :: "r"(slab + (((uint32_t)c4 ^ sw) << 4)), "f"(acc[i]), "f"(acc[i + 1]), "f"(acc[i + 2]), "f"(acc[i + 3]) : "memory");
+          }
+          fence_proxy_async();
+          __syncwarp();
+          if (lane == 0) {
+            if (ea.mode == EPI_ADD) tma_reduce_add_2d(&tmD, slab_base, col, row0);
+            else tma_store_2d(&tmD, slab_base, col, row0);
+            bulk_commit();
+          }
         }
       }
     }
@@ -271,65 +331,68 @@ gemm_tf32x3_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_cons
 
   tcgen05_fence_before();
   __syncthreads();
+  cluster_sync_all();          // the peer may still multicast into / arrive on this CTA's barriers until here
   if (warp == 2) {
     tcgen05_fence_after();
-    tmem_dealloc(tmem_base, C::TMEM_COLS);
+    tmem_dealloc_pair(tmem_base, TMEM_COLS);
   }
 }
 
 // ---------------------------------------------------------------- host side
-template <int BN>
-static int launch_bn(const float* A_hi, const float* A_lo, const float* Wt_hi, const float* Wt_lo, float* D,
-                     long long ldd, int M, int N, int K, int k_drain, int num_sms, cudaStream_t s,
-                     const char** err, const ConcArgs* conc) {
-  using C = Cfg<BN>;
-  CUtensorMap tout;
-  const bool fused_conc = conc && conc->part;
-  // fused concretisation stores no D: the output map is a placeholder over the partial-sum buffer
-  if (!(fused_conc ? make_tmap_out(&tout, conc->part, M, 4, 4) : make_tmap_out(&tout, D, M, N, ldd))) {
-    if (err) *err = "cuTensorMapEncodeTiled failed";
-    return -1;
-  }
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(gemm_tf32x3_kernel<BN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         C::SMEM_BYTES);
-    if (e != cudaSuccess) { if (err) *err = cudaGetErrorString(e); return -1; }
-    attr_set = true;
-  }
-  int m_tiles = (M + BM - 1) / BM, n_tiles = (N + BN - 1) / BN;
-  long long tiles = (long long)m_tiles * n_tiles;
-  int grid = (int)(tiles < num_sms ? tiles : num_sms);
-  if (k_drain <= 0) k_drain = 128;   // 16 hi.hi MMAs per TMEM chain: truncation bias ~4e-7 rel
+static int g_max_clusters = 0;     // per process AND device-independent upper bound is not assumed: see gemm_tc_init_device
+
+static int launch_pair(const float* A_hi, const float* A_lo, const float* Wt_hi, const float* Wt_lo, float* D, float* D_lo,
+                       long long ldd, int M, int N, int K, int k_drain, int num_sms, cudaStream_t s,
+                       const char** err, const EpiArgs& epi_in) {
+  EpiArgs epi = epi_in;
+  // tile width: the fewest 256-wide column blocks, evened out to a multiple of 32 (784 -> 4 x 224, not 3 x 256 + 16)
+  const int n_blocks = (N + BN_MAX - 1) / BN_MAX;
+  int BN = ((N + n_blocks - 1) / n_blocks + 31) / 32 * 32;
+  if (BN > BN_MAX) BN = BN_MAX;
+  if (BN < 32) BN = 32;
+  const int m_tiles = (M + PAIR_M - 1) / PAIR_M, n_tiles = (N + BN - 1) / BN;
+  const long long tiles = (long long)m_tiles * n_tiles;
+  int clusters = num_sms / 2;
+  if (g_max_clusters > 0 && clusters > g_max_clusters) clusters = g_max_clusters;
+  if (tiles < clusters) clusters = (int)tiles;
+  if (clusters < 1) clusters = 1;
+  if (k_drain <= 0) k_drain = 64;    // 24 MMAs per TMEM chain: truncation bias <= ~7e-7 of the chunk's magnitude
   int kb_per_chunk = (k_drain + BK - 1) / BK;
   if (kb_per_chunk < 1) kb_per_chunk = 1;
-  int chunks_per_small = 16384 / (kb_per_chunk * BK);   // small accumulator drained every 16384 elements of K
-  if (chunks_per_small < 1) chunks_per_small = 1;
-  // K panels.  One wave of 148 tiles shares ~8 m-blocks of A and ~19 n-blocks of W; streamed over the whole K their
-  // hi/lo limbs are (8 + 19) * 128 rows * K * 8 B, which for K = 16384 is 450 MB: far beyond the 126 MB L2, and
-  // measured (profiles/r1_gemm_tf32x3_cfg3.md) as DRAM traffic above the kernel's own request volume.  Cutting K
-  // into panels whose per-wave working set fits L2 makes operand re-use independent of how far CTAs drift apart;
-  // panels after the first add into D with the TMA's fp32 reduce-add (fixed order: deterministic).
-  const long long share_blocks = (long long)(m_tiles < GROUP_M ? m_tiles : GROUP_M) +
-                                 (long long)(n_tiles < 19 ? n_tiles : 19);
-  const long long bytes_per_k = share_blocks * 128 * 8;
+  // K panels.  One wave of 74 pair tiles shares ~8 m-blocks of A and ~10 n-blocks of W; streamed over the whole K their
+  // hi/lo limbs are 18 * 256 rows * K * 8 B, far beyond the 126 MB L2 for K = 16384 (measured in round 1 as DRAM traffic
+  // above the kernel's own request volume, profiles/r1_gemm_tf32x3_cfg3.md).  Cutting K into panels whose per-wave
+  // working set fits L2 makes operand re-use independent of how far CTAs drift apart; panels after the first add
+  // into D with the TMA's fp32 reduce-add (fixed order: deterministic).  The panel length depends on K only (not on
+  // M or N), so row-chunked and N-slabbed (streamed) runs sum in the same order: bitwise equal results.
+  const long long bytes_per_k = 18LL * 256 * 8;
   int kp = K;
   if (bytes_per_k * K > (96LL << 20)) {
     kp = (int)((64LL << 20) / bytes_per_k) / 512 * 512;
     if (kp < 1024) kp = 1024;
   }
-  if (fused_conc && kp != K) { if (err) *err = "gemm_tc: fused concretisation needs a single K panel"; return -1; }
-  const ConcArgs cargs = fused_conc ? *conc : ConcArgs();
+  if (epi.mode != EPI_STORE && kp != K) { if (err) *err = "gemm_tc: fused epilogues need a single K panel"; return -1; }
+  CUtensorMap tout, tout_lo;
+  bool ok = true;
+  if (epi.mode == EPI_CONC) {
+    // no D is stored: the output maps are placeholders over the partial-sum buffer
+    ok = make_tmap_out(&tout, epi.part, M, 4, 4) && make_tmap_out(&tout_lo, epi.part, M, 4, 4);
+  } else if (epi.mode == EPI_RELAX) {
+    ok = make_tmap_out(&tout, D, M, N, ldd) && make_tmap_out(&tout_lo, D_lo, M, N, ldd);
+  } else {
+    ok = make_tmap_out(&tout, D, M, N, ldd) && make_tmap_out(&tout_lo, D, M, N, ldd);
+  }
+  if (!ok) { if (err) *err = "cuTensorMapEncodeTiled failed"; return -1; }
   for (int k0 = 0; k0 < K; k0 += kp) {
     const int kk = K - k0 < kp ? K - k0 : kp;
     CUtensorMap ta, tb, tc_, td;
     if (!make_tmap(&ta, A_hi + k0, M, kk, BM, K) || !make_tmap(&tb, A_lo + k0, M, kk, BM, K) ||
-        !make_tmap(&tc_, Wt_hi + k0, N, kk, BN, K) || !make_tmap(&td, Wt_lo + k0, N, kk, BN, K)) {
+        !make_tmap(&tc_, Wt_hi + k0, N, kk, BN / 2, K) || !make_tmap(&td, Wt_lo + k0, N, kk, BN / 2, K)) {
       if (err) *err = "cuTensorMapEncodeTiled failed";
       return -1;
     }
-    gemm_tf32x3_kernel<BN><<<grid, C::THREADS, C::SMEM_BYTES, s>>>(ta, tb, tc_, td, tout, M, N, kk, kb_per_chunk,
-                                                                   chunks_per_small, k0 > 0 ? 1 : 0, cargs);
+    if (epi.mode == EPI_STORE || epi.mode == EPI_ADD) epi.mode = k0 > 0 ? EPI_ADD : EPI_STORE;
+    gemm2_tf32x3_kernel<<<2 * clusters, THREADS, SMEM_BYTES, s>>>(ta, tb, tc_, td, tout, tout_lo, M, N, kk, BN, kb_per_chunk, epi);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) { if (err) *err = cudaGetErrorString(e); return -1; }
   }
@@ -338,30 +401,57 @@ static int launch_bn(const float* A_hi, const float* A_lo, const float* Wt_hi, c
 
 }  // namespace tc
 
+int gemm_tc_init_device() {
+  if (cudaFuncSetAttribute(tc::gemm2_tf32x3_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::SMEM_BYTES) != cudaSuccess)
+    return -1;
+  // how many CTA pairs can be resident at once (one per TPC when every SM is available)
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(2, 1, 1); cfg.blockDim = dim3(tc::THREADS, 1, 1); cfg.dynamicSmemBytes = tc::SMEM_BYTES;
+  cudaLaunchAttribute at; at.id = cudaLaunchAttributeClusterDimension; at.val.clusterDim.x = 2; at.val.clusterDim.y = 1; at.val.clusterDim.z = 1;
+  cfg.attrs = &at; cfg.numAttrs = 1;
+  int n = 0;
+  if (cudaOccupancyMaxActiveClusters(&n, tc::gemm2_tf32x3_kernel, &cfg) == cudaSuccess && n > 0) tc::g_max_clusters = n;
+  else (void)cudaGetLastError();
+  return 0;
+}
+
 int gemm_tc_supported(int M, int N, int K) {
-  // TMA needs 16-byte row pitches (K % 4) and the epilogue stores float4 (N % 4).  M below one tile is fine (TMA
-  // zero-fills the missing rows) and still beats the CUDA-core kernel; N < 128 or K < 32 is left to that kernel.
+  // TMA needs 16-byte row pitches (K % 4) and the epilogue handles columns in float4 groups (N % 4).  M below one tile
+  // is fine (TMA zero-fills the missing rows) and still beats the CUDA-core kernel; N < 128 or K < 32 is left to that kernel.
   return M >= 1 && N >= 128 && K >= 32 && (K % 4 == 0) && (N % 4 == 0);
 }
 
-int gemm_tc_conc_parts(int N) { return 2 * ((N + 127) / 128); }
+int gemm_tc_parts(int N_total) { return (N_total + 31) / 32; }
 
-int gemm_tc_conc_supported(int M, int N, int K) {
-  // single K panel (see launch_bn): the working-set rule only cuts K above ~3000 for >= 27 shared blocks
-  return gemm_tc_supported(M, N, K) && K <= 2048;
-}
+int gemm_tc_single_panel(int K) { return 18LL * 256 * 8 * K <= (96LL << 20); }
+
+static bool mis16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) != 0; }
 
 int launch_gemm_tc(const float* A_hi, const float* A_lo, const float* Wt_hi, const float* Wt_lo, float* D,
                    long long ldd, int M, int N, int K, int k_drain, int num_sms, cudaStream_t s,
-                   const char** err, const ConcArgs* conc) {
-  auto mis = [](const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) != 0; };
+                   const char** err, const ConcArgs* conc, const RelaxEpiArgs* rel) {
   const bool fc = conc && conc->part;
-  if (!gemm_tc_supported(M, N, K) || mis(A_hi) || mis(A_lo) || mis(Wt_hi) || mis(Wt_lo) || (!fc && (mis(D) || (ldd % 4) != 0)) ||
-      (fc && (mis(conc->x_lo) || mis(conc->x_hi) || mis(conc->part)))) {
+  const bool fr = rel && rel->part;
+  if (!gemm_tc_supported(M, N, K) || mis16(A_hi) || mis16(A_lo) || mis16(Wt_hi) || mis16(Wt_lo) ||
+      (!fc && (mis16(D) || (ldd % 4) != 0)) || (fc && fr) ||
+      (fc && (mis16(conc->x_lo) || mis16(conc->x_hi) || mis16(conc->part) || (conc->col_off % 32) != 0)) ||
+      (fr && (mis16(rel->out_lo) || mis16(rel->coef) || (rel->col_off % 32) != 0))) {
     if (err) *err = "gemm_tc: unsupported shape or misaligned operand";
     return -1;
   }
-  return tc::launch_bn<128>(A_hi, A_lo, Wt_hi, Wt_lo, D, ldd, M, N, K, k_drain, num_sms, s, err, conc);
+  tc::EpiArgs e;
+  float* D_lo = nullptr;
+  if (fc) {
+    e.mode = tc::EPI_CONC; e.B = conc->B; e.R = conc->R; e.col_off = conc->col_off; e.parts = conc->parts;
+    e.part = conc->part; e.x_lo = conc->x_lo; e.x_hi = conc->x_hi; e.ldx = conc->ldx;
+  } else if (fr) {
+    e.mode = tc::EPI_RELAX; e.B = rel->B; e.R = rel->R; e.col_off = rel->col_off; e.parts = rel->parts;
+    e.part = rel->part; e.coef = rel->coef; e.coef_ld = rel->coef_ld; e.bias = rel->bias;
+    D_lo = rel->out_lo;
+  } else {
+    e.mode = tc::EPI_STORE; e.B = 1; e.R = M > 0 ? M : 1;
+  }
+  return tc::launch_pair(A_hi, A_lo, Wt_hi, Wt_lo, D, D_lo, ldd, M, N, K, k_drain, num_sms, s, err, e);
 }
 
 }  // namespace crownb200

@@ -129,8 +129,6 @@ static void ibp_launch(const float* W, const float* bias, const float* l_in, con
   const int kc_max = kIbpSmemMax / (2 * BT * 4) / 512 * 512;
   if (KC > kc_max) KC = kc_max;
   const size_t smem = (size_t)2 * BT * KC * 4;
-  static bool attr = false;
-  if (!attr) { cudaFuncSetAttribute(ibp_linear_kernel<BT, RW>, cudaFuncAttributeMaxDynamicSharedMemorySize, kIbpSmemMax); attr = true; }
   int gx = ceil_div(n_out, kIbpWarps * RW);
   if (KC >= n_in) {                                // persistent: stage c/r once per block, then stream row groups
     int dev = 0, sms = 148;
@@ -141,6 +139,13 @@ static void ibp_launch(const float* W, const float* bias, const float* l_in, con
   }
   dim3 grid(gx, ceil_div(B, BT));
   ibp_linear_kernel<BT, RW><<<grid, kIbpWarps * 32, smem, s>>>(W, bias, l_in, u_in, relu_in, l_out, u_out, B, n_out, n_in, ldo, KC);
+}
+
+int ibp_init_device() {
+  cudaError_t e1 = cudaFuncSetAttribute(ibp_linear_kernel<1, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, kIbpSmemMax);
+  cudaError_t e2 = cudaFuncSetAttribute(ibp_linear_kernel<2, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, kIbpSmemMax);
+  cudaError_t e3 = cudaFuncSetAttribute(ibp_linear_kernel<4, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, kIbpSmemMax);
+  return (e1 == cudaSuccess && e2 == cudaSuccess && e3 == cudaSuccess) ? 0 : -1;
 }
 
 void launch_ibp_linear(const float* W, const float* bias, const float* l_in, const float* u_in,

@@ -17,10 +17,8 @@ struct AView {
 };
 
 // a3 -- relaxation coefficients of a ReLU from its pre-activation bounds.
-// coef[b*n+j] = {dU, bU, dL_fixed, unstable?1:0}; planes[p*plane_stride + b*n+j], p = 0 dU, 1 bU, 2 dL (the same
-// values as planes, for 128-bit loads along the neuron axis).  rule: 0 adaptive, 1 zero, 2 one.
-void launch_relax_coeffs(const float* l, const float* u, float4* coef, float* planes, long long plane_stride,
-                         long long count, int rule, cudaStream_t s);
+// coef[b*n+j] = {dU, bU, dL_fixed, unstable?1:0}.  rule: 0 adaptive, 1 zero, 2 one.
+void launch_relax_coeffs(const float* l, const float* u, float4* coef, long long count, int rule, cudaStream_t s);
 
 // a4 -- fused relaxation of A through a ReLU, both branches, with the bias
 // accumulation of the ReLU (bU through the sign-selected part of A) and of the linear layer below
@@ -73,39 +71,44 @@ void launch_split_tf32(const float* X, int rows, int cols, int transpose, float*
 void launch_gemm_ffma(const float* A, long long lda, const float* W, long long ldw, float* D,
                       long long ldd, int M, int N, int K, cudaStream_t s);
 
-// a5 -- 3xTF32 contraction on tcgen05 tensor cores: D[M,N] = (A_hi + A_lo)[M,K] . (Wt_hi + Wt_lo)[N,K]^T
-// with the three products hi.hi + hi.lo + lo.hi accumulated in fp32 (TMEM), drained to an fp32
-// CUDA-core running sum every k_drain elements of K.
-// a8 fused into the last contraction: when `part` != nullptr the epilogue does not store D; every epilogue warp
-// reduces its 64 columns of the tile against the box instead (dot = sum A.x_c, ab = sum |A|.x_r) and writes the pair
-// to part[(row * parts + piece) * 2 + {0,1}], piece = 2 * n_block + column half.  launch_concretize_parts then adds
-// the pieces in index order (deterministic).  Only valid when K is a single panel (|.| is not linear in K).
+// a5 -- 3xTF32 contraction on tcgen05 tensor cores (CTA-pair tiles, gemm_tc.cu):
+// D[M,N] = (A_hi + A_lo)[M,K] . (Wt_hi + Wt_lo)[N,K]^T with the three products hi.hi + hi.lo + lo.hi accumulated in
+// fp32 (TMEM), drained to an fp32 CUDA-core running sum every k_drain elements of K.  Two fused epilogues replace the
+// store of D; both need K to be a single panel (gemm_tc_single_panel) and emit one partial sum per (row, 32-column
+// piece of the FULL row), which a small kernel adds in index order -- the grouping does not depend on the tiling,
+// so N-slabbed (streamed) and row-chunked runs give bitwise the same sums:
+//   a8 fused (ConcArgs):     no D; part[(row*parts + piece)] = float2(sum A.x_c, sum |A|.x_r) against the row's box;
+//                            launch_concretize_parts finishes lb/ub.  A_0 never reaches HBM.
+//   a4 fused (RelaxEpiArgs): D receives the TF32 hi limb and out_lo the lo limb of Abar = relaxation of the product
+//                            through the ReLU below (fixed-rule slopes); part[row*parts + piece] = that piece's
+//                            contribution to d (A-/+ . bU and Abar . bias); launch_reduce_parts adds them into d.
 struct ConcArgs {
   const float* x_lo = nullptr; const float* x_hi = nullptr;   // [B, ldx]
-  float* part = nullptr;                                       // [M, parts, 2]
+  float* part = nullptr;                                       // [M, parts] float2
   int B = 0, R = 0, parts = 0;
   int ldx = 0;        // row pitch of x_lo / x_hi (the full input width)
-  int col_off = 0;    // first input column of this launch (N-slab of a streamed operand), multiple of 128
-  int piece0 = 0;     // first piece index of this launch = 2 * col_off / 128
+  int col_off = 0;    // first input column of this launch (N-slab of a streamed operand), multiple of 32
 };
-int gemm_tc_conc_parts(int N);                 // pieces per row for an N-wide output
-int gemm_tc_conc_supported(int M, int N, int K);
+struct RelaxEpiArgs {
+  const float4* coef = nullptr;   // [B, coef_ld] {dU, bU, dL, unstable} of the ReLU below
+  long long coef_ld = 0;          // = width of the full row (neurons of the ReLU)
+  const float* bias = nullptr;    // bias of the Linear below the ReLU [coef_ld] or nullptr
+  float* out_lo = nullptr;        // lo limb output, same addressing as D
+  float* part = nullptr;          // [M, parts] float
+  int B = 0, R = 0, parts = 0;
+  int col_off = 0;                // first column of this launch inside the full row, multiple of 32
+};
+int gemm_tc_parts(int N_total);                // 32-column pieces per row of an N_total-wide output
+int gemm_tc_single_panel(int K);               // 1 if the contraction runs as one K panel (fused epilogues allowed)
 void launch_concretize_parts(const float* part, int parts, const float* d, float* lb, float* ub, int out_stride,
                              int B, int R, cudaStream_t s);
+// d[m] += part[m*parts + 0] + part[m*parts + 1] + ... (index order), m < rows
+void launch_reduce_parts(const float* part, int parts, float* d, long long rows, cudaStream_t s);
 int gemm_tc_supported(int M, int N, int K);
 int launch_gemm_tc(const float* A_hi, const float* A_lo, const float* Wt_hi, const float* Wt_lo,
                    float* D, long long ldd, int M, int N, int K, int k_drain, int num_sms,
-                   cudaStream_t s, const char** err, const ConcArgs* conc = nullptr);
-
-// a4 + a5 fused -- relaxation of A through a ReLU (planes != nullptr; fixed-rule slopes only), d += A-/+ . bU,
-// d += Abar . bias, TF32 split and the 3xTF32 contraction with the prepacked operand in one kernel
-// (gemm_fused.cu).  A is a raw fp32 view ([2,B,R,K], strides multiples of K); D [2*B*R, N] with row pitch ldd
-// (an N-slab of a wider output when the operand is streamed; pass d = nullptr for all slabs but the first).
-int gemm_fused_supported(const AView& A, int B, int R, int N, int K);
-int launch_gemm_fused(const AView& A, int B, int R, const float* planes, long long plane_stride, const float* bias,
-                      float* d,
-                      const float* Wt_hi, const float* Wt_lo, float* D, long long ldd, int N, int K, int k_drain,
-                      int num_sms, cudaStream_t s, const char** err);
+                   cudaStream_t s, const char** err, const ConcArgs* conc = nullptr,
+                   const RelaxEpiArgs* rel = nullptr);
 
 // a2 / a6 -- Conv2d IBP (centre/radius) and conv-transpose backward of A.
 void launch_ibp_conv(const float* W, const float* bias, const float* l_in, const float* u_in,
@@ -114,5 +117,13 @@ void launch_ibp_conv(const float* W, const float* bias, const float* l_in, const
 void launch_conv_transpose(const AView& A, const float* W, const float* addend, float* out,
                            int B, int R, int c_in, int h, int w, int c_out, int kh, int kw,
                            int stride, int pad, int ho, int wo, cudaStream_t s);
+
+// Per-device kernel attributes (opt-in dynamic shared memory sizes).  cudaFuncSetAttribute applies to the CURRENT
+// device only, so crown_init calls this for the device of every new context (a process-wide "done" flag would
+// leave a second device without them).  Returns 0 on success.
+int gemm_tc_init_device();
+int ibp_init_device();
+int conv_init_device();
+inline int kernels_init_device() { return gemm_tc_init_device() | ibp_init_device() | conv_init_device(); }
 
 }  // namespace crownb200

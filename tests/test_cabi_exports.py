@@ -47,8 +47,8 @@ def test_struct_layouts_match_the_header():
     from paper_2606_09377_b200 import binding
     # crown_node: 13 int32 + 3 pointers; crown_opts: u64, 4 x i32, u64, u64, i32 (+ tail padding)
     assert ctypes.sizeof(binding.CrownNode) == 13 * 4 + 4 + 3 * 8
-    assert ctypes.sizeof(binding.CrownOpts) == 8 + 4 * 4 + 8 + 8 + 8          # ..., enable_fusion, disable_conc_fusion
-    assert binding.CrownOpts.stream_min_elems.offset == 24 and binding.CrownOpts.enable_fusion.offset == 40
+    assert ctypes.sizeof(binding.CrownOpts) == 8 + 4 * 4 + 8 + 8 + 8          # ..., disable_epi_fusion, disable_conc_fusion
+    assert binding.CrownOpts.stream_min_elems.offset == 24 and binding.CrownOpts.disable_epi_fusion.offset == 40
 
 
 def test_version_and_error_paths_without_compute(lib):
