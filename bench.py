@@ -1,13 +1,15 @@
 #!/usr/bin/env python
 """bench.py -- one JSON line for the CROWN hot path on B200 (contract: DESIGN.md sec. "Measurement").
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2] [--impl b200|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3] [--impl b200|reference]
 
-A "step" is one pass of the whole hot path (IBP -> CROWN intermediate bounds for every ReLU -> alpha-CROWN
-final bound -> concretisation -> verdict) over one batch of synthetic input.
-Default workload = BASELINE.json configs[1]: MNIST-FC-shaped MLP 784-(256x6)-10, 64 properties x 3 eps
-(192 properties per step), 9 margin specs each, alpha ~ U[0,1].  Inputs are seeded and synthetic
-(workloads.py); they stand in for the paper's VNN-COMP MNIST-FC instances, which are not reproduced.
+A "step" is one pass of the whole hot path (IBP -> CROWN intermediate bounds for every ReLU -> (alpha-)CROWN final
+bound -> concretisation -> verdict) over one batch of synthetic input.
+Headline workload = BASELINE.json configs[2] (cfg3): the largest single-GPU configuration, wide MLP
+4096-16384x3-10, 16 properties, 9 margin specs, full CROWN row-chunked under a 64 GiB workspace cap (BASELINE.md
+sec. 3 puts the tensor-roofline target on cfg3 / cfg4).  The same JSON line carries a `per_config` object with the
+other four configs (fewer steps for the long ones).  Inputs are seeded and synthetic (workloads.py); they stand in
+for the paper's VNN-COMP / wide-MLP workloads, which are not reproduced.
 
 value  : properties/s, device-timed (CUDA events on the launching stream), inputs resident in HBM.
 e2e    : same metric through crown_run_host: pinned HOST buffers, H2D of x_lo/x_hi/C/alpha and D2H of
@@ -19,6 +21,7 @@ data-path collective; time = max over ranks.
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
 import sys
@@ -34,22 +37,25 @@ if ROOT not in sys.path:
 import workloads as W  # noqa: E402
 
 METRIC, UNIT = "properties_per_sec", "properties/s"
-TF32_OVER_BF16 = 1.1 / 2.25          # nominal dense ratio (B200_PROFILING.md table)
+TF32_OVER_BF16 = 1.1 / 2.25          # nominal dense ratio (B200_PROFILING.md table); used only if TF32 is not measured
+ALL_CFGS = ["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"]
 
 
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
+    ap.add_argument("--workload", default="cfg3", choices=ALL_CFGS)
+    ap.add_argument("--no-per-config", action="store_true", help="only the --workload config (no per_config block)")
     ap.add_argument("--scale", type=int, default=1, help="width divisor (debug only; 1 = the named config)")
     ap.add_argument("--batch", type=int, default=0, help="override B (debug only)")
     ap.add_argument("--mem-cap-gb", type=float, default=0.0)
     ap.add_argument("--stream-weights", action="store_true",
                     help="layers with >= 2^28 weights are streamed from pinned host memory (a7), not resident")
     ap.add_argument("--no-epi-fusion", action="store_true", help="run the relaxation as its own kernel (debug)")
+    ap.add_argument("--no-graph", action="store_true", help="do not replay crown_run from a CUDA graph (debug)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     return ap.parse_args()
@@ -65,69 +71,176 @@ def peaks():
     return {"hbm": 6650.0, "bf16": 1590.0, "bf16_sustained": 1400.0, "src": "fallback"}
 
 
+def kernel_source_sha1():
+    """sha1 over the CUDA sources: a committed ncu traffic figure is only quoted while the kernels are unchanged."""
+    h = hashlib.sha1()
+    d = os.path.join(ROOT, "paper_2606_09377_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        with open(os.path.join(d, f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def profiled_traffic(cfgname, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed ncu --set full capture of
+    this workload (profiles/traffic.json), or None when there is none for the current kernel sources."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        tab = json.load(f)
+    e = tab.get(f"{cfgname}:{kernel}")
+    if not e or e.get("src_sha1") != kernel_source_sha1():
+        return None
+    return e["dram_bytes_per_launch"]
+
+
 def workload_desc(wl, cfgname):
     return {"workload": f"{cfgname}:{wl.name}", "B": int(wl.B), "S": int(wl.S),
             "eps_set": sorted({round(float(e), 6) for e in wl.eps}), "properties_per_step": int(wl.B),
             "intermediate": wl.intermediate, "alpha": wl.alpha is not None}
 
 
-def boxes(wl):
-    """The (x_lo, x_hi) batches of a step.  Workloads with several eps (cfg2: 64 points x 3 eps) are stacked by
-    workloads.stack_eps into ONE batch of per-property radii before this is called (reading G13)."""
-    return [wl.box()]
+def make_workload(cfgname, args):
+    cfg = int(cfgname[3:])
+    return W.stack_eps(W.make(cfg, scale=args.scale, B=args.batch or None))
 
 
 # ------------------------------------------------------------------------------------------------
 # oracle legs (cpu_baseline and --impl reference): the ONLY places bench.py executes oracle/
 # ------------------------------------------------------------------------------------------------
-def oracle_sample(wl, bxs, budget_s, max_props=None):
-    """Runs the float64 oracle, as it stands, on properties 0,1,... of the eps batches (round robin) until
-    budget_s is spent (at least one property).  Returns (properties done, seconds, threads)."""
-    from oracle import crown_oracle as O
+def cpu_info():
+    model = "unknown"
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    model = line.split(":", 1)[1].strip()
+                    break
+    except OSError:
+        pass
+    blas, thr = "unknown", os.cpu_count() or 1
     try:
         from threadpoolctl import threadpool_info
-        thr = max([p.get("num_threads", 1) for p in threadpool_info()] + [1])
+        info = threadpool_info()
+        if info:
+            blas = ", ".join(sorted({f"{p.get('internal_api')} {p.get('version')}" for p in info}))
+            thr = max(p.get("num_threads", 1) for p in info)
     except Exception:
-        thr = os.cpu_count() or 1
+        pass
+    return model, blas, thr
+
+
+def oracle_props(wl, budget_s, max_props=None):
+    """Runs the float64 oracle, as it stands, on whole properties (eps groups round robin) until budget_s is spent
+    (at least one property).  Returns (properties done, seconds)."""
+    from oracle import crown_oracle as O
+    lo, hi = wl.box()
     done, t0 = 0, time.perf_counter()
-    k = max(1, len({float(e) for e in wl.eps}))          # stacked eps groups: visit them round robin
+    k = max(1, len({float(e) for e in wl.eps}))
     per = max(1, wl.B // k)
-    order = [(p, 0) for p in sorted(range(wl.B), key=lambda q: (q % per, q // per))]
-    for p, e in order:
-        lo, hi = bxs[e]
+    for p in sorted(range(wl.B), key=lambda q: (q % per, q // per)):
         al = None if wl.alpha is None else [a[p] for a in wl.alpha]
         O.run_property(wl.net, lo[p], hi[p], wl.C[p], al, wl.intermediate)
         done += 1
         if time.perf_counter() - t0 >= budget_s or (max_props and done >= max_props):
             break
-    return done, time.perf_counter() - t0, thr
+    return done, time.perf_counter() - t0
+
+
+def oracle_rows_time(wl, frac, p=0):
+    """Seconds the oracle needs for the intermediate bounds (O4) of property p when only the first ceil(frac * n_k)
+    identity rows of every CROWN pass are propagated (rows are independent linear bounds)."""
+    from oracle import crown_oracle as O
+    lo, hi = wl.box()
+    rows = {i: np.arange(max(1, int(np.ceil(frac * wl.net.nodes[i].size)))) for i in wl.net.relu_ids()}
+    t0 = time.perf_counter()
+    O.crown_bounds(wl.net, lo[p], hi[p], wl.intermediate, rows=rows)
+    return time.perf_counter() - t0
+
+
+def oracle_final_time(wl, p=0):
+    """Seconds of the oracle's final pass (O5) for property p; intermediate bounds = IBP (the arithmetic and its cost
+    do not depend on their values)."""
+    from oracle import crown_oracle as O
+    lo, hi = wl.box()
+    ib = O.ibp(wl.net, lo[p], hi[p])
+    pre = {i: (ib[wl.net.nodes[i].in0][0].reshape(-1), ib[wl.net.nodes[i].in0][1].reshape(-1)) for i in wl.net.relu_ids()}
+    t0 = time.perf_counter()
+    O.final_bounds(wl.net, lo[p], hi[p], wl.C[p], pre, None, None)
+    return time.perf_counter() - t0
+
+
+LARGE = ("cfg3", "cfg4")
+F1, F2 = 1.0 / 512, 1.0 / 128          # row fractions of the two sampled runs (cfg3: 32 and 128 of 16384 rows)
+
+
+def oracle_baseline(wl, cfgname, budget_s):
+    """cpu_baseline object: whole properties for cfg1/2/5; for cfg3/cfg4 one property is timed on two row samples
+    (F1 and F2 of every identity pass) and extrapolated linearly in the row count -- stated as scaled."""
+    model, blas, thr = cpu_info()
+    base = {"unit": UNIT, "cores": thr, "kind": "oracle", "cpu_model": model, "blas": blas}
+    if cfgname not in LARGE:
+        n, secs = oracle_props(wl, budget_s)
+        base.update(value=n / secs, sample=f"first {n} of {wl.B} properties (eps round robin), {secs:.1f} s, float64 numpy")
+        try:
+            from threadpoolctl import threadpool_limits
+            with threadpool_limits(limits=1):
+                n1, s1 = oracle_props(wl, min(budget_s, 6.0))
+            base["single_thread_value"] = n1 / s1
+        except Exception:
+            base["single_thread_value"] = None
+        return base
+    t1 = oracle_rows_time(wl, F1)
+    t2 = oracle_rows_time(wl, F2)
+    tf = oracle_final_time(wl)
+    slope = max(t2 - t1, 0.0) / (F2 - F1)
+    t_full = t2 + slope * (1.0 - F2) + tf
+    base.update(value=1.0 / t_full, single_thread_value=None,
+                sample=f"1 property, identity rows sampled at {F1:.5f} ({t1:.1f} s) and {F2:.5f} ({t2:.1f} s) of every "
+                       f"CROWN pass + final pass ({tf:.1f} s), extrapolated linearly to all rows: {t_full:.0f} s per "
+                       "property (SCALED, not run in full), float64 numpy")
+    return base
 
 
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    cfg = int(args.workload[3:])
-    wl = W.stack_eps(W.make(cfg, scale=args.scale, B=args.batch or None))
-    bxs = boxes(wl)
-    # each step = a bounded sample (first `per_step` properties) so K+W steps end within minutes
-    n1, t1, thr = oracle_sample(wl, bxs, 0.0, max_props=1)
-    per_step = max(1, min(wl.B * len(bxs), int(5.0 / max(t1 / n1, 1e-6))))
-    for _ in range(min(args.warmup, 1)):
-        oracle_sample(wl, bxs, 1e9, max_props=per_step)
-    tot_n, tot_t = 0, 0.0
-    for _ in range(args.steps):
-        n, t, thr = oracle_sample(wl, bxs, 1e9, max_props=per_step)
-        tot_n += n
-        tot_t += t
-    v = tot_n / tot_t
-    sample = f"{per_step} of {wl.B * len(bxs)} properties per step (first ones, eps round robin), float64 numpy"
+    wl = make_workload(args.workload, args)
+    model, blas, thr = cpu_info()
+    if args.workload in LARGE:
+        t1 = oracle_rows_time(wl, F1)               # calibration of the fixed part, once (the warm-up step)
+        tf = oracle_final_time(wl)
+        tot_t = 0.0
+        for _ in range(args.steps):
+            t2 = oracle_rows_time(wl, F2)
+            slope = max(t2 - t1, 0.0) / (F2 - F1)
+            tot_t += t2 + slope * (1.0 - F2) + tf
+        v = args.steps / tot_t
+        ms = 1e3 * tot_t / args.steps
+        sample = (f"per step: 1 property with {F2:.5f} of the identity rows of every CROWN pass, extrapolated linearly "
+                  f"to all rows with the fixed part calibrated once at {F1:.5f} (SCALED), float64 numpy")
+    else:
+        n1, t1 = oracle_props(wl, 0.0, max_props=1)
+        per_step = max(1, min(wl.B, int(5.0 / max(t1 / n1, 1e-6))))
+        for _ in range(min(args.warmup, 1)):
+            oracle_props(wl, 1e9, max_props=per_step)
+        tot_n, tot_t = 0, 0.0
+        for _ in range(args.steps):
+            n, t = oracle_props(wl, 1e9, max_props=per_step)
+            tot_n += n
+            tot_t += t
+        v = tot_n / tot_t
+        ms = 1e3 * tot_t / args.steps
+        sample = f"{per_step} of {wl.B} properties per step (first ones, eps round robin), float64 numpy"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps, "higher_is_better": True,
+        "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": workload_desc(wl, args.workload),
-        "cpu_baseline": {"value": v, "unit": UNIT, "cores": thr, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": thr, "kind": "oracle", "sample": sample,
+                         "cpu_model": model, "blas": blas},
         "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
 
@@ -178,78 +291,96 @@ class ClockSampler:
         return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons)}
 
 
+def measure_tf32_peak(dev):
+    """Dense TF32 tensor throughput of this box, measured the way MEASURED_PEAKS.json measures bf16: torch.matmul
+    (cuBLAS) on 8192^3 fp32 operands with TF32 allowed, best of 10 (burst) and back to back for ~2 s (sustained).
+    A measuring stick only: no library GEMM is on the hot path."""
+    import torch
+    old = torch.backends.cuda.matmul.allow_tf32
+    torch.backends.cuda.matmul.allow_tf32 = True
+    try:
+        n = 8192
+        a = torch.randn(n, n, device=dev)
+        b = torch.randn(n, n, device=dev)
+        for _ in range(3):
+            a @ b
+        torch.cuda.synchronize()
+        best = 1e9
+        for _ in range(10):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); a @ b; e1.record(); e1.synchronize()
+            best = min(best, e0.elapsed_time(e1))
+        reps = max(10, int(2000.0 / best))
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            a @ b
+        e1.record(); e1.synchronize()
+        sus = e0.elapsed_time(e1) / reps
+        fl = 2.0 * n ** 3
+        return {"burst": fl / (best * 1e-3) / 1e12, "sustained": fl / (sus * 1e-3) / 1e12}
+    finally:
+        torch.backends.cuda.matmul.allow_tf32 = old
+
+
 # ------------------------------------------------------------------------------------------------
-# the CUDA arm
+# the CUDA arm: one configuration
 # ------------------------------------------------------------------------------------------------
-def run_b200(args):
+def measure_config(cfgname, args, steps, warmup, dev, local, world, tf32_peak, with_cpu):
+    import gc
     import torch
     import torch.distributed as dist
     from paper_2606_09377_b200 import CrownContext, multi
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device; the crownb200 hot path has no CPU fallback")
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
-
-    cfg = int(args.workload[3:])
-    wl = W.stack_eps(W.make(cfg, scale=args.scale, B=args.batch or None))
-    bxs = boxes(wl)
-    B, S, nE = wl.B, wl.S, len(bxs)
-    props_per_step = B * nE
+    cfg = int(cfgname[3:])
+    wl = make_workload(cfgname, args)
+    lo, hi = wl.box()
+    B, S = wl.B, wl.S
     cap = int(args.mem_cap_gb * (1 << 30))
     if cap == 0 and cfg in (3, 4):
         cap = 64 << 30
+    free0, _ = torch.cuda.mem_get_info(dev)
     ctx = CrownContext(wl.net, B, S, device=f"cuda:{local}", mem_cap_bytes=cap,
-                       stream_weights=int(args.stream_weights), disable_epi_fusion=int(args.no_epi_fusion))
+                       stream_weights=int(args.stream_weights), disable_epi_fusion=int(args.no_epi_fusion),
+                       disable_graph=int(args.no_graph))
     inter = 1 if wl.intermediate == "ibp" else 0
 
     # ---- inputs resident in HBM -------------------------------------------------------------------
     t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
-    xlo = [t(lo) for lo, _ in bxs]
-    xhi = [t(hi) for _, hi in bxs]
-    Cd = t(wl.C)
+    xlo, xhi, Cd = t(lo), t(hi), t(wl.C)
     alpha = None if wl.alpha is None else {i: t(a) for i, a in zip(ctx.relu_ids, wl.alpha)}
     io = ctx.alloc_io(B, S)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
 
     def step_device():
-        for e in range(nE):
-            ctx.run_device(xlo[e], xhi[e], Cd, alpha, inter, io)
+        ctx.run_device(xlo, xhi, Cd, alpha, inter, io)
 
     # ---- pinned host buffers for the end-to-end leg ---------------------------------------------------
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
-    h_xlo = [pin(lo) for lo, _ in bxs]
-    h_xhi = [pin(hi) for _, hi in bxs]
-    h_C = pin(wl.C)
+    h_xlo, h_xhi, h_C = pin(lo), pin(hi), pin(wl.C)
     h_alpha = None if wl.alpha is None else [pin(a) for a in wl.alpha]
     h_lb = torch.empty(B, S).pin_memory()
     h_ub = torch.empty(B, S).pin_memory()
     h_ver = torch.empty(B, dtype=torch.uint8).pin_memory()
-    h2d = nE * (2 * B * ctx.n0 * 4 + h_C.numel() * 4 + (sum(a.numel() for a in h_alpha) * 4 if h_alpha else 0))
-    d2h = nE * (2 * B * S * 4 + B)
+    h2d = 2 * B * ctx.n0 * 4 + h_C.numel() * 4 + (sum(a.numel() for a in h_alpha) * 4 if h_alpha else 0)
+    d2h = 2 * B * S * 4 + B
 
     def step_host():
-        for e in range(nE):
-            ctx.run_host(h_xlo[e].numpy(), h_xhi[e].numpy(), h_C.numpy(),
-                         None if h_alpha is None else [a.numpy() for a in h_alpha], wl.intermediate,
-                         h_lb.numpy(), h_ub.numpy(), h_ver.numpy())
+        ctx.run_host(h_xlo.numpy(), h_xhi.numpy(), h_C.numpy(),
+                     None if h_alpha is None else [a.numpy() for a in h_alpha], wl.intermediate,
+                     h_lb.numpy(), h_ub.numpy(), h_ver.numpy())
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    def timed(fn, steps, warmup, host_clock=False):
-        for _ in range(warmup):
+    def timed(fn, n, w, host_clock=False):
+        for _ in range(w):
             fn()
         barrier()
         ms = []
-        for _ in range(steps):
+        for _ in range(n):
             flush.fill_(1)                       # L2 flush between timed iterations (outside the event pair)
             torch.cuda.synchronize()
             if host_clock:
@@ -265,25 +396,29 @@ def run_b200(args):
                 b.synchronize()
                 ms.append(a.elapsed_time(b))
         barrier()
-        return multi.max_over_ranks(sum(ms)) / steps       # the job is as slow as its slowest replica
+        return multi.max_over_ranks(sum(ms)) / n       # the job is as slow as its slowest replica
 
     clk = ClockSampler(local)
-    l0 = ctx.launch_count()
+    k0 = ctx.launch_count()
     step_device()
-    launches_per_step = ctx.launch_count() - l0
+    torch.cuda.synchronize()
+    launches_per_step = ctx.launch_count() - k0
+    free1, _ = torch.cuda.mem_get_info(dev)
     f0 = ctx.gemm_flops()
     clk.start()
-    ms_step = timed(step_device, args.steps, max(args.warmup - 1, 0))
+    ms_step = timed(step_device, steps, max(warmup - 1, 0))
     clocks = clk.stop()
-    flops_step = (ctx.gemm_flops() - f0) / (args.steps + max(args.warmup - 1, 0))
-    w_h2d_step = ctx.h2d_bytes() / (args.steps + max(args.warmup - 1, 0) + 1)
-    verified = int(io["verified"].sum().item())      # of the last eps batch
-    # end-to-end: host buffers in, host results out, wall clock around the blocking C-ABI call
-    ms_e2e = timed(step_host, args.steps, max(args.warmup, 1), host_clock=True)
+    nrun = steps + max(warmup - 1, 0)
+    flops_step = (ctx.gemm_flops() - f0) / nrun
+    w_h2d_step = ctx.h2d_bytes() / (nrun + 1)
+    verified = int(io["verified"].sum().item())
+    # long steps: the end-to-end and the instrumented legs run fewer steps (they re-measure the same kernels)
+    n_aux = steps if ms_step < 200.0 else max(2, min(steps, int(15000.0 / ms_step)))
+    ms_e2e = timed(step_host, n_aux, 1 if ms_step >= 200.0 else max(warmup, 1), host_clock=True)
 
-    # ---- per-kernel-class device times over the same steps (CUDA events around every launch) ------------
+    # ---- per-kernel-class device times (CUDA events around every launch; graph replay is off for this leg) ----------
     ctx.timing(True)
-    for _ in range(args.steps):
+    for _ in range(n_aux):
         flush.fill_(1)
         step_device()
     torch.cuda.synchronize()
@@ -294,63 +429,110 @@ def run_b200(args):
     pk = peaks()
     long_step = ms_step > 1000.0
     shares = {k: round(c["ms"] / tot_class_ms, 4) for k, c in classes.items() if c["launches"]}
-    # per kernel class: launches per step, mean device time, achieved algorithmic GB/s and TFLOP/s (bytes / flops are the
-    # library's own per-launch algorithmic counts)
-    per_class = {k: {"launches_per_step": c["launches"] / args.steps, "ms_per_step": c["ms"] / args.steps,
+    # per kernel class: launches per step, mean device time, achieved ALGORITHMIC GB/s and TFLOP/s (bytes / flops are
+    # the library's own per-launch algorithmic counts; rows shared by all branches / properties at
+    # the start of a pass are counted once)
+    per_class = {k: {"launches_per_step": c["launches"] / n_aux, "ms_per_step": c["ms"] / n_aux,
                      "gbs": (c["bytes"] / (c["ms"] * 1e-3) / 1e9) if c["ms"] > 0 and c["bytes"] > 0 else None,
                      "tflops": (c["flops"] / (c["ms"] * 1e-3) / 1e12) if c["ms"] > 0 and c["flops"] > 0 else None}
                  for k, c in classes.items() if c["launches"]}
     d = classes[dom]
     avg_ms = d["ms"] / max(d["launches"], 1)
-    if dom == "gemm_tc":
-        bf16 = pk["bf16_sustained"] if long_step else pk["bf16"]
-        peak = bf16 * TF32_OVER_BF16 / 3.0           # fp32-equivalent: 3 TF32 MMAs per useful product
-        ach = d["flops"] / d["launches"] / (avg_ms * 1e-3) / 1e12
-        # DRAM bytes per launch from the committed ncu --set full capture of this command (profiles/r1_gemm_tf32x3_cfg2.md:
-        # 202 MB read + 70 MB written per N = 256 launch at B = 192; algorithmic 4(2MK + 2KN + MN) = 302 MB, the
-        # difference is L2 hits on limbs the relax kernel just wrote); null for workloads without a committed capture
-        traffic = 2.72e8 if (cfg == 2 and args.scale == 1 and not args.batch and not args.no_epi_fusion) else None
-        roof = {"kernel": "gemm_tf32x3_kernel", "bound": "tensor", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
-                "frac": ach / peak, "traffic": traffic,
-                "peak_source": f"{pk['src']} bf16 {'sustained' if long_step else 'burst'} x nominal tf32/bf16 ratio / 3"}
+    if tf32_peak:
+        tf32 = tf32_peak["sustained"] if long_step else tf32_peak["burst"]
+        tc_peak = tf32 / 3.0
+        tc_src = f"TF32 dense measured in this run (torch.matmul 8192^3, {'sustained' if long_step else 'burst'}) / 3"
     else:
-        ach = d["bytes"] / max(d["launches"], 1) / (avg_ms * 1e-3) / 1e9
-        roof = {"kernel": dom, "bound": "hbm", "achieved": ach, "peak": pk["hbm"], "unit": "GB/s",
-                "frac": ach / pk["hbm"], "traffic": None, "peak_source": f"{pk['src']} copy bandwidth"}
-    roof["avg_launch_ms"] = avg_ms
-    roof["launches_per_step"] = d["launches"] / args.steps
-    roof["share_of_kernel_time"] = shares.get(dom)
+        bf16 = pk["bf16_sustained"] if long_step else pk["bf16"]
+        tc_peak = bf16 * TF32_OVER_BF16 / 3.0
+        tc_src = f"{pk['src']} bf16 {'sustained' if long_step else 'burst'} x nominal tf32/bf16 ratio / 3"
     g = classes["gemm_tc"]
     aw_tflops = (g["flops"] / (g["ms"] * 1e-3) / 1e12) if g["ms"] > 0 else None
+    if dom == "gemm_tc":
+        ach = d["flops"] / (d["ms"] * 1e-3) / 1e12
+        roof = {"kernel": "gemm2_tf32x3_kernel", "bound": "tensor", "achieved": ach, "peak": tc_peak, "unit": "TFLOP/s",
+                "frac": ach / tc_peak, "traffic": profiled_traffic(cfgname, "gemm2_tf32x3_kernel"), "peak_source": tc_src}
+    elif dom == "conv":
+        # CUDA-core FFMA peak: SMs x 128 lanes x 2 flop x SM clock under load
+        sm_clk = (clocks.get("sm_mhz") or 1965.0) * 1e6
+        peak = 148 * 128 * 2 * sm_clk / 1e12
+        ach = d["flops"] / (d["ms"] * 1e-3) / 1e12
+        roof = {"kernel": "conv backward / conv IBP", "bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
+                "frac": ach / peak, "traffic": profiled_traffic(cfgname, "conv"),
+                "peak_source": "148 SMs x 128 FP32 lanes x 2 x SM clock under load"}
+    else:
+        ach = d["bytes"] / (d["ms"] * 1e-3) / 1e9
+        roof = {"kernel": dom, "bound": "hbm", "achieved": ach, "peak": pk["hbm"], "unit": "GB/s",
+                "frac": ach / pk["hbm"], "traffic": profiled_traffic(cfgname, dom), "peak_source": f"{pk['src']} copy bandwidth"}
+    roof["avg_launch_ms"] = avg_ms
+    roof["launches_per_step"] = d["launches"] / n_aux
+    roof["share_of_kernel_time"] = shares.get(dom)
+    if dom != "gemm_tc" and aw_tflops:
+        roof["aw_contraction"] = {"achieved": aw_tflops, "peak": tc_peak, "frac": aw_tflops / tc_peak, "unit": "TFLOP/s"}
 
     peak_ws = ctx.peak_bytes()
     peak_torch = torch.cuda.max_memory_allocated(dev)
-
-    # ---- CPU baseline: the oracle as it stands, bounded sample, rank 0 only --------------------------------
-    cpu = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        n, secs, thr = oracle_sample(wl, bxs, args.cpu_seconds)
-        cpu = {"value": n / secs, "unit": UNIT, "cores": thr, "kind": "oracle",
-               "sample": f"first {n} of {props_per_step} properties (eps round robin), {secs:.1f} s, float64 numpy"}
-
-    if rank == 0:
-        value = world * props_per_step / (ms_step * 1e-3)
-        e2e = world * props_per_step / (ms_e2e * 1e-3)
-        print(json.dumps({
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f32 (3xTF32 products, fp32 accumulate)", "data": "synthetic",
-            "config": dict(workload_desc(wl, args.workload), l2="flushed between timed steps (256 MB write)",
-                           mem_cap_bytes=cap, stream_weights=bool(args.stream_weights), epi_fusion=not args.no_epi_fusion,
-                           streamed_layers=len(ctx.streamed_ids), weight_h2d_bytes_per_step=w_h2d_step),
-            "verified_last_batch": verified, "aw_tflops": aw_tflops, "aw_flops_per_step": flops_step,
-            "peak_hbm_gb": {"workspace_high_water": peak_ws / 1e9, "torch_max_allocated": peak_torch / 1e9},
-            "kernel_time_shares": shares, "kernel_classes": per_class,
-            "roofline": roof, "cpu_baseline": cpu,
-            "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-                    "ms_per_step": ms_e2e},
-            "gpu_launches": int(launches_per_step * args.steps), "clocks": clocks}))
+    rc_rows = ctx.row_chunk()
+    graph_on = bool(ctx.graph_active())
+    cpu = oracle_baseline(wl, cfgname, args.cpu_seconds) if with_cpu else None
+    out = {
+        "value": world * B / (ms_step * 1e-3), "unit": UNIT, "steps": steps, "ms_per_step": ms_step,
+        "config": dict(workload_desc(wl, cfgname), l2="flushed between timed steps (256 MB write)", mem_cap_bytes=cap,
+                       row_chunk=rc_rows, stream_weights=bool(args.stream_weights), epi_fusion=not args.no_epi_fusion,
+                       graph_replay=graph_on, streamed_layers=len(ctx.streamed_ids),
+                       weight_h2d_bytes_per_step=w_h2d_step),
+        "verified_last_batch": verified, "aw_tflops": aw_tflops, "aw_flops_per_step": flops_step,
+        "peak_hbm_gb": {"workspace_high_water": peak_ws / 1e9, "torch_max_allocated": peak_torch / 1e9,
+                        "cudaMemGetInfo_delta": (free0 - free1) / 1e9},
+        "kernel_time_shares": shares, "kernel_classes": per_class, "roofline": roof, "cpu_baseline": cpu,
+        "e2e": {"value": world * B / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+                "d2h_bytes_per_step": int(d2h), "ms_per_step": ms_e2e, "steps": n_aux},
+        "gpu_launches": int(launches_per_step * steps), "gpu_launches_per_step": int(launches_per_step), "clocks": clocks}
     ctx.close()
+    del ctx, xlo, xhi, Cd, alpha, io, flush, wl
+    gc.collect()
+    torch.cuda.empty_cache()
+    torch.cuda.reset_peak_memory_stats(dev)
+    return out
+
+
+def run_b200(args):
+    import torch
+    import torch.distributed as dist
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the crownb200 hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    tf32_peak = measure_tf32_peak(dev)
+    with_cpu = rank == 0 and world == 1 and not args.no_cpu_baseline
+    main = measure_config(args.workload, args, args.steps, args.warmup, dev, local, world, tf32_peak, with_cpu)
+    per = {}
+    if world == 1 and not args.no_per_config and args.scale == 1 and not args.batch:
+        for c in ALL_CFGS:
+            if c == args.workload:
+                continue
+            st = {"cfg1": max(args.steps, 20), "cfg2": max(args.steps, 10), "cfg3": min(args.steps, 3),
+                  "cfg4": min(args.steps, 5), "cfg5": max(args.steps, 10)}[c]
+            r = measure_config(c, args, st, 3, dev, local, world, tf32_peak, with_cpu)
+            per[c] = {k: r[k] for k in ("value", "unit", "steps", "ms_per_step", "config", "verified_last_batch", "aw_tflops",
+                                        "peak_hbm_gb", "kernel_time_shares", "kernel_classes", "roofline", "cpu_baseline",
+                                        "e2e", "gpu_launches_per_step", "clocks")}
+    if rank == 0:
+        line = {"metric": METRIC, "value": main["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": main["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f32 (3xTF32 products, fp32 accumulate)", "data": "synthetic"}
+        for k in ("config", "verified_last_batch", "aw_tflops", "aw_flops_per_step", "peak_hbm_gb", "kernel_time_shares",
+                  "kernel_classes", "roofline", "cpu_baseline", "e2e", "gpu_launches", "gpu_launches_per_step", "clocks"):
+            line[k] = main[k]
+        line["tf32_dense_peak_tflops"] = tf32_peak
+        line["per_config"] = per
+        print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
 

@@ -91,6 +91,9 @@ typedef struct {
                                kernel).  1: always run the separate relaxation kernel               */
   int32_t disable_conc_fusion; /* 1: always materialise A_0 and run the concretise kernel (default 0: when the
                                last contraction of a pass has a single K panel, concretise in its epilogue) */
+  int32_t disable_graph;    /* 0 (default): crown_run captures its launch sequence once per (B, S, pointer set) into
+                               a CUDA graph and replays it (the sequence depends on shapes only); 1: plain launches */
+  int32_t reserved0;        /* must be 0 */
 } crown_opts;
 
 typedef struct crown_ctx crown_ctx;   /* opaque; owned by the library; freed by crown_destroy */
@@ -162,7 +165,9 @@ int crown_run(crown_ctx* ctx, int B, const float* x_lo_dev, const float* x_hi_de
               float* lb_dev, float* ub_dev, uint8_t* verified_dev);
 
 /* Same as crown_run with HOST buffers: copies x_lo/x_hi/C/alpha H2D, runs, copies lb/ub/verified
- * D2H, synchronises.  Staging comes from the workspace.  alpha_host entries as in crown_run. */
+ * D2H, synchronises.  Staging comes from the workspace.  alpha_host entries as in crown_run.
+ * Returns CROWN_EINVAL if some x_lo > x_hi (checked here because the box is in host memory; the device-pointer
+ * entry points do not check it: NaN/Inf and inverted boxes propagate). */
 int crown_run_host(crown_ctx* ctx, int B, const float* x_lo_host, const float* x_hi_host,
                    const float* C_host, int S, const float* const* alpha_host, int intermediate,
                    float* lb_host, float* ub_host, uint8_t* verified_host);
@@ -180,7 +185,9 @@ int crown_split_tf32(crown_ctx* ctx, const float* X_dev, int rows, int cols, int
 
 /* Introspection. */
 int crown_peak_bytes(crown_ctx* ctx, size_t* out);         /* high-water mark of workspace use   */
-int crown_launch_count(crown_ctx* ctx, uint64_t* out);      /* kernels launched so far            */
+int crown_row_chunk(crown_ctx* ctx, int* out);             /* rows per chunk of identity-start passes under mem_cap */
+int crown_launch_count(crown_ctx* ctx, uint64_t* out);      /* kernels launched so far (graph replays count their kernels) */
+int crown_graph_replays(crown_ctx* ctx, uint64_t* out);     /* crown_run calls served by a CUDA-graph replay */
 int crown_gemm_flops(crown_ctx* ctx, double* out);          /* useful 2MNK flops of A.W so far    */
 int crown_h2d_bytes(crown_ctx* ctx, double* out);           /* weight bytes streamed H2D so far   */
 int crown_timing(crown_ctx* ctx, int enable);               /* 1: record CUDA events per kernel class */

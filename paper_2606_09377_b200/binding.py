@@ -19,7 +19,7 @@ OP_CODES = {"linear": 1, "conv": 2, "relu": 3, "add": 4, "flatten": 5}
 K_CLASSES = ["ibp", "coeff", "relax", "gemm_tc", "gemm_ffma", "concretize", "conv", "misc"]
 
 EXPORTS = ["crown_h2d_bytes", "crown_workspace_bytes", "crown_init", "ibp_forward", "crown_backward", "concretize", "crown_run",
-           "crown_run_host", "crown_gemm", "crown_split_tf32", "crown_peak_bytes", "crown_launch_count",
+           "crown_run_host", "crown_gemm", "crown_split_tf32", "crown_peak_bytes", "crown_row_chunk", "crown_launch_count", "crown_graph_replays",
            "crown_gemm_flops", "crown_timing", "crown_timing_read", "crown_last_error", "crown_destroy",
            "crown_version"]
 
@@ -35,7 +35,7 @@ class CrownOpts(C.Structure):
     _fields_ = [("mem_cap_bytes", C.c_uint64), ("stream_weights", C.c_int32), ("mma_scheme", C.c_int32),
                 ("slope_rule", C.c_int32), ("k_drain", C.c_int32), ("stream_min_elems", C.c_uint64),
                 ("stream_stage_bytes", C.c_uint64), ("disable_epi_fusion", C.c_int32),
-                ("disable_conc_fusion", C.c_int32)]
+                ("disable_conc_fusion", C.c_int32), ("disable_graph", C.c_int32), ("reserved0", C.c_int32)]
 
 
 class CrownError(RuntimeError):
@@ -73,7 +73,9 @@ def load_library() -> C.CDLL:
     lib.crown_gemm.argtypes = [vp, i32, i32, i32, i32, vp, vp, vp, vp, vp]
     lib.crown_split_tf32.argtypes = [vp, vp, i32, i32, i32, vp, vp]
     lib.crown_peak_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
+    lib.crown_row_chunk.argtypes = [vp, C.POINTER(C.c_int)]
     lib.crown_launch_count.argtypes = [vp, C.POINTER(C.c_uint64)]
+    lib.crown_graph_replays.argtypes = [vp, C.POINTER(C.c_uint64)]
     lib.crown_gemm_flops.argtypes = [vp, C.POINTER(C.c_double)]
     lib.crown_h2d_bytes.argtypes = [vp, C.POINTER(C.c_double)]
     lib.crown_timing.argtypes = [vp, i32]
@@ -97,7 +99,7 @@ class CrownContext:
     def __init__(self, net, B_max: int, S_max: int, device: str = "cuda:0", mem_cap_bytes: int = 0,
                  mma_scheme: int = 0, slope_rule: int = 0, k_drain: int = 0, stream_weights: int = 0,
                  stream_min_elems: int = 0, stream_stage_bytes: int = 0, disable_epi_fusion: int = 0,
-                 disable_conc_fusion: int = 0):
+                 disable_conc_fusion: int = 0, disable_graph: int = 0):
         if not torch.cuda.is_available():
             raise CrownError("no CUDA device: the crownb200 hot path has no CPU fallback")
         self.lib = load_library()
@@ -140,7 +142,7 @@ class CrownContext:
                     cn.W_dev = Wd.data_ptr()
         self._nodes = arr
         self.opts = CrownOpts(mem_cap_bytes, stream_weights, mma_scheme, slope_rule, k_drain, stream_min_elems,
-                              stream_stage_bytes, disable_epi_fusion, disable_conc_fusion)
+                              stream_stage_bytes, disable_epi_fusion, disable_conc_fusion, disable_graph, 0)
         need = C.c_size_t(0)
         self._check(self.lib.crown_workspace_bytes(arr, self.n_nodes, *self.in_chw, self.B_max, self.S_max,
                                                    C.byref(self.opts), C.byref(need)), None)
@@ -316,6 +318,21 @@ class CrownContext:
         v = C.c_size_t(0)
         self._check(self.lib.crown_peak_bytes(self.h, C.byref(v)), self.h)
         return v.value
+
+    def row_chunk(self) -> int:
+        """Rows per chunk of an identity-start pass under mem_cap_bytes (chunks start at multiples of it)."""
+        v = C.c_int(0)
+        self._check(self.lib.crown_row_chunk(self.h, C.byref(v)), self.h)
+        return v.value
+
+    def graph_replays(self) -> int:
+        v = C.c_uint64(0)
+        self._check(self.lib.crown_graph_replays(self.h, C.byref(v)), self.h)
+        return v.value
+
+    def graph_active(self) -> bool:
+        """True once crown_run has been served from a captured CUDA graph."""
+        return self.graph_replays() > 0
 
     def launch_count(self) -> int:
         v = C.c_uint64(0)

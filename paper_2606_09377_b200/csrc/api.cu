@@ -124,12 +124,17 @@ extern "C" int crown_destroy(crown_ctx* ctx) {
   for (auto& ni : ctx->nodes) { if (ni.hWt_hi) cudaFreeHost(ni.hWt_hi); if (ni.hWt_lo) cudaFreeHost(ni.hWt_lo); }
   for (int b = 0; b < 2; ++b) { if (ctx->ev_copied[b]) cudaEventDestroy(ctx->ev_copied[b]); if (ctx->ev_free[b]) cudaEventDestroy(ctx->ev_free[b]); }
   if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
+  for (auto& g : ctx->graphs) if (g.exec) cudaGraphExecDestroy(g.exec);
+  if (ctx->ev_gin) cudaEventDestroy(ctx->ev_gin);
+  if (ctx->ev_gout) cudaEventDestroy(ctx->ev_gout);
+  if (ctx->gstream) cudaStreamDestroy(ctx->gstream);
   delete ctx;
   return CROWN_OK;
 }
 extern "C" const char* crown_last_error(crown_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
 extern "C" const char* crown_version(void) { return "crownb200 0.1 (sm_100a)"; }
 extern "C" int crown_peak_bytes(crown_ctx* ctx, size_t* out) { if (!ctx || !out) return CROWN_EINVAL; *out = ctx->peak; return CROWN_OK; }
+extern "C" int crown_row_chunk(crown_ctx* ctx, int* out) { if (!ctx || !out) return CROWN_EINVAL; *out = ctx->plan.rc; return CROWN_OK; }
 extern "C" int crown_launch_count(crown_ctx* ctx, uint64_t* out) { if (!ctx || !out) return CROWN_EINVAL; *out = ctx->launches; return CROWN_OK; }
 extern "C" int crown_gemm_flops(crown_ctx* ctx, double* out) { if (!ctx || !out) return CROWN_EINVAL; *out = ctx->gemm_flops; return CROWN_OK; }
 extern "C" int crown_h2d_bytes(crown_ctx* ctx, double* out) { if (!ctx || !out) return CROWN_EINVAL; *out = ctx->h2d_bytes; return CROWN_OK; }

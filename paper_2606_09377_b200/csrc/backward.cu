@@ -69,6 +69,7 @@ int tc_contract(crown_ctx* ctx, const NodeInfo& ni, const float* hi, const float
     Scope sc(ctx, CROWN_K_GEMM_TC, 8.0 * (double)M_full * K + 8.0 * (double)K * N + out_bytes * N, 2.0 * M_full * (double)N * K);
     if (launch_gemm_tc(hi, lo, ni.Wt_hi, ni.Wt_lo, D, N, M_full, N, K, ctx->opts.k_drain, ctx->num_sms, s, &e, conc, rel))
       return fail(ctx, CROWN_ECUDA, std::string("gemm_tc: ") + (e ? e : "?"));
+    ctx->launches += gemm_tc_num_panels(K) - 1;      // the Scope counted one kernel
     return CROWN_OK;
   }
   const int ns_max = slab_rows(ctx->plan.stage_bytes, N, K, 2);
@@ -92,6 +93,7 @@ int tc_contract(crown_ctx* ctx, const NodeInfo& ni, const float* hi, const float
       if (launch_gemm_tc(hi, lo, whi, whi + (size_t)ns * K, D ? D + n0 : nullptr, N, M_full, ns, K, ctx->opts.k_drain,
                          ctx->num_sms, s, &e, conc ? &ca : nullptr, rel ? &ra : nullptr))
         return fail(ctx, CROWN_ECUDA, std::string("gemm_tc: ") + (e ? e : "?"));
+      ctx->launches += gemm_tc_num_panels(K) - 1;
       return (int)CROWN_OK;
     });
 }
@@ -348,10 +350,10 @@ extern "C" int concretize(crown_ctx* ctx, int B, int rows, const float* A_dev, c
 // ================================================================================================
 // O4 + O5 + verdict: the whole hot path for one batch
 // ================================================================================================
-extern "C" int crown_run(crown_ctx* ctx, int B, const float* x_lo_dev, const float* x_hi_dev,
-                         const float* C_dev, int S, const float* const* alpha_dev, int intermediate,
-                         float* const* l_dev, float* const* u_dev, float* lb_dev, float* ub_dev,
-                         uint8_t* verified_dev) {
+static int crown_run_enqueue(crown_ctx* ctx, int B, const float* x_lo_dev, const float* x_hi_dev,
+                             const float* C_dev, int S, const float* const* alpha_dev, int intermediate,
+                             float* const* l_dev, float* const* u_dev, float* lb_dev, float* ub_dev,
+                             uint8_t* verified_dev) {
   if (!ctx) return CROWN_EINVAL;
   const int n = (int)ctx->nodes.size();
   if (B <= 0 || B > ctx->B_max || S <= 0 || S > ctx->S_max || !x_lo_dev || !x_hi_dev || !C_dev || !l_dev ||
@@ -404,6 +406,84 @@ extern "C" int crown_run(crown_ctx* ctx, int B, const float* x_lo_dev, const flo
   return CROWN_OK;
 }
 
+
+// ---- CUDA-graph replay of crown_run ------------------------------------------------------------------------------
+// The launch sequence of a step depends only on shapes and pointers, never on data, so a step is captured once per
+// (B, S, intermediate, pointer set) into a CUDA graph and replayed: one cudaGraphLaunch instead of 12-70 kernel
+// launches.  For the latency-bound configs (cfg1: ~0.2 GFLOP behind a dozen dependent launches) the host launch
+// path is the step time.  Capture needs a capturable stream: when the caller gave the legacy default stream, the
+// graph runs on a side stream joined to it by events.  Streamed layers (side-stream copies) and timing mode bypass it.
+static bool graph_eligible(crown_ctx* ctx) {
+  if (ctx->opts.disable_graph || ctx->timing) return false;
+  for (const auto& ni : ctx->nodes) if (ni.streamed) return false;
+  return true;
+}
+
+extern "C" int crown_run(crown_ctx* ctx, int B, const float* x_lo_dev, const float* x_hi_dev,
+                         const float* C_dev, int S, const float* const* alpha_dev, int intermediate,
+                         float* const* l_dev, float* const* u_dev, float* lb_dev, float* ub_dev,
+                         uint8_t* verified_dev) {
+  if (!ctx) return CROWN_EINVAL;
+  if (!graph_eligible(ctx) || !l_dev || !u_dev)
+    return crown_run_enqueue(ctx, B, x_lo_dev, x_hi_dev, C_dev, S, alpha_dev, intermediate, l_dev, u_dev, lb_dev, ub_dev, verified_dev);
+  const int n = (int)ctx->nodes.size();
+  std::vector<uintptr_t> key;
+  key.reserve(8 + 3 * n);
+  key.push_back((uintptr_t)B); key.push_back((uintptr_t)S); key.push_back((uintptr_t)intermediate);
+  for (const void* q : {(const void*)x_lo_dev, (const void*)x_hi_dev, (const void*)C_dev, (const void*)lb_dev,
+                        (const void*)ub_dev, (const void*)verified_dev}) key.push_back((uintptr_t)q);
+  for (int i = 0; i < n; ++i) {
+    key.push_back((uintptr_t)l_dev[i]); key.push_back((uintptr_t)u_dev[i]);
+    key.push_back(alpha_dev ? (uintptr_t)alpha_dev[i] : 0);
+  }
+  const bool legacy = ctx->stream == nullptr || ctx->stream == cudaStreamLegacy;
+  cudaStream_t user = ctx->stream;
+  if (legacy && !ctx->gstream) {
+    CK(ctx, cudaStreamCreateWithFlags(&ctx->gstream, cudaStreamNonBlocking));
+    CK(ctx, cudaEventCreateWithFlags(&ctx->ev_gin, cudaEventDisableTiming));
+    CK(ctx, cudaEventCreateWithFlags(&ctx->ev_gout, cudaEventDisableTiming));
+  }
+  cudaStream_t gs = legacy ? ctx->gstream : user;
+  GraphEntry* ge = nullptr;
+  for (auto& e : ctx->graphs) if (e.key == key) { ge = &e; break; }
+  if (!ge) {
+    // capture: the normal enqueue path runs with the capture stream as the context's stream; nothing executes yet
+    GraphEntry e; e.key = key;
+    const uint64_t l0 = ctx->launches; const double f0 = ctx->gemm_flops;
+    ctx->stream = gs;
+    cudaError_t ce = cudaStreamBeginCapture(gs, cudaStreamCaptureModeThreadLocal);
+    int rc = CROWN_OK;
+    if (ce == cudaSuccess) {
+      rc = crown_run_enqueue(ctx, B, x_lo_dev, x_hi_dev, C_dev, S, alpha_dev, intermediate, l_dev, u_dev, lb_dev, ub_dev, verified_dev);
+      cudaGraph_t g = nullptr;
+      ce = cudaStreamEndCapture(gs, &g);
+      if (rc == CROWN_OK && ce == cudaSuccess && g) ce = cudaGraphInstantiate(&e.exec, g, 0);
+      if (g) cudaGraphDestroy(g);
+    }
+    ctx->stream = user;
+    e.launches = ctx->launches - l0; e.flops = ctx->gemm_flops - f0;
+    ctx->launches = l0; ctx->gemm_flops = f0;
+    if (rc != CROWN_OK) { (void)cudaGetLastError(); return rc; }
+    if (ce != cudaSuccess || !e.exec) {
+      // capture not possible here (e.g. an uncapturable stream): run the plain path from now on
+      (void)cudaGetLastError();
+      ctx->opts.disable_graph = 1;
+      return crown_run_enqueue(ctx, B, x_lo_dev, x_hi_dev, C_dev, S, alpha_dev, intermediate, l_dev, u_dev, lb_dev, ub_dev, verified_dev);
+    }
+    if (ctx->graphs.size() >= 8) { cudaGraphExecDestroy(ctx->graphs.front().exec); ctx->graphs.erase(ctx->graphs.begin()); }
+    ctx->graphs.push_back(e);
+    ge = &ctx->graphs.back();
+  }
+  if (legacy) { CK(ctx, cudaEventRecord(ctx->ev_gin, user)); CK(ctx, cudaStreamWaitEvent(gs, ctx->ev_gin, 0)); }
+  CK(ctx, cudaGraphLaunch(ge->exec, gs));
+  if (legacy) { CK(ctx, cudaEventRecord(ctx->ev_gout, gs)); CK(ctx, cudaStreamWaitEvent(user, ctx->ev_gout, 0)); }
+  ctx->launches += ge->launches; ctx->gemm_flops += ge->flops;
+  ctx->graph_replays++;
+  return CROWN_OK;
+}
+
+extern "C" int crown_graph_replays(crown_ctx* ctx, uint64_t* out) { if (!ctx || !out) return CROWN_EINVAL; *out = ctx->graph_replays; return CROWN_OK; }
+
 extern "C" int crown_run_host(crown_ctx* ctx, int B, const float* x_lo_host, const float* x_hi_host,
                               const float* C_host, int S, const float* const* alpha_host, int intermediate,
                               float* lb_host, float* ub_host, uint8_t* verified_host) {
@@ -411,6 +491,10 @@ extern "C" int crown_run_host(crown_ctx* ctx, int B, const float* x_lo_host, con
   const int n = (int)ctx->nodes.size();
   if (B <= 0 || B > ctx->B_max || S <= 0 || S > ctx->S_max || !x_lo_host || !x_hi_host || !C_host || !lb_host || !ub_host)
     return fail(ctx, CROWN_EINVAL, "crown_run_host: bad arguments");
+  // the box is in host memory here, so x_lo <= x_hi is checked (CROWN_EINVAL); the device-pointer
+  // entry points do not check it (it would need a device->host sync) and propagate whatever they are given
+  for (size_t k = 0; k < (size_t)B * ctx->n0; ++k)
+    if (x_lo_host[k] > x_hi_host[k]) return fail(ctx, CROWN_EINVAL, "crown_run_host: x_lo > x_hi");
   cudaStream_t s = ctx->stream;
   uint8_t* cur = ctx->io_base;
   auto take = [&](size_t bytes) { uint8_t* p = cur; cur += align_up(bytes); return p; };
@@ -469,6 +553,7 @@ extern "C" int crown_gemm(crown_ctx* ctx, int scheme, int M, int N, int K, const
     Scope sc(ctx, CROWN_K_GEMM_TC, 4.0 * ((double)M * K + (double)K * N + (double)M * N), 2.0 * M * (double)N * K);
     if (launch_gemm_tc(A_hi_dev, A_lo_dev, Wt_hi_dev, Wt_lo_dev, D_dev, N, M, N, K, ctx->opts.k_drain, ctx->num_sms, ctx->stream, &e))
       return fail(ctx, CROWN_EINVAL, std::string("crown_gemm: ") + (e ? e : "?"));
+    ctx->launches += gemm_tc_num_panels(K) - 1;
   } else if (scheme == 2) {
     // FFMA path takes W [K,N] row-major in Wt_hi_dev (NOT transposed) and fp32 A in A_hi_dev
     Scope sc(ctx, CROWN_K_GEMM_FFMA, 4.0 * ((double)M * K + (double)K * N + (double)M * N), 2.0 * M * (double)N * K);

@@ -45,6 +45,9 @@ struct Plan {
 
 struct TimingRec { cudaEvent_t a, b; int cls; double bytes, flops; };
 
+// one captured step of crown_run: key = (B, S, intermediate, every pointer argument)
+struct GraphEntry { std::vector<uintptr_t> key; cudaGraphExec_t exec = nullptr; uint64_t launches = 0; double flops = 0; };
+
 }  // namespace
 
 struct crown_ctx {
@@ -74,6 +77,11 @@ struct crown_ctx {
   bool timing = false;
   std::vector<TimingRec> recs;
   std::vector<cudaEvent_t> free_events;
+  // CUDA-graph replay of crown_run
+  std::vector<GraphEntry> graphs;
+  cudaStream_t gstream = nullptr;            // capture / replay stream when the caller's stream is the legacy default
+  cudaEvent_t ev_gin = nullptr, ev_gout = nullptr;
+  uint64_t graph_replays = 0;
   // weight streaming
   cudaStream_t copy_stream = nullptr;
   uint8_t* stage[2] = {nullptr, nullptr};

@@ -425,6 +425,13 @@ int gemm_tc_parts(int N_total) { return (N_total + 31) / 32; }
 
 int gemm_tc_single_panel(int K) { return 18LL * 256 * 8 * K <= (96LL << 20); }
 
+int gemm_tc_num_panels(int K) {     // kernel launches of one contraction (same rule as launch_pair)
+  if (gemm_tc_single_panel(K)) return 1;
+  int kp = (int)((64LL << 20) / (18LL * 256 * 8)) / 512 * 512;
+  if (kp < 1024) kp = 1024;
+  return (K + kp - 1) / kp;
+}
+
 static bool mis16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) != 0; }
 
 int launch_gemm_tc(const float* A_hi, const float* A_lo, const float* Wt_hi, const float* Wt_lo, float* D,

@@ -100,6 +100,7 @@ struct RelaxEpiArgs {
 };
 int gemm_tc_parts(int N_total);                // 32-column pieces per row of an N_total-wide output
 int gemm_tc_single_panel(int K);               // 1 if the contraction runs as one K panel (fused epilogues allowed)
+int gemm_tc_num_panels(int K);                 // kernel launches of one contraction over K
 void launch_concretize_parts(const float* part, int parts, const float* d, float* lb, float* ub, int out_stride,
                              int B, int R, cudaStream_t s);
 // d[m] += part[m*parts + 0] + part[m*parts + 1] + ... (index order), m < rows

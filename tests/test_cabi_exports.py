@@ -45,9 +45,9 @@ def test_binding_binds_exactly_the_declared_symbols():
 
 def test_struct_layouts_match_the_header():
     from paper_2606_09377_b200 import binding
-    # crown_node: 13 int32 + 3 pointers; crown_opts: u64, 4 x i32, u64, u64, i32 (+ tail padding)
+    # crown_node: 13 int32 + 3 pointers; crown_opts: u64, 4 x i32, u64, u64, 4 x i32
     assert ctypes.sizeof(binding.CrownNode) == 13 * 4 + 4 + 3 * 8
-    assert ctypes.sizeof(binding.CrownOpts) == 8 + 4 * 4 + 8 + 8 + 8          # ..., disable_epi_fusion, disable_conc_fusion
+    assert ctypes.sizeof(binding.CrownOpts) == 8 + 4 * 4 + 8 + 8 + 4 * 4      # ..., disable_epi_fusion, disable_conc_fusion, disable_graph, reserved
     assert binding.CrownOpts.stream_min_elems.offset == 24 and binding.CrownOpts.disable_epi_fusion.offset == 40
 
 

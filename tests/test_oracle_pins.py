@@ -429,3 +429,29 @@ def test_residual_dag_affine_exactness():
             for x in X:
                 z = O.forward(net, x)[i]
                 assert np.all(z >= ib[i][0] - 1e-12) and np.all(z <= ib[i][1] + 1e-12)
+
+
+# ------------------------------------------------------------------------------------------ verdict and box helpers
+def test_verified_is_strict_and_fails_closed():
+    """a property is proved iff EVERY margin row is strictly positive; an undefined (NaN) bound
+    proves nothing."""
+    assert O.verified(np.array([0.5, 1e-30, 3.0])) is True
+    assert O.verified(np.array([0.5, 0.0, 3.0])) is False          # strict: lb = 0 is not a proof
+    assert O.verified(np.array([0.5, -1e-30, 3.0])) is False
+    assert O.verified(np.array([np.nan, 1.0])) is False
+    assert O.verified(np.array([np.inf])) is True
+
+
+def test_box_is_x0_plus_minus_the_float32_radius():
+    """_box(x0, eps): corners are float32(x0 -+ float32(eps)) with the subtraction done in float64, the same
+    rounding as workloads.Workload.box (hand values: 0.5 -+ 0.25 exactly; 0.1 is not a float32 number)."""
+    x0 = np.array([[0.5, -1.0]], dtype=np.float32)
+    lo, hi = O._box(x0, 0.25)
+    assert lo.dtype == np.float32 and hi.dtype == np.float32
+    assert lo.tolist() == [[0.25, -1.25]] and hi.tolist() == [[0.75, -0.75]]
+    lo, hi = O._box(x0, 0.1)
+    e32 = 0.100000001490116119384765625                              # float32(0.1), written out
+    assert lo[0, 0] == np.float32(0.5 - e32) and hi[0, 1] == np.float32(-1.0 + e32)
+    wl = wl_mod.small_mlp([4, 4, 2], 0, eps=0.1)
+    l2, h2 = O._box(wl.x0, 0.1)
+    assert np.array_equal(l2, wl.box()[0]) and np.array_equal(h2, wl.box()[1])
