@@ -172,7 +172,7 @@ def oracle_final_time(wl, p=0):
 
 
 LARGE = ("cfg3", "cfg4")
-F1, F2 = 1.0 / 512, 1.0 / 128          # row fractions of the two sampled runs (cfg3: 32 and 128 of 16384 rows)
+F1, F2 = 1.0 / 64, 1.0 / 16            # row fractions of the two sampled runs (cfg3: 256 and 1024 of 16384 rows)
 
 
 def oracle_baseline(wl, cfgname, budget_s):
@@ -438,14 +438,16 @@ def measure_config(cfgname, args, steps, warmup, dev, local, world, tf32_peak, w
                  for k, c in classes.items() if c["launches"]}
     d = classes[dom]
     avg_ms = d["ms"] / max(d["launches"], 1)
-    if tf32_peak:
-        tf32 = tf32_peak["sustained"] if long_step else tf32_peak["burst"]
-        tc_peak = tf32 / 3.0
-        tc_src = f"TF32 dense measured in this run (torch.matmul 8192^3, {'sustained' if long_step else 'burst'}) / 3"
-    else:
-        bf16 = pk["bf16_sustained"] if long_step else pk["bf16"]
-        tc_peak = bf16 * TF32_OVER_BF16 / 3.0
-        tc_src = f"{pk['src']} bf16 {'sustained' if long_step else 'burst'} x nominal tf32/bf16 ratio / 3"
+    # fp32-equivalent tensor peak = TF32 dense / 3 (three TF32 MMAs per useful product).  Two estimates of the TF32 dense
+    # rate: measured in this run (cuBLAS TF32 8192^3) and the driver-measured bf16 rate x the nominal TF32/bf16 ratio;
+    # the LARGER one is the denominator (cuBLAS TF32 measured below half of its bf16 rate on this pool)
+    which = "sustained" if long_step else "burst"
+    bf16 = pk["bf16_sustained"] if long_step else pk["bf16"]
+    tf32_nom = bf16 * TF32_OVER_BF16
+    tf32_meas = tf32_peak[which] if tf32_peak else 0.0
+    tc_peak = max(tf32_meas, tf32_nom) / 3.0
+    tc_src = (f"max(TF32 dense measured in this run {tf32_meas:.0f}, {pk['src']} bf16 {bf16:.0f} x nominal ratio "
+              f"{TF32_OVER_BF16:.3f} = {tf32_nom:.0f}) TFLOP/s {which} / 3")
     g = classes["gemm_tc"]
     aw_tflops = (g["flops"] / (g["ms"] * 1e-3) / 1e12) if g["ms"] > 0 else None
     if dom == "gemm_tc":

@@ -215,7 +215,7 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
           int r = nd.in0, j = -1;
           bool fr = false;
           if (!fc && r >= 0 && ctx->nodes[r].n.op == CROWN_RELU && ctx->nodes[r].n_consumers == 1 &&
-              ps.pend.find(r) == ps.pend.end() && !ctx->opts.disable_epi_fusion && single &&
+              ps.pend.find(r) == ps.pend.end() && !ctx->opts.disable_epi_fusion && single && (R % 32) == 0 &&
               !(alpha_lo && alpha_lo[r]) && !(alpha_up && alpha_up[r]) && (size_t)M_full * parts * 4 <= ctx->plan.part_bytes) {
             j = ctx->nodes[r].n.in0;
             fr = j >= 0 && ctx->nodes[j].n.op == CROWN_LINEAR && ctx->nodes[j].tc_ok &&

@@ -55,6 +55,12 @@ constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + EPI_STAGE_BYTES + 1024 /*align
 
 enum { EPI_STORE = 0, EPI_ADD = 1, EPI_RELAX = 2, EPI_CONC = 3 };
 
+// round-to-nearest (ties away) to TF32 on the bit pattern: the arithmetic of cvt.rna.tf32.f32 for finite inputs in
+// two integer instructions (the PTX conversion compiles to a longer sequence that also handles NaN payloads)
+__device__ __forceinline__ float tf32_rn_bits(float x) {
+  return __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xffffe000u);
+}
+
 struct EpiArgs {
   int mode = EPI_STORE;
   int B = 0, R = 0;              // row m -> branch m / (B*R), property (m / R) % B
@@ -65,6 +71,7 @@ struct EpiArgs {
   const float4* coef = nullptr;  // [B, coef_ld] {dU, bU, dL, unstable}
   long long coef_ld = 0;
   const float* bias = nullptr;   // bias of the Linear below the ReLU, [coef_ld], or nullptr
+  float* out_hi = nullptr; float* out_lo = nullptr; long long ldd = 0;   // limbs of the relaxed product (this launch's slab)
   // EPI_CONC
   const float* x_lo = nullptr; const float* x_hi = nullptr; int ldx = 0;
 };
@@ -217,113 +224,174 @@ gemm2_tf32x3_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_con
         }
         tcgen05_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive_cluster(accempty_remote[buf]);
+        if (lane == 0) mbar_arrive_cluster_relaxed(accempty_remote[buf]);
         ++cnt;
       }
       const int row = mb * PAIR_M + (int)rank * BM + quad * 32 + lane;       // this thread's output row
       const int row0 = mb * PAIR_M + (int)rank * BM + quad * 32;             // first row of the warp's slab
       const int tcol0 = nb * BN + chalf * EC;                                 // first column of the warp (in this launch)
+      const bool rok = row < M;
+      const int rr = rok ? row : 0;
+      // do the warp's 32 rows share (branch, property)?  Always for identity passes with R % 32 == 0 (the hot case).
+      const bool uni = (ea.R & 31) == 0;
 
       if (ea.mode == EPI_CONC) {
         // a8 fused: 32-column pieces of this row against the box of the row's property; A_0 is never stored
-        if (row < M) {
-          const int b = (row / ea.R) % ea.B;
-          const float* xl = ea.x_lo + (long long)b * ea.ldx + ea.col_off;
-          const float* xh = ea.x_hi + (long long)b * ea.ldx + ea.col_off;
-          float2* prow = reinterpret_cast<float2*>(ea.part) + (long long)row * ea.parts + (ea.col_off >> 5);
+        const int b = (rr / ea.R) % ea.B;
+        const float* xl = ea.x_lo + (long long)b * ea.ldx + ea.col_off;
+        const float* xh = ea.x_hi + (long long)b * ea.ldx + ea.col_off;
+        float2* prow = reinterpret_cast<float2*>(ea.part) + (long long)rr * ea.parts + (ea.col_off >> 5);
 #pragma unroll
-          for (int sl = 0; sl < EC / 32; ++sl) {
-            const int col = tcol0 + sl * 32;
-            if (chalf * EC + sl * 32 < BN && col < N) {
-              float dot = 0.f, ab = 0.f;
+        for (int sl = 0; sl < EC / 32; ++sl) {
+          const int col = tcol0 + sl * 32;
+          if (chalf * EC + sl * 32 >= BN || col >= N) continue;            // warp-uniform
+          float dot = 0.f, ab = 0.f;
+          if (uni) {
+            // box centre / radius of the 32 columns: loaded once per warp (lane = column), read back as broadcasts
+            float2 cr = make_float2(0.f, 0.f);
+            if (col + lane < N) { const float l = __ldg(xl + col + lane), h = __ldg(xh + col + lane); cr = make_float2(0.5f * (l + h), 0.5f * (h - l)); }
+            __syncwarp();
+            asm volatile("st.shared.v2.f32 [%0], {%1,%2};" :: "r"(slab_base + (uint32_t)lane * 8u), "f"(cr.x), "f"(cr.y) : "memory");
+            __syncwarp();
 #pragma unroll
-              for (int i = 0; i < 32; i += 4) {
-                if (col + i < N) {                     // N % 4 == 0: whole float4 in range
-                  const float4 lo = __ldg(reinterpret_cast<const float4*>(xl + col + i));
-                  const float4 hi = __ldg(reinterpret_cast<const float4*>(xh + col + i));
-                  const float a0 = acc[sl * 32 + i], a1 = acc[sl * 32 + i + 1], a2 = acc[sl * 32 + i + 2], a3 = acc[sl * 32 + i + 3];
-                  dot = fmaf(a0, 0.5f * (lo.x + hi.x), dot); ab = fmaf(fabsf(a0), 0.5f * (hi.x - lo.x), ab);
-                  dot = fmaf(a1, 0.5f * (lo.y + hi.y), dot); ab = fmaf(fabsf(a1), 0.5f * (hi.y - lo.y), ab);
-                  dot = fmaf(a2, 0.5f * (lo.z + hi.z), dot); ab = fmaf(fabsf(a2), 0.5f * (hi.z - lo.z), ab);
-                  dot = fmaf(a3, 0.5f * (lo.w + hi.w), dot); ab = fmaf(fabsf(a3), 0.5f * (hi.w - lo.w), ab);
-                }
+            for (int i = 0; i < 32; ++i) {
+              float2 c;
+              asm volatile("ld.shared.v2.f32 {%0,%1}, [%2];" : "=f"(c.x), "=f"(c.y) : "r"(slab_base + (uint32_t)i * 8u));
+              const float a = acc[sl * 32 + i];
+              dot = fmaf(a, c.x, dot); ab = fmaf(fabsf(a), c.y, ab);
+            }
+          } else {
+#pragma unroll
+            for (int i = 0; i < 32; i += 4) {
+              if (col + i < N) {                     // N % 4 == 0: whole float4 in range
+                const float4 lo = __ldg(reinterpret_cast<const float4*>(xl + col + i));
+                const float4 hi = __ldg(reinterpret_cast<const float4*>(xh + col + i));
+                const float a0 = acc[sl * 32 + i], a1 = acc[sl * 32 + i + 1], a2 = acc[sl * 32 + i + 2], a3 = acc[sl * 32 + i + 3];
+                dot = fmaf(a0, 0.5f * (lo.x + hi.x), dot); ab = fmaf(fabsf(a0), 0.5f * (hi.x - lo.x), ab);
+                dot = fmaf(a1, 0.5f * (lo.y + hi.y), dot); ab = fmaf(fabsf(a1), 0.5f * (hi.y - lo.y), ab);
+                dot = fmaf(a2, 0.5f * (lo.z + hi.z), dot); ab = fmaf(fabsf(a2), 0.5f * (hi.z - lo.z), ab);
+                dot = fmaf(a3, 0.5f * (lo.w + hi.w), dot); ab = fmaf(fabsf(a3), 0.5f * (hi.w - lo.w), ab);
               }
-              prow[col >> 5] = make_float2(dot, ab);
+            }
+          }
+          if (rok) prow[col >> 5] = make_float2(dot, ab);
+        }
+        continue;
+      }
+
+      if (ea.mode == EPI_RELAX) {
+        // a4 fused: lower: Abar = A+ dL + A- dU, d += A- . bU; upper: Abar = A+ dU + A- dL,
+        // d += A+ . bU; both: d += Abar . b.  One fp32 partial per (row, 32-column piece), summed in index order later.
+        // Host side guarantees R % 32 == 0: the warp's 32 rows share (branch, property).  The warp's 4 KB slab is used
+        // three times in turn: (1) the 32 columns' {slope for a > 0, slope for a <= 0, bU, bias}, loaded once per warp
+        // (lane = column) and read back as broadcasts; (2) the hi limbs and (3) the lo limbs, written row-per-lane
+        // (swizzled, conflict-free) and read back four rows per warp instruction, so the global stores are full
+        // 128-byte row segments.
+        const bool upper = rr >= BR;
+        const float4* crow = ea.coef + (long long)((rr / ea.R) % ea.B) * ea.coef_ld + ea.col_off;
+#pragma unroll
+        for (int sl = 0; sl < EC / 32; ++sl) {
+          const int col = tcol0 + sl * 32;
+          if (chalf * EC + sl * 32 >= BN || col >= N) continue;            // warp-uniform
+          float4 cf = make_float4(0.f, 0.f, 0.f, 0.f);
+          if (col + lane < N) {
+            const float4 c = __ldg(crow + col + lane);                      // {dU, bU, dL, unstable}
+            cf = make_float4(upper ? c.x : c.z, upper ? c.z : c.x, c.y, ea.bias ? __ldg(ea.bias + ea.col_off + col + lane) : 0.f);
+          }
+          __syncwarp();
+          asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};"
+                       :: "r"(slab_base + (uint32_t)lane * 16u), "f"(cf.x), "f"(cf.y), "f"(cf.z), "f"(cf.w) : "memory");
+          __syncwarp();
+          float hi[32], dsum = 0.f;
+#pragma unroll
+          for (int i = 0; i < 32; ++i) {
+            float4 c;
+            asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(c.x), "=f"(c.y), "=f"(c.z), "=f"(c.w) : "r"(slab_base + (uint32_t)i * 16u));
+            const float a = acc[sl * 32 + i];
+            const float o = a * (a > 0.f ? c.x : c.y);     // == A+ s_pos + A- s_neg (one of the two terms is +-0)
+            dsum = fmaf(upper ? fmaxf(a, 0.f) : fminf(a, 0.f), c.z, dsum);
+            dsum = fmaf(o, c.w, dsum);
+            hi[i] = tf32_rn_bits(o);
+            acc[sl * 32 + i] = tf32_rn_bits(o - hi[i]);    // lo limb, kept in the accumulator registers
+          }
+          if (rok) ea.part[(long long)row * ea.parts + ((ea.col_off + col) >> 5)] = dsum;
+#pragma unroll
+          for (int limb = 0; limb < 2; ++limb) {
+            __syncwarp();                                   // the slab's previous contents have been read by every lane
+#pragma unroll
+            for (int c4 = 0; c4 < 8; ++c4) {
+              const int i = sl * 32 + c4 * 4;
+              if (limb == 0)
+                asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};"
+                             :: "r"(slab + (((uint32_t)c4 ^ sw) << 4)), "f"(hi[c4 * 4]), "f"(hi[c4 * 4 + 1]), "f"(hi[c4 * 4 + 2]), "f"(hi[c4 * 4 + 3]) : "memory");
+              else
+                asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};"
+                             :: "r"(slab + (((uint32_t)c4 ^ sw) << 4)), "f"(acc[i]), "f"(acc[i + 1]), "f"(acc[i + 2]), "f"(acc[i + 3]) : "memory");
+            }
+            __syncwarp();
+            float* outp = limb == 0 ? ea.out_hi : ea.out_lo;
+            const int c4 = lane & 7;
+#pragma unroll
+            for (int it = 0; it < 8; ++it) {
+              const int r = it * 4 + (lane >> 3);
+              float4 v;
+              asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
+                           : "r"(slab_base + (uint32_t)r * 128u + (((uint32_t)c4 ^ (uint32_t)(r & 7)) << 4)));
+              if (row0 + r < M && col + c4 * 4 < N)
+                stg_stream4(outp + (long long)(row0 + r) * ea.ldd + col + c4 * 4, v);
             }
           }
         }
         continue;
       }
 
-      // row -> (branch, property) for the relaxation coefficients
-      const bool rok = row < M;
-      const int rr = rok ? row : 0;
-      const bool upper = rr >= BR;
-      const float4* crow = nullptr;
-      if (ea.mode == EPI_RELAX) crow = ea.coef + (long long)((rr / ea.R) % ea.B) * ea.coef_ld + ea.col_off;
+      if (ea.mode == EPI_STORE) {
+        // product -> global: row-per-lane into the swizzled slab, read back four rows per warp instruction, stored as
+        // full 128-byte row segments (no asynchronous store to wait for: short-K tiles stay MMA-bound)
+#pragma unroll
+        for (int sl = 0; sl < EC / 32; ++sl) {
+          const int col = tcol0 + sl * 32;
+          if (chalf * EC + sl * 32 >= BN || col >= N) continue;            // warp-uniform
+          __syncwarp();
+#pragma unroll
+          for (int c4 = 0; c4 < 8; ++c4) {
+            const int i = sl * 32 + c4 * 4;
+            asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};"
+                         :: "r"(slab + (((uint32_t)c4 ^ sw) << 4)), "f"(acc[i]), "f"(acc[i + 1]), "f"(acc[i + 2]), "f"(acc[i + 3]) : "memory");
+          }
+          __syncwarp();
+          const int c4 = lane & 7;
+#pragma unroll
+          for (int it = 0; it < 8; ++it) {
+            const int r = it * 4 + (lane >> 3);
+            float4 v;
+            asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
+                         : "r"(slab_base + (uint32_t)r * 128u + (((uint32_t)c4 ^ (uint32_t)(r & 7)) << 4)));
+            if (row0 + r < M && col + c4 * 4 < N)
+              stg_stream4(ea.out_hi + (long long)(row0 + r) * ea.ldd + col + c4 * 4, v);
+          }
+        }
+        continue;
+      }
 
+      // EPI_ADD (K panels after the first): D += tile through shared memory and the TMA's fp32 reduce-add; lane = row
+      // writes its 32 columns of a slab in the 128B-swizzled layout, one lane issues the bulk tensor reduction, which
+      // also clips the M / N edges
 #pragma unroll
       for (int sl = 0; sl < EC / 32; ++sl) {
         const int col = tcol0 + sl * 32;
-        if (chalf * EC + sl * 32 >= BN || col >= N) continue;        // warp-uniform
-        if (ea.mode == EPI_RELAX) {
-          // a4 fused: lower: Abar = A+ dL + A- dU, d += A- . bU; upper: Abar = A+ dU + A- dL,
-          // d += A+ . bU; both: d += Abar . b.  One fp32 partial per (row, 32-column piece), summed in index order later.
-          float hi[32], dsum = 0.f;
+        if (chalf * EC + sl * 32 >= BN || col >= N) continue;              // warp-uniform
+        if (lane == 0) bulk_wait_read0();          // the previous reduction has finished reading this warp's slab
+        __syncwarp();
 #pragma unroll
-          for (int i = 0; i < 32; ++i) {
-            float o = 0.f;
-            if (col + i < N) {
-              const float4 cf = __ldg(crow + col + i);
-              const float a = acc[sl * 32 + i];
-              const float pos = fmaxf(a, 0.f), neg = fminf(a, 0.f);
-              const float sp = upper ? cf.x : cf.z, sn = upper ? cf.z : cf.x;
-              o = pos * sp + neg * sn;
-              dsum = fmaf(upper ? pos : neg, cf.y, dsum);
-              if (ea.bias) dsum = fmaf(o, __ldg(ea.bias + ea.col_off + col + i), dsum);
-            }
-            hi[i] = tf32_rna(o);
-            acc[sl * 32 + i] = tf32_rna(o - hi[i]);       // lo limb, kept in the accumulator registers
-          }
-          if (rok) ea.part[(long long)row * ea.parts + ((ea.col_off + col) >> 5)] = dsum;
-          if (lane == 0) bulk_wait_read0();
-          __syncwarp();
-#pragma unroll
-          for (int c4 = 0; c4 < 8; ++c4)
-            asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};"
-                         :: "r"(slab + (((uint32_t)c4 ^ sw) << 4)), "f"(hi[c4 * 4]), "f"(hi[c4 * 4 + 1]), "f"(hi[c4 * 4 + 2]), "f"(hi[c4 * 4 + 3]) : "memory");
-          fence_proxy_async();
-          __syncwarp();
-          if (lane == 0) { tma_store_2d(&tmD, slab_base, col, row0); bulk_commit(); bulk_wait_read0(); }
-          __syncwarp();
-#pragma unroll
-          for (int c4 = 0; c4 < 8; ++c4) {
-            const int i = sl * 32 + c4 * 4;
-            asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};"
-                         :: "r"(slab + (((uint32_t)c4 ^ sw) << 4)), "f"(acc[i]), "f"(acc[i + 1]), "f"(acc[i + 2]), "f"(acc[i + 3]) : "memory");
-          }
-          fence_proxy_async();
-          __syncwarp();
-          if (lane == 0) { tma_store_2d(&tmD_lo, slab_base, col, row0); bulk_commit(); }
-        } else {
-          // tile -> global through shared memory and the TMA: lane = row writes its 32 columns (128 B) of a slab in the
-          // 128B-swizzled layout (conflict-free), one lane issues the bulk tensor store, which also clips the M / N edges
-          if (lane == 0) bulk_wait_read0();          // the previous store has finished reading this warp's slab
-          __syncwarp();
-#pragma unroll
-          for (int c4 = 0; c4 < 8; ++c4) {
-            const int i = sl * 32 + c4 * 4;
-            asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};"
-                         :: "r"(slab + (((uint32_t)c4 ^ sw) << 4)), "f"(acc[i]), "f"(acc[i + 1]), "f"(acc[i + 2]), "f"(acc[i + 3]) : "memory");
-          }
-          fence_proxy_async();
-          __syncwarp();
-          if (lane == 0) {
-            if (ea.mode == EPI_ADD) tma_reduce_add_2d(&tmD, slab_base, col, row0);
-            else tma_store_2d(&tmD, slab_base, col, row0);
-            bulk_commit();
-          }
+        for (int c4 = 0; c4 < 8; ++c4) {
+          const int i = sl * 32 + c4 * 4;
+          asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};"
+                       :: "r"(slab + (((uint32_t)c4 ^ sw) << 4)), "f"(acc[i]), "f"(acc[i + 1]), "f"(acc[i + 2]), "f"(acc[i + 3]) : "memory");
         }
+        fence_proxy_async();
+        __syncwarp();
+        if (lane == 0) { tma_reduce_add_2d(&tmD, slab_base, col, row0); bulk_commit(); }
       }
     }
     if (lane == 0) bulk_wait0();
@@ -350,10 +418,14 @@ static int launch_pair(const float* A_hi, const float* A_lo, const float* Wt_hi,
   int BN = ((N + n_blocks - 1) / n_blocks + 31) / 32 * 32;
   if (BN > BN_MAX) BN = BN_MAX;
   if (BN < 32) BN = 32;
-  const int m_tiles = (M + PAIR_M - 1) / PAIR_M, n_tiles = (N + BN - 1) / BN;
-  const long long tiles = (long long)m_tiles * n_tiles;
   int clusters = num_sms / 2;
   if (g_max_clusters > 0 && clusters > g_max_clusters) clusters = g_max_clusters;
+  const int m_tiles = (M + PAIR_M - 1) / PAIR_M;
+  // small problems (cfg1: M = 512, latency-bound): narrower tiles put more CTA pairs to work and shorten the
+  // per-tile MMA chain; the per-element summation order does not depend on BN
+  while (BN > 32 && (long long)m_tiles * ((N + BN - 1) / BN) * 2 <= clusters) BN = (BN / 2 + 31) / 32 * 32;
+  const int n_tiles = (N + BN - 1) / BN;
+  const long long tiles = (long long)m_tiles * n_tiles;
   if (tiles < clusters) clusters = (int)tiles;
   if (clusters < 1) clusters = 1;
   if (k_drain <= 0) k_drain = 64;    // 24 MMAs per TMEM chain: truncation bias <= ~7e-7 of the chunk's magnitude
@@ -378,8 +450,10 @@ static int launch_pair(const float* A_hi, const float* A_lo, const float* Wt_hi,
     // no D is stored: the output maps are placeholders over the partial-sum buffer
     ok = make_tmap_out(&tout, epi.part, M, 4, 4) && make_tmap_out(&tout_lo, epi.part, M, 4, 4);
   } else if (epi.mode == EPI_RELAX) {
-    ok = make_tmap_out(&tout, D, M, N, ldd) && make_tmap_out(&tout_lo, D_lo, M, N, ldd);
+    epi.out_hi = D; epi.out_lo = D_lo; epi.ldd = ldd;       // written with plain coalesced stores, no output maps
+    ok = make_tmap_out(&tout, epi.part, M, 4, 4) && make_tmap_out(&tout_lo, epi.part, M, 4, 4);
   } else {
+    epi.out_hi = D; epi.ldd = ldd;                          // first panel: plain coalesced stores; later panels: TMA reduce-add
     ok = make_tmap_out(&tout, D, M, N, ldd) && make_tmap_out(&tout_lo, D, M, N, ldd);
   }
   if (!ok) { if (err) *err = "cuTensorMapEncodeTiled failed"; return -1; }

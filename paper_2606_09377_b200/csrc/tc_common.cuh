@@ -167,6 +167,11 @@ __device__ __forceinline__ void cluster_sync_all() {
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
   asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" :: "r"(cluster_addr) : "memory");
 }
+// same without a fence: ordering of the TMEM reads that precede it comes from tcgen05.wait::ld +
+// tcgen05.fence::before_thread_sync (a release at cluster scope would drain every outstanding global store first)
+__device__ __forceinline__ void mbar_arrive_cluster_relaxed(uint32_t cluster_addr) {
+  asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" :: "r"(cluster_addr) : "memory");
+}
 // TMA tile load issued by either CTA of a pair; the transaction bytes are counted on the mbarrier `bar_cluster`
 // (a shared::cluster address: the LEADER CTA's full barrier), the data lands in this CTA's shared memory.
 __device__ __forceinline__ void tma_load_2d_pair(uint32_t dst, const CUtensorMap* map, int x, int y, uint32_t bar_cluster) {
