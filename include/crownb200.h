@@ -93,7 +93,8 @@ typedef struct {
                                last contraction of a pass has a single K panel, concretise in its epilogue) */
   int32_t disable_graph;    /* 0 (default): crown_run captures its launch sequence once per (B, S, pointer set) into
                                a CUDA graph and replays it (the sequence depends on shapes only); 1: plain launches */
-  int32_t reserved0;        /* must be 0 */
+  int32_t disable_conv_tc;  /* 0 (default): 3x3 stride-1 BoundConv backward steps on 16/32-wide maps with <= 32 channels run as a
+                               per-tap implicit GEMM on the tensor cores (3xTF32); 1: CUDA-core kernel everywhere */
 } crown_opts;
 
 typedef struct crown_ctx crown_ctx;   /* opaque; owned by the library; freed by crown_destroy */

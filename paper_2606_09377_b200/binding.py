@@ -35,7 +35,7 @@ class CrownOpts(C.Structure):
     _fields_ = [("mem_cap_bytes", C.c_uint64), ("stream_weights", C.c_int32), ("mma_scheme", C.c_int32),
                 ("slope_rule", C.c_int32), ("k_drain", C.c_int32), ("stream_min_elems", C.c_uint64),
                 ("stream_stage_bytes", C.c_uint64), ("disable_epi_fusion", C.c_int32),
-                ("disable_conc_fusion", C.c_int32), ("disable_graph", C.c_int32), ("reserved0", C.c_int32)]
+                ("disable_conc_fusion", C.c_int32), ("disable_graph", C.c_int32), ("disable_conv_tc", C.c_int32)]
 
 
 class CrownError(RuntimeError):
@@ -99,7 +99,7 @@ class CrownContext:
     def __init__(self, net, B_max: int, S_max: int, device: str = "cuda:0", mem_cap_bytes: int = 0,
                  mma_scheme: int = 0, slope_rule: int = 0, k_drain: int = 0, stream_weights: int = 0,
                  stream_min_elems: int = 0, stream_stage_bytes: int = 0, disable_epi_fusion: int = 0,
-                 disable_conc_fusion: int = 0, disable_graph: int = 0):
+                 disable_conc_fusion: int = 0, disable_graph: int = 0, disable_conv_tc: int = 0):
         if not torch.cuda.is_available():
             raise CrownError("no CUDA device: the crownb200 hot path has no CPU fallback")
         self.lib = load_library()
@@ -142,7 +142,7 @@ class CrownContext:
                     cn.W_dev = Wd.data_ptr()
         self._nodes = arr
         self.opts = CrownOpts(mem_cap_bytes, stream_weights, mma_scheme, slope_rule, k_drain, stream_min_elems,
-                              stream_stage_bytes, disable_epi_fusion, disable_conc_fusion, disable_graph, 0)
+                              stream_stage_bytes, disable_epi_fusion, disable_conc_fusion, disable_graph, disable_conv_tc)
         need = C.c_size_t(0)
         self._check(self.lib.crown_workspace_bytes(arr, self.n_nodes, *self.in_chw, self.B_max, self.S_max,
                                                    C.byref(self.opts), C.byref(need)), None)

@@ -281,7 +281,7 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
         { Scope sc(ctx, CROWN_K_CONV, 4.0 * 2 * B * R * ((double)ni.size + in_size),
                    2.0 * 2 * B * R * (double)ni.size * nd.c_in * nd.kh * nd.kw);
           launch_conv_transpose(cur.v, nd.W_dev, nullptr, D, B, R, nd.c_in, nd.h_in, nd.w_in, nd.c_out, nd.kh, nd.kw,
-                                nd.stride, nd.pad, ni.h, ni.w, s); }
+                                nd.stride, nd.pad, ni.h, ni.w, s, ctx->opts.mma_scheme == 0 && !ctx->opts.disable_conv_tc, ctx->num_sms); }
         out.v = canon_view(D, B, R, in_size);
         release(ctx, cur);
         rc = contribute(ps, nd.in0, out);

@@ -357,9 +357,11 @@ int conv_init_device() {
 
 void launch_conv_transpose(const AView& A, const float* W, const float* addend, float* out, int B, int R,
                            int c_in, int h, int w, int c_out, int kh, int kw, int stride, int pad, int ho,
-                           int wo, cudaStream_t s) {
+                           int wo, cudaStream_t s, int allow_tc, int num_sms) {
   long long rows = 2LL * B * R;
   if (rows <= 0) return;
+  if (allow_tc && conv_tc_supported(c_in, h, w, c_out, kh, kw, stride, pad, ho, wo) &&
+      launch_conv_transpose_tc(A, W, addend, out, B, R, c_in, h, w, c_out, num_sms, s) == 0) return;
   if ((A.sB % 1 == 0) && rows < (1LL << 31)) {
     bool done = false;
     if (kh == 3 && kw == 3 && stride == 1) done = launch_conv_bwd_ct<3, 3, 1>(A, W, addend, out, B, R, c_in, h, w, c_out, pad, ho, wo, s);

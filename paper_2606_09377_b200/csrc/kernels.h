@@ -115,9 +115,14 @@ int launch_gemm_tc(const float* A_hi, const float* A_lo, const float* Wt_hi, con
 void launch_ibp_conv(const float* W, const float* bias, const float* l_in, const float* u_in,
                      int relu_in, float* l_out, float* u_out, int B, int c_in, int h, int w,
                      int c_out, int kh, int kw, int stride, int pad, int ho, int wo, cudaStream_t s);
+// allow_tc: 3x3 / stride 1 / pad 1 layers on 16- or 32-wide maps with <= 32 channels run as a per-tap implicit GEMM on
+// tcgen05 (conv_tc.cu, 3xTF32); everything else on the CUDA-core kernels of conv.cu.
 void launch_conv_transpose(const AView& A, const float* W, const float* addend, float* out,
                            int B, int R, int c_in, int h, int w, int c_out, int kh, int kw,
-                           int stride, int pad, int ho, int wo, cudaStream_t s);
+                           int stride, int pad, int ho, int wo, cudaStream_t s, int allow_tc = 0, int num_sms = 148);
+int conv_tc_supported(int c_in, int h, int w, int c_out, int kh, int kw, int stride, int pad, int ho, int wo);
+int launch_conv_transpose_tc(const AView& A, const float* W, const float* addend, float* out, int B, int R,
+                             int c_in, int h, int w, int c_out, int num_sms, cudaStream_t s);
 
 // Per-device kernel attributes (opt-in dynamic shared memory sizes).  cudaFuncSetAttribute applies to the CURRENT
 // device only, so crown_init calls this for the device of every new context (a process-wide "done" flag would
@@ -125,6 +130,7 @@ void launch_conv_transpose(const AView& A, const float* W, const float* addend, 
 int gemm_tc_init_device();
 int ibp_init_device();
 int conv_init_device();
-inline int kernels_init_device() { return gemm_tc_init_device() | ibp_init_device() | conv_init_device(); }
+int conv_tc_init_device();
+inline int kernels_init_device() { return gemm_tc_init_device() | ibp_init_device() | conv_init_device() | conv_tc_init_device(); }
 
 }  // namespace crownb200

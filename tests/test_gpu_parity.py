@@ -223,3 +223,14 @@ def test_boundary_calls_one_by_one():
             _close(g, olb, "lb")
         for g in (_np(out["ub"])[p], _np(ub2)[p], _np(res["ub"])[p]):
             _close(g, oub, "ub")
+
+
+def test_cfg5_half_scale_tensor_core_conv():
+    """cfg5 / 2 (16 x 16 maps, 8..32 channels): the stem and block-1 BoundConv backward steps run as the per-tap
+    implicit GEMM on tcgen05 (conv_tc.cu); same parity bar, and the CUDA-core path agrees within the tolerance."""
+    wl = W.make(5, scale=2, B=2)
+    ctx, res = _check_workload(wl)
+    lo, hi = wl.box()
+    res2 = _ctx(wl.net, wl.B, wl.S, disable_conv_tc=1).run(lo, hi, wl.C, wl.alpha, wl.intermediate)
+    _close(_np(res["lb"]), _np(res2["lb"]), "tensor-core vs CUDA-core conv lb")
+    _close(_np(res["ub"]), _np(res2["ub"]), "tensor-core vs CUDA-core conv ub")
