@@ -228,7 +228,7 @@ def backward(net, start: int, C0: np.ndarray,
              pre: Dict[int, Tuple[np.ndarray, np.ndarray]],
              alpha_lo: Optional[Dict[int, np.ndarray]] = None,
              alpha_up: Optional[Dict[int, np.ndarray]] = None,
-             rule: str = "adaptive"):
+             rule: str = "adaptive", trace: Optional[Dict[int, Tuple[np.ndarray, np.ndarray]]] = None):
     """Linear bounds  A_lo x + d_lo <= C0 . v_start(x) <= A_up x + d_up  for ONE property.
 
     start : node whose OUTPUT the start matrix C0 [R, n_start] multiplies.
@@ -245,6 +245,8 @@ def backward(net, start: int, C0: np.ndarray,
       Flatten            : A_x += A (row-major reshape)
       ReLU y = ReLU(x)   : lower: A_x = A+ * dL + A- * dU ; d += A- . bU
                            upper: A_x = A+ * dU + A- * dL ; d += A+ . bU   (PAPER.md:64)
+    trace : if a dict is given, it receives {relu node id: (A_lo, A_up)}: the coefficients w.r.t. each
+            ReLU's OUTPUT as they arrive at that ReLU (what oracle/alpha_oracle.py differentiates through).
     Returns (A_lo [R,n0], A_up [R,n0], d_lo [R], d_up [R]).
     """
     C0 = np.asarray(C0, F64)
@@ -289,6 +291,8 @@ def backward(net, start: int, C0: np.ndarray,
             contribute(n.in0, A)
         elif n.op == RELU:
             l, u = pre[i]
+            if trace is not None:
+                trace[i] = (A[0].copy(), A[1].copy())
             a_lo = None if alpha_lo is None or alpha_lo.get(i) is None else alpha_lo[i]
             a_up = None if alpha_up is None or alpha_up.get(i) is None else alpha_up[i]
             dU, bU, dL_lo = relax_coeffs(l, u, a_lo, rule)
