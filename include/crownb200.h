@@ -173,6 +173,43 @@ int crown_run_host(crown_ctx* ctx, int B, const float* x_lo_host, const float* x
                    const float* C_host, int S, const float* const* alpha_host, int intermediate,
                    float* lb_host, float* ub_host, uint8_t* verified_host);
 
+/* NEXT-1 -- alpha optimisation (sec. 2.1: "alpha-CROWN promotes the fixed slopes to per-neuron optimisable
+ * parameters alpha_i in [0,1]; gradient ascent over alpha tightens the lower bound (or lowers the upper bound)"; alpha
+ * tensors are [B, S, size_i] per ReLU).  The intermediate bounds l_dev/u_dev stay fixed (reading G8);
+ * only the final pass from the last node with C_dev [B,S,n_L] is differentiated / optimised.  The gradient is the
+ * transpose of that pass: a forward sweep of the 2*B*S bound-attaining box corners through the
+ * network with every ReLU replaced by the line the sign of the saved A selects; at A = 0 the one-sided derivative 0 is
+ * taken (reading G23).  Every ReLU needs an alpha_lo and an alpha_up entry.  scratch_dev: caller-owned device memory of
+ * at least crown_alpha_scratch_bytes(B, S) bytes, 256-byte aligned (saved A per ReLU, the sweep's vectors).
+ * Streamed layers are CROWN_EUNSUPPORTED here. */
+int crown_alpha_scratch_bytes(crown_ctx* ctx, int B, int S, size_t* out);
+
+/* Bounds of the final pass at the given alpha (lb_dev / ub_dev [B,S], may be NULL) and their derivatives
+ * g_lo_dev[i] = d lb[b,s] / d alpha_lo[i][b,s,:], g_up_dev[i] = d ub[b,s] / d alpha_up[i][b,s,:]  (arrays of n_nodes
+ * pointers, [B,S,size_i] for ReLU i; NULL array or entry = not wanted).  Zero on stable neurons.  alpha may alias. */
+int crown_alpha_grad(crown_ctx* ctx, int B, const float* C_dev, int S,
+                     const float* const* l_dev, const float* const* u_dev,
+                     const float* const* alpha_lo_dev, const float* const* alpha_up_dev,
+                     const float* x_lo_dev, const float* x_hi_dev,
+                     float* const* g_lo_dev, float* const* g_up_dev, float* lb_dev, float* ub_dev,
+                     void* scratch_dev, size_t scratch_bytes);
+
+/* `iters` projected gradient steps, in place: with a = clip(alpha, 0, 1),
+ *   alpha_lo <- clip(a + step * dir(g_lo), 0, 1)   (ascent on lb),   alpha_up <- clip(a - step * dir(g_up), 0, 1),
+ * dir = g (mode 0, plain) or sign(g) (mode 1) -- the step rule is reading G24; step = eta * decay^t at iteration t.
+ * The bounds are evaluated at iters + 1 points (the start and after every step); every iterate is a valid alpha, so every
+ * iterate is sound and the best per spec row is returned (reading G25):
+ *   lb_best_dev = max_t lb_t, ub_best_dev = min_t ub_t  [B,S];  lb_last_dev / ub_last_dev [B,S] (may be NULL) = bounds
+ *   at the final alpha;  verified_dev [B] (may be NULL) = verdict on lb_best.
+ * alpha_lo_dev[i] and alpha_up_dev[i] must be DISTINCT tensors for every ReLU (CROWN_EINVAL otherwise). */
+int crown_alpha_ascent(crown_ctx* ctx, int B, const float* C_dev, int S,
+                       const float* const* l_dev, const float* const* u_dev,
+                       float* const* alpha_lo_dev, float* const* alpha_up_dev,
+                       const float* x_lo_dev, const float* x_hi_dev,
+                       float eta, float decay, int iters, int mode,
+                       float* lb_best_dev, float* ub_best_dev, float* lb_last_dev, float* ub_last_dev,
+                       uint8_t* verified_dev, void* scratch_dev, size_t scratch_bytes);
+
 /* D[M,N] = A[M,K] . W[K,N] (row-major fp32) through the same contraction kernel the backward
  * pass uses (scheme: 0 = 3xTF32 tcgen05 on prepared limbs, 2 = FFMA; 1 -- reserved in SURVEY.md for a split-bf16
  * scheme -- is intentionally absent); exposed for parity tests and roofline

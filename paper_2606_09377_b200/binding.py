@@ -19,7 +19,7 @@ OP_CODES = {"linear": 1, "conv": 2, "relu": 3, "add": 4, "flatten": 5}
 K_CLASSES = ["ibp", "coeff", "relax", "gemm_tc", "gemm_ffma", "concretize", "conv", "misc"]
 
 EXPORTS = ["crown_h2d_bytes", "crown_workspace_bytes", "crown_init", "ibp_forward", "crown_backward", "concretize", "crown_run",
-           "crown_run_host", "crown_gemm", "crown_split_tf32", "crown_peak_bytes", "crown_row_chunk", "crown_launch_count", "crown_graph_replays",
+           "crown_run_host", "crown_alpha_scratch_bytes", "crown_alpha_grad", "crown_alpha_ascent", "crown_gemm", "crown_split_tf32", "crown_peak_bytes", "crown_row_chunk", "crown_launch_count", "crown_graph_replays",
            "crown_gemm_flops", "crown_timing", "crown_timing_read", "crown_last_error", "crown_destroy",
            "crown_version"]
 
@@ -70,6 +70,11 @@ def load_library() -> C.CDLL:
     lib.concretize.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp, vp, i32]
     lib.crown_run.argtypes = [vp, i32, vp, vp, vp, i32, C.POINTER(vp), i32, C.POINTER(vp), C.POINTER(vp), vp, vp, vp]
     lib.crown_run_host.argtypes = [vp, i32, vp, vp, vp, i32, C.POINTER(vp), i32, vp, vp, vp]
+    lib.crown_alpha_scratch_bytes.argtypes = [vp, i32, i32, C.POINTER(C.c_size_t)]
+    lib.crown_alpha_grad.argtypes = [vp, i32, vp, i32, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), vp, vp,
+                                     C.POINTER(vp), C.POINTER(vp), vp, vp, vp, C.c_size_t]
+    lib.crown_alpha_ascent.argtypes = [vp, i32, vp, i32, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), vp, vp,
+                                       C.c_float, C.c_float, i32, i32, vp, vp, vp, vp, vp, vp, C.c_size_t]
     lib.crown_gemm.argtypes = [vp, i32, i32, i32, i32, vp, vp, vp, vp, vp]
     lib.crown_split_tf32.argtypes = [vp, vp, i32, i32, i32, vp, vp]
     lib.crown_peak_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
@@ -284,6 +289,66 @@ class CrownContext:
         self._check(self.lib.crown_run_host(self.h, B, x_lo.ctypes.data, x_hi.ctypes.data, Cmat.ctypes.data, S, arr,
                                             1 if intermediate == "ibp" else 0, lb.ctypes.data, ub.ctypes.data,
                                             verified.ctypes.data), self.h)
+
+    # ---- NEXT-1: alpha optimisation ---------------------------------------------------
+    def _alpha_scratch(self, B: int, S: int) -> torch.Tensor:
+        need = C.c_size_t(0)
+        self._check(self.lib.crown_alpha_scratch_bytes(self.h, B, S, C.byref(need)), self.h)
+        cur = getattr(self, "_alpha_scr", None)
+        if cur is None or cur.numel() < need.value:
+            self._alpha_scr = torch.empty(need.value, dtype=torch.uint8, device=self.device)
+        return self._alpha_scr
+
+    def alpha_grad(self, pre: Dict[int, tuple], Cmat, alpha_lo: Dict[int, torch.Tensor], alpha_up: Dict[int, torch.Tensor], box):
+        """Bounds of the final pass at (alpha_lo, alpha_up) and their derivatives w.r.t. the slopes.
+        Returns dict lb, ub [B,S], g_lo, g_up {relu id: [B,S,n]}."""
+        Cmat = self._dev(Cmat)
+        B, S = Cmat.shape[0], Cmat.shape[1]
+        l = {i: self._dev(v[0]) for i, v in pre.items()}
+        u = {i: self._dev(v[1]) for i, v in pre.items()}
+        al = {i: self._dev(v) for i, v in alpha_lo.items()}
+        au = al if alpha_up is alpha_lo else {i: self._dev(v) for i, v in alpha_up.items()}
+        x_lo, x_hi = self._dev(box[0]), self._dev(box[1])
+        g_lo = {i: torch.empty(B, S, self.sizes[i], device=self.device) for i in self.relu_ids}
+        g_up = {i: torch.empty(B, S, self.sizes[i], device=self.device) for i in self.relu_ids}
+        lb = torch.empty(B, S, device=self.device)
+        ub = torch.empty(B, S, device=self.device)
+        scr = self._alpha_scratch(B, S)
+        self._check(self.lib.crown_alpha_grad(self.h, B, Cmat.data_ptr(), S, self._ptr_array(l), self._ptr_array(u),
+                                              self._ptr_array(al), self._ptr_array(au), x_lo.data_ptr(), x_hi.data_ptr(),
+                                              self._ptr_array(g_lo), self._ptr_array(g_up), lb.data_ptr(), ub.data_ptr(),
+                                              scr.data_ptr(), scr.numel()), self.h)
+        self.stream.synchronize()
+        return {"lb": lb, "ub": ub, "g_lo": g_lo, "g_up": g_up}
+
+    def alpha_ascent_device(self, l, u, Cmat, alpha_lo, alpha_up, x_lo, x_hi, eta, decay, iters, mode, out) -> None:
+        """crown_alpha_ascent on device tensors (asynchronous); alpha_lo / alpha_up are updated in place."""
+        B, S = Cmat.shape[0], Cmat.shape[1]
+        scr = self._alpha_scratch(B, S)
+        self._check(self.lib.crown_alpha_ascent(self.h, B, Cmat.data_ptr(), S, self._ptr_array(l), self._ptr_array(u),
+                                                self._ptr_array(alpha_lo), self._ptr_array(alpha_up), x_lo.data_ptr(),
+                                                x_hi.data_ptr(), float(eta), float(decay), int(iters), int(mode),
+                                                out["lb_best"].data_ptr(), out["ub_best"].data_ptr(),
+                                                out["lb_last"].data_ptr(), out["ub_last"].data_ptr(),
+                                                out["verified"].data_ptr(), scr.data_ptr(), scr.numel()), self.h)
+
+    def alpha_ascent(self, pre: Dict[int, tuple], Cmat, alpha_lo: Dict[int, torch.Tensor], alpha_up: Dict[int, torch.Tensor],
+                     box, eta: float, iters: int, mode: str = "sign", decay: float = 1.0):
+        """Projected gradient ascent on alpha_lo (lb) / descent on alpha_up (ub) with fixed intermediate bounds.
+        Returns dict alpha_lo, alpha_up (optimised copies), lb_best, ub_best, lb_last, ub_last [B,S], verified [B]."""
+        Cmat = self._dev(Cmat)
+        B, S = Cmat.shape[0], Cmat.shape[1]
+        l = {i: self._dev(v[0]) for i, v in pre.items()}
+        u = {i: self._dev(v[1]) for i, v in pre.items()}
+        al = {i: self._dev(v).clone() for i, v in alpha_lo.items()}
+        au = {i: self._dev(v).clone() for i, v in alpha_up.items()}
+        x_lo, x_hi = self._dev(box[0]), self._dev(box[1])
+        out = {k: torch.empty(B, S, device=self.device) for k in ("lb_best", "ub_best", "lb_last", "ub_last")}
+        out["verified"] = torch.empty(B, dtype=torch.uint8, device=self.device)
+        self.alpha_ascent_device(l, u, Cmat, al, au, x_lo, x_hi, eta, decay, iters, {"plain": 0, "sign": 1}[mode], out)
+        self.stream.synchronize()
+        out["alpha_lo"], out["alpha_up"] = al, au
+        return out
 
     # ---- kernel 1 on its own ---------------------------------------------------------------------
     def split_tf32(self, X: torch.Tensor, transpose: bool = False):

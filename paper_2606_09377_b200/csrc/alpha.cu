@@ -1,0 +1,251 @@
+// NEXT-1 -- alpha optimisation of alpha-CROWN ("gradient ascent over alpha tightens the lower bound (or
+// lowers the upper bound)"; alpha tensors [layers x specs x batch x neurons]).
+//
+// The derivative of the final bound with respect to the slopes is the transpose of the backward pass O3 (DESIGN.md
+// sec. 11): with G_i = d bound / d A_i (one vector per (branch, property, spec row)),
+//   input   : G = x_c -/+ sign(A_0) * x_r                    (the corner of the box that attains the bound)
+//   Linear i: G_i = G_in . W_i^T + b_i      Conv i: G_i = conv(G_in, W_i) + b_i      Add: G_i = G_a + G_b
+//   ReLU   i: lower  G_i = [A_i>0] dL G_in + [A_i<0] (dU G_in + bU),   d lb / d alpha_i = A_i^+ * G_in  (unstable only)
+//             upper  G_i = [A_i>0] (dU G_in + bU) + [A_i<0] dL G_in,   d ub / d alpha_i = A_i^- * G_in
+// i.e. a forward sweep of 2*B*S "points" through the network, every ReLU replaced by the line the sign of the saved
+// A_i selects.  Kernels of that sweep; the host side is in backward.cu (crown_alpha_grad / crown_alpha_ascent).
+#include "common.cuh"
+#include "kernels.h"
+
+namespace crownb200 {
+
+// ---- corner of the box: G[br,b,s,:] = x_c - sign(A0[0,b,s,:]) x_r (br 0), x_c + sign(A0[1,b,s,:]) x_r (br 1) -------
+__global__ void __launch_bounds__(256)
+alpha_corner_kernel(const float* __restrict__ A0, const float* __restrict__ x_lo, const float* __restrict__ x_hi,
+                    float* __restrict__ G, int B, int S, int n0) {
+  const long long per_br = (long long)B * S * n0;
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= 2 * per_br) return;
+  const int br = (int)(i / per_br);
+  const long long r = i % per_br;
+  const int b = (int)(r / ((long long)S * n0)), j = (int)(r % n0);
+  const float lo = x_lo[(long long)b * n0 + j], hi = x_hi[(long long)b * n0 + j];
+  const float xc = 0.5f * (lo + hi), xr = 0.5f * (hi - lo);
+  const float a = A0[i];
+  const float sg = a > 0.f ? 1.f : (a < 0.f ? -1.f : 0.f);        // one-sided derivative 0 at the kink (reading G23)
+  G[i] = br == 0 ? xc - sg * xr : xc + sg * xr;
+}
+
+void launch_alpha_corner(const float* A0, const float* x_lo, const float* x_hi, float* G, int B, int S, int n0,
+                         cudaStream_t s) {
+  const long long cnt = 2LL * B * S * n0;
+  if (cnt <= 0) return;
+  alpha_corner_kernel<<<ceil_div(cnt, 256), 256, 0, s>>>(A0, x_lo, x_hi, G, B, S, n0);
+}
+
+// ---- Linear: D[M,N] = G[M,K] . W[N,K]^T + bias[N]  (W row-major [n_out, n_in] as the network stores it) ------------
+// CUDA-core FFMA, 64x64x16 tiles, 256 threads x (4x4) outputs, both operands K-contiguous (128-bit loads when K % 4 == 0).
+constexpr int ABM = 64, ABN = 64, ABK = 16;
+
+template <bool VEC>
+__global__ void __launch_bounds__(256)
+alpha_linear_kernel(const float* __restrict__ G, const float* __restrict__ W, const float* __restrict__ bias,
+                    float* __restrict__ D, int M, int N, int K) {
+  __shared__ float sG[ABK][ABM + 4];   // [k][m]
+  __shared__ float sW[ABK][ABN + 4];   // [k][n]
+  const int tid = threadIdx.x;
+  const int tx = tid % 16, ty = tid / 16;
+  const int m0 = blockIdx.y * ABM, n0 = blockIdx.x * ABN;
+  float acc[4][4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+#pragma unroll
+    for (int j = 0; j < 4; ++j) acc[i][j] = 0.f;
+  const int lr = tid / 4, lk = (tid % 4) * 4;    // this thread's row of the tile and first k of its 4
+  for (int k0 = 0; k0 < K; k0 += ABK) {
+    const int gk = k0 + lk;
+    float4 g = make_float4(0.f, 0.f, 0.f, 0.f), w = g;
+    const int gm = m0 + lr, gn = n0 + lr;
+    if (VEC) {
+      if (gm < M && gk < K) g = *reinterpret_cast<const float4*>(G + (long long)gm * K + gk);
+      if (gn < N && gk < K) w = __ldg(reinterpret_cast<const float4*>(W + (long long)gn * K + gk));
+    } else {
+      if (gm < M) {
+        const float* q = G + (long long)gm * K;
+        g.x = gk < K ? q[gk] : 0.f; g.y = gk + 1 < K ? q[gk + 1] : 0.f; g.z = gk + 2 < K ? q[gk + 2] : 0.f; g.w = gk + 3 < K ? q[gk + 3] : 0.f;
+      }
+      if (gn < N) {
+        const float* q = W + (long long)gn * K;
+        w.x = gk < K ? q[gk] : 0.f; w.y = gk + 1 < K ? q[gk + 1] : 0.f; w.z = gk + 2 < K ? q[gk + 2] : 0.f; w.w = gk + 3 < K ? q[gk + 3] : 0.f;
+      }
+    }
+    sG[lk][lr] = g.x; sG[lk + 1][lr] = g.y; sG[lk + 2][lr] = g.z; sG[lk + 3][lr] = g.w;
+    sW[lk][lr] = w.x; sW[lk + 1][lr] = w.y; sW[lk + 2][lr] = w.z; sW[lk + 3][lr] = w.w;
+    __syncthreads();
+#pragma unroll
+    for (int kk = 0; kk < ABK; ++kk) {
+      const float4 a = *reinterpret_cast<const float4*>(&sG[kk][ty * 4]);
+      const float4 b = *reinterpret_cast<const float4*>(&sW[kk][tx * 4]);
+      const float av[4] = {a.x, a.y, a.z, a.w}, bv[4] = {b.x, b.y, b.z, b.w};
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j] = fmaf(av[i], bv[j], acc[i][j]);
+    }
+    __syncthreads();
+  }
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int gm = m0 + ty * 4 + i;
+    if (gm >= M) continue;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const int gn = n0 + tx * 4 + j;
+      if (gn < N) D[(long long)gm * N + gn] = acc[i][j] + (bias ? __ldg(bias + gn) : 0.f);
+    }
+  }
+}
+
+void launch_alpha_linear(const float* G, const float* W, const float* bias, float* D, int M, int N, int K,
+                         cudaStream_t s) {
+  if (M <= 0 || N <= 0) return;
+  dim3 grid(ceil_div(N, ABN), ceil_div(M, ABM));
+  const bool vec = (K % 4 == 0) && ((reinterpret_cast<uintptr_t>(G) | reinterpret_cast<uintptr_t>(W)) & 15) == 0;
+  if (vec) alpha_linear_kernel<true><<<grid, 256, 0, s>>>(G, W, bias, D, M, N, K);
+  else alpha_linear_kernel<false><<<grid, 256, 0, s>>>(G, W, bias, D, M, N, K);
+}
+
+// ---- Conv2d forward of points: out[m, co, p, q] = bias[co] + sum W[co,ci,i,j] * in[m, ci, p*s+i-pad, q*s+j-pad] -----
+// one thread per output pixel of four output channels (the gather of ibp_conv_kernel without the radius half)
+constexpr int kPtConvCO = 4;
+__global__ void __launch_bounds__(256)
+alpha_conv_kernel(const float* __restrict__ W, const float* __restrict__ bias, const float* __restrict__ in,
+                  float* __restrict__ out, int c_in, int h, int w, int c_out, int kh, int kw, int stride, int pad,
+                  int ho, int wo) {
+  extern __shared__ float sw[];   // [kPtConvCO][c_in*kh*kw]
+  const int co0 = blockIdx.y * kPtConvCO;
+  const long long m = blockIdx.z;
+  const int fsz = c_in * kh * kw;
+  for (int i = threadIdx.x; i < kPtConvCO * fsz; i += blockDim.x) {
+    const int o = i / fsz, k = i % fsz;
+    sw[i] = (co0 + o < c_out) ? W[(long long)(co0 + o) * fsz + k] : 0.f;
+  }
+  __syncthreads();
+  const int pix = blockIdx.x * blockDim.x + threadIdx.x;
+  if (pix >= ho * wo) return;
+  const int p = pix / wo, q = pix % wo;
+  const float* src = in + m * c_in * h * w;
+  float c[kPtConvCO];
+#pragma unroll
+  for (int o = 0; o < kPtConvCO; ++o) c[o] = 0.f;
+  for (int ci = 0; ci < c_in; ++ci)
+    for (int i = 0; i < kh; ++i) {
+      const int y = p * stride + i - pad;
+      if (y < 0 || y >= h) continue;
+      for (int j = 0; j < kw; ++j) {
+        const int x = q * stride + j - pad;
+        if (x < 0 || x >= w) continue;
+        const float v = src[(ci * h + y) * w + x];
+        const int k = (ci * kh + i) * kw + j;
+#pragma unroll
+        for (int o = 0; o < kPtConvCO; ++o) c[o] = fmaf(sw[o * fsz + k], v, c[o]);
+      }
+    }
+#pragma unroll
+  for (int o = 0; o < kPtConvCO; ++o) {
+    const int co = co0 + o;
+    if (co >= c_out) break;
+    out[(m * c_out + co) * ho * wo + pix] = c[o] + (bias ? bias[co] : 0.f);
+  }
+}
+
+void launch_alpha_conv(const float* W, const float* bias, const float* in, float* out, long long M, int c_in, int h,
+                       int w, int c_out, int kh, int kw, int stride, int pad, int ho, int wo, cudaStream_t s) {
+  if (M <= 0) return;
+  int threads = 256;
+  while (threads > 32 && threads / 2 >= ho * wo) threads /= 2;
+  const size_t smem = (size_t)kPtConvCO * c_in * kh * kw * sizeof(float);
+  for (long long m0 = 0; m0 < M; m0 += 65535) {       // gridDim.z limit
+    const long long mz = M - m0 < 65535 ? M - m0 : 65535;
+    dim3 grid(ceil_div(ho * wo, threads), ceil_div(c_out, kPtConvCO), (unsigned)mz);
+    alpha_conv_kernel<<<grid, threads, smem, s>>>(W, bias, in + m0 * c_in * h * w, out + m0 * c_out * ho * wo, c_in, h,
+                                                  w, c_out, kh, kw, stride, pad, ho, wo);
+  }
+}
+
+// ---- Add: G = Ga + Gb ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+alpha_add_kernel(const float* __restrict__ a, const float* __restrict__ b, float* __restrict__ o, long long cnt) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < cnt) o[i] = a[i] + b[i];
+}
+void launch_alpha_add(const float* a, const float* b, float* o, long long cnt, cudaStream_t s) {
+  if (cnt <= 0) return;
+  alpha_add_kernel<<<ceil_div(cnt, 256), 256, 0, s>>>(a, b, o, cnt);
+}
+
+// ---- ReLU: forward value through the selected line, gradient w.r.t. alpha, optional in-place projected step ---------
+// element (b, s, j) for both branches.  A, Gin, Gout: [2, B, S, n]; coef [B, n] {dU, bU, dL_fixed, unstable};
+// alpha_lo / alpha_up [B, S, n].  step != nullptr: alpha <- clip(clip(alpha) +/- step[0] * dir(g), 0, 1) with
+// dir = g (mode 0, "plain") or sign(g) (mode 1, "sign"); else g_lo / g_up receive the gradients (may be nullptr).
+__device__ __forceinline__ float clip01f(float a) { return fminf(fmaxf(a, 0.f), 1.f); }
+__device__ __forceinline__ float sgnf(float a) { return a > 0.f ? 1.f : (a < 0.f ? -1.f : 0.f); }
+
+__global__ void __launch_bounds__(256)
+alpha_relu_kernel(const float* __restrict__ A, const float* __restrict__ Gin, const float4* __restrict__ coef,
+                  float* alpha_lo, float* alpha_up, float* __restrict__ Gout, float* __restrict__ g_lo,
+                  float* __restrict__ g_up, const float* __restrict__ step, int mode, int B, int S, int n) {
+  const long long per_br = (long long)B * S * n;
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= per_br) return;
+  const int b = (int)(i / ((long long)S * n)), j = (int)(i % n);
+  const float4 c = __ldg(coef + (long long)b * n + j);
+  const bool unstable = c.w != 0.f;
+  const float aL = A[i], aU = A[per_br + i];
+  const float gL = Gin[i], gU = Gin[per_br + i];
+  const float alL = alpha_lo[i], alU = alpha_up[i];
+  const float sL = unstable ? clip01f(alL) : c.z, sU = unstable ? clip01f(alU) : c.z;
+  const float dU = c.x, bU = c.y;
+  Gout[i] = aL > 0.f ? sL * gL : (aL < 0.f ? fmaf(dU, gL, bU) : 0.f);
+  Gout[per_br + i] = aU > 0.f ? fmaf(dU, gU, bU) : (aU < 0.f ? sU * gU : 0.f);
+  const float dl = unstable ? fmaxf(aL, 0.f) * gL : 0.f;
+  const float du = unstable ? fminf(aU, 0.f) * gU : 0.f;
+  if (step) {
+    const float eta = step[0];
+    alpha_lo[i] = clip01f(clip01f(alL) + eta * (mode ? sgnf(dl) : dl));      // ascent on lb
+    alpha_up[i] = clip01f(clip01f(alU) - eta * (mode ? sgnf(du) : du));      // descent on ub
+  } else {
+    if (g_lo) g_lo[i] = dl;
+    if (g_up) g_up[i] = du;
+  }
+}
+
+void launch_alpha_relu(const float* A, const float* Gin, const float4* coef, float* alpha_lo, float* alpha_up,
+                       float* Gout, float* g_lo, float* g_up, const float* step, int mode, int B, int S, int n,
+                       cudaStream_t s) {
+  const long long cnt = (long long)B * S * n;
+  if (cnt <= 0) return;
+  alpha_relu_kernel<<<ceil_div(cnt, 256), 256, 0, s>>>(A, Gin, coef, alpha_lo, alpha_up, Gout, g_lo, g_up, step, mode,
+                                                      B, S, n);
+}
+
+// ---- best-so-far bounds over the iterates (every iterate is sound): lb_best = max, ub_best = min; the step size
+// decays for the next iteration.  first != 0: initialise instead of combine.
+__global__ void __launch_bounds__(256)
+alpha_best_kernel(const float* __restrict__ lb, const float* __restrict__ ub, float* __restrict__ lb_best,
+                  float* __restrict__ ub_best, float* step, float decay, int first, int count) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < count) {
+    // NaN-propagating on purpose: fmaxf / fminf would drop a NaN iterate and keep the (finite) best
+    const float l = lb[i], u = ub[i];
+    lb_best[i] = first ? l : ((l > lb_best[i] || l != l) ? l : lb_best[i]);
+    ub_best[i] = first ? u : ((u < ub_best[i] || u != u) ? u : ub_best[i]);
+  }
+  if (i == 0 && step && !first) step[0] *= decay;
+}
+
+void launch_alpha_best(const float* lb, const float* ub, float* lb_best, float* ub_best, float* step, float decay,
+                       int first, int count, cudaStream_t s) {
+  if (count <= 0) return;
+  alpha_best_kernel<<<ceil_div(count, 256), 256, 0, s>>>(lb, ub, lb_best, ub_best, step, decay, first, count);
+}
+
+__global__ void alpha_set_step_kernel(float* step, float v) { step[0] = v; }
+void launch_alpha_set_step(float* step, float v, cudaStream_t s) { alpha_set_step_kernel<<<1, 1, 0, s>>>(step, v); }
+
+}  // namespace crownb200

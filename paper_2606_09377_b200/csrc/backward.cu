@@ -103,7 +103,7 @@ int tc_contract(crown_ctx* ctx, const NodeInfo& ni, const float* hi, const float
 int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_dev,
              const float* const* l_dev, const float* const* u_dev, const float* const* alpha_lo,
              const float* const* alpha_up, float* A_dev, float* d_dev, const float* x_lo, const float* x_hi,
-             float* lb, float* ub, int out_stride, std::vector<char>* coef_ready) {
+             float* lb, float* ub, int out_stride, std::vector<char>* coef_ready, float* const* A_save = nullptr) {
   const int n = (int)ctx->nodes.size();
   cudaStream_t s = ctx->stream;
   if (B <= 0 || B > ctx->B_max || R <= 0 || R > ctx->plan.rows_cap || start < 0 || start >= n)
@@ -159,6 +159,10 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
       case CROWN_RELU: {
         if ((rc = ensure_coef(i))) return rc;
         const int j = nd.in0;
+        if (A_save && A_save[i]) {   // alpha optimisation: keep A as it arrives at this ReLU, contiguous [2,B,R,n]
+          Scope sc(ctx, CROWN_K_MISC, 8.0 * 2 * B * R * ni.size);
+          launch_view_add(cur.v, nullptr, A_save[i], B, R, s);
+        }
         const bool lin_below = j >= 0 && (ctx->nodes[j].n.op == CROWN_LINEAR || ctx->nodes[j].n.op == CROWN_CONV2D);
         // the product that follows runs on the tensor cores when the producer is a prepacked Linear
         const bool tc = lin_below && ctx->nodes[j].tc_ok && (ctx->nodes[j].streamed || gemm_tc_supported(2 * B * R, ctx->nodes[j].n.n_in, ctx->nodes[j].n.n_out));
@@ -272,17 +276,42 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
         rc = contribute(ps, nd.in0, out);
         break; }
       case CROWN_CONV2D: {
+        if (cur.v.lo) {   // the conv kernels take plain fp32: fold a TF32-split view back (hi + lo is exact)
+          float* F = nullptr;
+          Pending f; f.buf = new_buf(ps, F);
+          if (f.buf < 0) return fail(ctx, CROWN_ENOMEM, "backward: A-buffer pool exhausted");
+          { Scope sc(ctx, CROWN_K_MISC, 12.0 * 2 * B * R * cur.v.n); launch_view_add(cur.v, nullptr, F, B, R, s); }
+          f.v = canon_view(F, B, R, cur.v.n); f.bias_done_for = cur.bias_done_for;
+          release(ctx, cur); cur = f;
+        }
         add_bias(ps, cur, i);
         Pending out;
         float* D = nullptr;
         out.buf = new_buf(ps, D);
         if (out.buf < 0) return fail(ctx, CROWN_ENOMEM, "backward: A-buffer pool exhausted");
         const int in_size = nd.c_in * nd.h_in * nd.w_in;
-        { Scope sc(ctx, CROWN_K_CONV, 4.0 * 2 * B * R * ((double)ni.size + in_size),
+        // residual fork: when the node this conv feeds already holds the other consumer's contribution (a plain
+        // contiguous buffer, no bias bookkeeping attached), the kernel adds it in its epilogue (no separate sum pass)
+        const float* addend = nullptr;
+        Pending other;
+        {
+          auto itp = ps.pend.find(nd.in0);
+          const bool plain_node = nd.in0 < 0 || (ctx->nodes[nd.in0].n.op != CROWN_LINEAR && ctx->nodes[nd.in0].n.op != CROWN_CONV2D);
+          // only the tensor-core kernel absorbs the addend for free (its loads hide behind the MMAs); on the CUDA-core
+          // kernel it measured the same as the separate sum pass
+          const bool tc_conv = ctx->opts.mma_scheme == 0 && !ctx->opts.disable_conv_tc && !cur.v.lo &&
+                               conv_tc_supported(nd.c_in, nd.h_in, nd.w_in, nd.c_out, nd.kh, nd.kw, nd.stride, nd.pad, ni.h, ni.w);
+          if (itp != ps.pend.end() && plain_node && tc_conv && !itp->second.v.lo && itp->second.v.n == in_size && itp->second.v.ld == in_size &&
+              itp->second.v.sB == (long long)R * in_size && itp->second.v.sBr == (long long)B * R * in_size) {
+            other = itp->second; addend = other.v.p; ps.pend.erase(itp);
+          }
+        }
+        { Scope sc(ctx, CROWN_K_CONV, 4.0 * 2 * B * R * ((double)ni.size + in_size * (addend ? 2.0 : 1.0)),
                    2.0 * 2 * B * R * (double)ni.size * nd.c_in * nd.kh * nd.kw);
-          launch_conv_transpose(cur.v, nd.W_dev, nullptr, D, B, R, nd.c_in, nd.h_in, nd.w_in, nd.c_out, nd.kh, nd.kw,
+          launch_conv_transpose(cur.v, nd.W_dev, addend, D, B, R, nd.c_in, nd.h_in, nd.w_in, nd.c_out, nd.kh, nd.kw,
                                 nd.stride, nd.pad, ni.h, ni.w, s, ctx->opts.mma_scheme == 0 && !ctx->opts.disable_conv_tc, ctx->num_sms); }
         out.v = canon_view(D, B, R, in_size);
+        if (addend) release(ctx, other);
         release(ctx, cur);
         rc = contribute(ps, nd.in0, out);
         break; }
@@ -528,6 +557,175 @@ extern "C" int crown_run_host(crown_ctx* ctx, int B, const float* x_lo_host, con
   CK(ctx, cudaMemcpyAsync(ub_host, ub, (size_t)B * S * 4, cudaMemcpyDeviceToHost, s));
   if (verified_host) CK(ctx, cudaMemcpyAsync(verified_host, ver, (size_t)B, cudaMemcpyDeviceToHost, s));
   CK(ctx, cudaStreamSynchronize(s));
+  return CROWN_OK;
+}
+
+// ================================================================================================
+// NEXT-1 -- alpha optimisation of the final bound
+// ================================================================================================
+namespace {
+
+struct AlphaScratch {
+  float* A0 = nullptr;             // [2,B,S,n0]   A w.r.t. the input, as the final pass leaves it
+  float* Gin = nullptr;            // [2,B,S,n0]   the corner of the box that attains each bound
+  std::vector<float*> Asave;       // per ReLU node [2,B,S,size]: A as it arrived at that ReLU
+  std::vector<float*> G;           // per node [2,B,S,size]: d bound / d A_i (Flatten aliases its producer)
+  float* lb = nullptr; float* ub = nullptr;   // [B,S] bounds of the current iterate
+  float* step = nullptr;           // current step size (device scalar: the iteration is data-independent on the host)
+  int last_relu = -1;
+  size_t bytes = 0;
+};
+
+void alpha_layout(crown_ctx* ctx, int B, int S, uint8_t* base, AlphaScratch& sc) {
+  const int n = (int)ctx->nodes.size();
+  size_t off = 0;
+  auto take = [&](size_t elems) { float* p = reinterpret_cast<float*>(base + off); off += align_up(elems * 4, 256); return p; };
+  const size_t rows = (size_t)2 * B * S;
+  sc.A0 = take(rows * ctx->n0);
+  sc.Gin = take(rows * ctx->n0);
+  sc.Asave.assign(n, nullptr); sc.G.assign(n, nullptr);
+  sc.last_relu = -1;
+  for (int i = 0; i < n; ++i) if (ctx->nodes[i].n.op == CROWN_RELU) sc.last_relu = i;
+  for (int i = 0; i <= sc.last_relu; ++i) {
+    const NodeInfo& ni = ctx->nodes[i];
+    if (ni.n.op == CROWN_RELU) sc.Asave[i] = take(rows * ni.size);
+    if (ni.n.op == CROWN_FLATTEN) sc.G[i] = ni.n.in0 < 0 ? sc.Gin : sc.G[ni.n.in0];
+    else sc.G[i] = take(rows * ni.size);
+  }
+  sc.lb = take((size_t)B * S); sc.ub = take((size_t)B * S);
+  sc.step = take(1);
+  sc.bytes = off;
+}
+
+int alpha_check(crown_ctx* ctx, int B, int S, const float* C_dev, const float* const* l_dev, const float* const* u_dev,
+                const float* const* alpha_lo, const float* const* alpha_up, const float* x_lo, const float* x_hi,
+                const void* scratch, size_t scratch_bytes, bool distinct, AlphaScratch& sc) {
+  if (B <= 0 || B > ctx->B_max || S <= 0 || S > ctx->S_max || !C_dev || !l_dev || !u_dev || !alpha_lo || !alpha_up ||
+      !x_lo || !x_hi || !scratch)
+    return fail(ctx, CROWN_EINVAL, "crown_alpha: bad arguments");
+  if (reinterpret_cast<uintptr_t>(scratch) & 255) return fail(ctx, CROWN_EINVAL, "crown_alpha: scratch must be 256-byte aligned");
+  for (size_t i = 0; i < ctx->nodes.size(); ++i) {
+    const NodeInfo& ni = ctx->nodes[i];
+    if (ni.n.op == CROWN_RELU && (!alpha_lo[i] || !alpha_up[i] || !l_dev[i] || !u_dev[i]))
+      return fail(ctx, CROWN_EINVAL, "crown_alpha: every ReLU needs alpha_lo, alpha_up and its pre-activation bounds");
+    if (ni.n.op == CROWN_RELU && distinct && alpha_lo[i] == alpha_up[i])
+      return fail(ctx, CROWN_EINVAL, "crown_alpha_ascent: alpha_lo and alpha_up must be distinct tensors (they are optimised separately)");
+    if (ni.n.op == CROWN_LINEAR && !ni.n.W_dev) return fail(ctx, CROWN_EUNSUPPORTED, "crown_alpha: streamed layers are not supported");
+  }
+  alpha_layout(ctx, B, S, reinterpret_cast<uint8_t*>(const_cast<void*>(scratch)), sc);
+  if (scratch_bytes < sc.bytes) return fail(ctx, CROWN_ENOMEM, "crown_alpha: scratch smaller than crown_alpha_scratch_bytes");
+  return CROWN_OK;
+}
+
+// final pass at the current alpha (keeping A at every ReLU and at the input), bounds into sc.lb / sc.ub
+int alpha_backward(crown_ctx* ctx, int B, int S, const float* C_dev, const float* const* l_dev, const float* const* u_dev,
+                   const float* const* alpha_lo, const float* const* alpha_up, const float* x_lo, const float* x_hi,
+                   const AlphaScratch& sc, std::vector<char>* coef_ready) {
+  return run_pass(ctx, B, (int)ctx->nodes.size() - 1, 0, S, C_dev, l_dev, u_dev, alpha_lo, alpha_up, sc.A0, nullptr, x_lo, x_hi,
+                  sc.lb, sc.ub, S, coef_ready, sc.Asave.data());
+}
+
+// forward sweep of G; step == nullptr: gradients into g_lo / g_up, else the projected step on alpha in place
+int alpha_forward(crown_ctx* ctx, int B, int S, const AlphaScratch& sc, const float* x_lo, const float* x_hi,
+                  float* const* alpha_lo, float* const* alpha_up, float* const* g_lo, float* const* g_up,
+                  const float* step, int mode) {
+  cudaStream_t s = ctx->stream;
+  const long long M = 2LL * B * S;
+  { Scope scp(ctx, CROWN_K_MISC, 4.0 * M * ctx->n0 * 2); launch_alpha_corner(sc.A0, x_lo, x_hi, sc.Gin, B, S, ctx->n0, s); }
+  for (int i = 0; i <= sc.last_relu; ++i) {
+    const NodeInfo& ni = ctx->nodes[i];
+    const crown_node& nd = ni.n;
+    const float* gin = nd.in0 < 0 ? sc.Gin : sc.G[nd.in0];
+    switch (nd.op) {
+      case CROWN_LINEAR: {
+        Scope scp(ctx, CROWN_K_GEMM_FFMA, 4.0 * ((double)M * nd.n_in + (double)nd.n_in * nd.n_out + (double)M * nd.n_out),
+                  2.0 * M * (double)nd.n_in * nd.n_out);
+        launch_alpha_linear(gin, nd.W_dev, nd.b_dev, sc.G[i], (int)M, nd.n_out, nd.n_in, s);
+        break; }
+      case CROWN_CONV2D: {
+        Scope scp(ctx, CROWN_K_CONV, 4.0 * M * ((double)ni.size + (double)nd.c_in * nd.h_in * nd.w_in),
+                  2.0 * M * (double)ni.size * nd.c_in * nd.kh * nd.kw);
+        launch_alpha_conv(nd.W_dev, nd.b_dev, gin, sc.G[i], M, nd.c_in, nd.h_in, nd.w_in, nd.c_out, nd.kh, nd.kw, nd.stride,
+                          nd.pad, ni.h, ni.w, s);
+        break; }
+      case CROWN_ADD: {
+        const float* gb = nd.in1 < 0 ? sc.Gin : sc.G[nd.in1];
+        Scope scp(ctx, CROWN_K_MISC, 12.0 * M * ni.size);
+        launch_alpha_add(gin, gb, sc.G[i], M * ni.size, s);
+        break; }
+      case CROWN_FLATTEN:
+        break;                                  // aliases its producer
+      case CROWN_RELU: {
+        Scope scp(ctx, CROWN_K_RELAX, 4.0 * ni.size * (3.0 * M + 2.0 * B * S));
+        launch_alpha_relu(sc.Asave[i], gin, coef_ptr(ctx, i), alpha_lo[i], alpha_up[i], sc.G[i],
+                          g_lo ? g_lo[i] : nullptr, g_up ? g_up[i] : nullptr, step, mode, B, S, ni.size, s);
+        break; }
+      default:
+        return fail(ctx, CROWN_EUNSUPPORTED, "crown_alpha: unsupported op");
+    }
+  }
+  CK(ctx, cudaGetLastError());
+  return CROWN_OK;
+}
+
+}  // namespace
+
+extern "C" int crown_alpha_scratch_bytes(crown_ctx* ctx, int B, int S, size_t* out) {
+  if (!ctx || !out || B <= 0 || S <= 0) return CROWN_EINVAL;
+  AlphaScratch sc;
+  alpha_layout(ctx, B, S, nullptr, sc);
+  *out = sc.bytes;
+  return CROWN_OK;
+}
+
+extern "C" int crown_alpha_grad(crown_ctx* ctx, int B, const float* C_dev, int S, const float* const* l_dev,
+                                const float* const* u_dev, const float* const* alpha_lo_dev,
+                                const float* const* alpha_up_dev, const float* x_lo_dev, const float* x_hi_dev,
+                                float* const* g_lo_dev, float* const* g_up_dev, float* lb_dev, float* ub_dev,
+                                void* scratch_dev, size_t scratch_bytes) {
+  if (!ctx) return CROWN_EINVAL;
+  AlphaScratch sc;
+  int rc = alpha_check(ctx, B, S, C_dev, l_dev, u_dev, alpha_lo_dev, alpha_up_dev, x_lo_dev, x_hi_dev, scratch_dev,
+                       scratch_bytes, false, sc);
+  if (rc) return rc;
+  CK(ctx, cudaMemsetAsync(scratch_dev, 0, sc.bytes, ctx->stream));
+  rc = alpha_backward(ctx, B, S, C_dev, l_dev, u_dev, alpha_lo_dev, alpha_up_dev, x_lo_dev, x_hi_dev, sc, nullptr);
+  if (rc) return rc;
+  if (lb_dev) CK(ctx, cudaMemcpyAsync(lb_dev, sc.lb, (size_t)B * S * 4, cudaMemcpyDeviceToDevice, ctx->stream));
+  if (ub_dev) CK(ctx, cudaMemcpyAsync(ub_dev, sc.ub, (size_t)B * S * 4, cudaMemcpyDeviceToDevice, ctx->stream));
+  return alpha_forward(ctx, B, S, sc, x_lo_dev, x_hi_dev, const_cast<float* const*>(reinterpret_cast<const float* const*>(alpha_lo_dev)),
+                       const_cast<float* const*>(reinterpret_cast<const float* const*>(alpha_up_dev)), g_lo_dev, g_up_dev, nullptr, 0);
+}
+
+extern "C" int crown_alpha_ascent(crown_ctx* ctx, int B, const float* C_dev, int S, const float* const* l_dev,
+                                  const float* const* u_dev, float* const* alpha_lo_dev, float* const* alpha_up_dev,
+                                  const float* x_lo_dev, const float* x_hi_dev, float eta, float decay, int iters,
+                                  int mode, float* lb_best_dev, float* ub_best_dev, float* lb_last_dev,
+                                  float* ub_last_dev, uint8_t* verified_dev, void* scratch_dev, size_t scratch_bytes) {
+  if (!ctx) return CROWN_EINVAL;
+  if (iters < 0 || (mode != 0 && mode != 1) || !(eta >= 0.f) || !(decay > 0.f) || !lb_best_dev || !ub_best_dev)
+    return fail(ctx, CROWN_EINVAL, "crown_alpha_ascent: bad arguments");
+  AlphaScratch sc;
+  const float* const* al = reinterpret_cast<const float* const*>(alpha_lo_dev);
+  const float* const* au = reinterpret_cast<const float* const*>(alpha_up_dev);
+  int rc = alpha_check(ctx, B, S, C_dev, l_dev, u_dev, al, au, x_lo_dev, x_hi_dev, scratch_dev, scratch_bytes, true, sc);
+  if (rc) return rc;
+  cudaStream_t s = ctx->stream;
+  CK(ctx, cudaMemsetAsync(scratch_dev, 0, sc.bytes, s));
+  { Scope scp(ctx, CROWN_K_MISC); launch_alpha_set_step(sc.step, eta, s); }
+  std::vector<char> coef_ready(ctx->nodes.size(), 0);      // the intermediate bounds are fixed: coefficients once
+  for (int t = 0; t <= iters; ++t) {
+    rc = alpha_backward(ctx, B, S, C_dev, l_dev, u_dev, al, au, x_lo_dev, x_hi_dev, sc, &coef_ready);
+    if (rc) return rc;
+    { Scope scp(ctx, CROWN_K_MISC); launch_alpha_best(sc.lb, sc.ub, lb_best_dev, ub_best_dev, sc.step, decay, t == 0, B * S, s); }
+    if (t == iters) break;
+    rc = alpha_forward(ctx, B, S, sc, x_lo_dev, x_hi_dev, alpha_lo_dev, alpha_up_dev, nullptr, nullptr, sc.step, mode);
+    if (rc) return rc;
+  }
+  if (lb_last_dev) CK(ctx, cudaMemcpyAsync(lb_last_dev, sc.lb, (size_t)B * S * 4, cudaMemcpyDeviceToDevice, s));
+  if (ub_last_dev) CK(ctx, cudaMemcpyAsync(ub_last_dev, sc.ub, (size_t)B * S * 4, cudaMemcpyDeviceToDevice, s));
+  if (verified_dev) { Scope scp(ctx, CROWN_K_MISC); launch_verdict(lb_best_dev, verified_dev, B, S, s); }
+  CK(ctx, cudaGetLastError());
   return CROWN_OK;
 }
 

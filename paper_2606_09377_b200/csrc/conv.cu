@@ -239,11 +239,20 @@ conv_bwd_tiled_kernel(const float* __restrict__ A, long long sBr, long long sB, 
     uv[t] = active && ut < g.NX && (cx + S * ut) < g.w && y < g.h;
     u[t] = uv[t] ? ut : 0;
   }
+  // accumulators start from the residual fork's other contribution (addend) when there is one: its loads are issued
+  // here, all at once, and complete behind the first shared-memory fill
+  const long long m_row = m_base + rb;
   float acc[4][CT];
 #pragma unroll
   for (int t = 0; t < 4; ++t)
 #pragma unroll
-    for (int c = 0; c < CT; ++c) acc[t][c] = 0.f;
+    for (int c = 0; c < CT; ++c) {
+      const int ci = ci_base + cg * CT + c;
+      float a0 = 0.f;
+      if (addend != nullptr && active && m_row < rows && uv[t] && ci < g.c_in)
+        a0 = __ldg(addend + ((m_row * g.c_in + ci) * g.h + y) * (long long)g.w + (cx + S * u[t]));
+      acc[t][c] = a0;
+    }
 
   const int nchunks = (g.c_out + g.COC - 1) / g.COC;
   fill(0, 0);
@@ -290,7 +299,7 @@ conv_bwd_tiled_kernel(const float* __restrict__ A, long long sBr, long long sB, 
     for (int t = 0; t < 4; ++t) {
       if (!uv[t]) continue;
       const long long o = ((m * g.c_in + ci) * g.h + y) * (long long)g.w + (cx + S * u[t]);
-      out[o] = addend ? acc[t][c] + addend[o] : acc[t][c];
+      out[o] = acc[t][c];
     }
   }
 }

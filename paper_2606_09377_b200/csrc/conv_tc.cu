@@ -8,11 +8,12 @@
 // (coalesced along x), split it into TF32 hi / lo limbs and write both; one tile per horizontal shift dx (a 4-byte
 // shift cannot be expressed in a 16-byte-granular shared-memory descriptor), the three vertical taps of a dx are
 // descriptor offsets of W rows (multiples of 1024 B).  The 9 x C_in x 32 weight tiles stay resident in shared memory.
-//   warp 0      : MMA issuer (36 tcgen05.mma.kind::tf32 per dx: 3 dy x 4 k-steps x {lo.hi, hi.lo, hi.hi})
-//   warp 1      : TMEM allocator
-//   warps 4-7   : epilogue, lane = output pixel: drains the TMEM accumulator after every dx into an fp32 register sum
-//                 (round 1 measured that long TMEM accumulation chains truncate: 36 MMAs per chain keeps fp32 accuracy),
-//                 adds the residual fork's other contribution (addend) and stores A_in coalesced along x
+//   warp 0      : MMA issuer (up to 36 tcgen05.mma.kind::tf32 per dx: 3 dy x 4 k-steps x {lo.hi, hi.lo, hi.hi}),
+//                 dealt round robin to 8 accumulators
+//   warp 1      : TMEM allocator;  warp 2: signaller (named barrier of the transform warps -> mbarrier of the issuer)
+//   warps 4-7   : epilogue, lane = output pixel: adds up the item's 8 independent TMEM accumulators (each a chain of
+//                 <= 14 MMAs: round 1 measured that long TMEM accumulation chains truncate), adds the residual fork's
+//                 other contribution (addend) and stores A_in coalesced along x
 //   warps 8-15  : transform (NCHW fp32 -> K-major swizzled hi / lo tiles), one dx tile ahead of the tensor core
 // Layers outside this shape (stride 2, 1x1, 8x8 maps, C > 32) stay on the CUDA-core kernel of conv.cu.
 #include <cuda.h>
@@ -28,12 +29,18 @@ namespace ctc {
 
 using namespace tc;
 
+// round-to-nearest (ties away) to TF32 on the bit pattern: cvt.rna.tf32.f32 for finite inputs in two integer ops
+__device__ __forceinline__ float tf32_rn_bits(float x) {
+  return __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xffffe000u);
+}
+
 constexpr int KC = 32;                     // output channels per K chunk = one 128-byte swizzle row
 constexpr int XF_WARPS = 8;
 constexpr int THREADS = 32 * (8 + XF_WARPS);
 constexpr int MAXROWS = 192;               // (TR + 2) * W rows of a dx tile: W = 32 -> 6 * 32, W = 16 -> 10 * 16
 constexpr int TILE_BYTES = MAXROWS * 128;  // one limb of one dx tile
 constexpr int NBUF = 3;                    // dx tiles in flight
+constexpr int NACC = 8;                    // independent TMEM accumulators per item (see the MMA issuer)
 
 template <int NPAD>
 struct Smem {
@@ -44,7 +51,7 @@ struct Smem {
 };
 
 struct Params {
-  const float* A; const float* A_lo; long long sBr, sB, ld;   // A_out view [2, B, R, c_out * H * W]
+  const float* A; long long sBr, sB, ld;                       // A_out view [2, B, R, c_out * H * W] (fp32, no lo limb)
   const float* Wgt;                                             // [c_out, c_in, 3, 3]
   const float* addend; float* out;                              // [rows, c_in * H * W] contiguous
   int B, R; long long rows;
@@ -87,11 +94,11 @@ __global__ void __launch_bounds__(THREADS, 1) conv_bwd_tc_kernel(const Params p)
     *reinterpret_cast<float4*>(gbase + S::W_BYTES + off) = lo;
   }
   if (warp == 0 && lane == 0) {
-    for (int b = 0; b < NBUF; ++b) { mbar_init(full_bar(b), XF_WARPS * 32); mbar_init(empty_bar(b), 1); }
+    for (int b = 0; b < NBUF; ++b) { mbar_init(full_bar(b), 1); mbar_init(empty_bar(b), 1); }
     for (int b = 0; b < 2; ++b) { mbar_init(accfull_bar(b), 1); mbar_init(accempty_bar(b), 4); }
     fence_barrier_init();
   }
-  if (warp == 1) { tmem_alloc(tmem_slot, 2 * NPAD < 32 ? 32 : 2 * NPAD); tmem_relinquish(); }
+  if (warp == 1) { tmem_alloc(tmem_slot, 2 * NACC * NPAD); tmem_relinquish(); }
   fence_proxy_async();                       // the weight tiles were written through the generic proxy
   tcgen05_fence_before();
   __syncthreads();
@@ -100,21 +107,24 @@ __global__ void __launch_bounds__(THREADS, 1) conv_bwd_tc_kernel(const Params p)
 
   if (warp == 0) {
     // ===================== MMA issuer =====================
+    // A 128 x NPAD accumulator tile is small: back-to-back MMAs into the SAME tile serialise on the tensor core's
+    // accumulate latency (measured: ~250 cycles per MMA with one accumulator, against ~32 cycles of operand reads).
+    // The MMAs of an item are therefore dealt round robin to NACC independent accumulators, which the epilogue adds
+    // up; every TMEM chain is then at most 14 MMAs long, so no intermediate drains are needed for fp32 accuracy.
     if (lane == 0) {
       constexpr uint32_t idesc = make_idesc_tf32(128, NPAD);
-      uint32_t seq = 0;                                 // dx passes issued so far
-      for (long long it = blockIdx.x; it < items; it += gridDim.x) {
+      const int ksteps = (p.c_out + UMMA_K - 1) / UMMA_K;   // channels >= c_out are zero padding: not multiplied
+      uint32_t seq = 0, item = 0;
+      for (long long it = blockIdx.x; it < items; it += gridDim.x, ++item) {
+        const int ab = item & 1u; const uint32_t apar = (item >> 1) & 1u;
+        mbar_wait(accempty_bar(ab), apar ^ 1u);
+        uint32_t cnt = 0;
         for (int dxb = 0; dxb < 3; ++dxb, ++seq) {
           const int buf = seq % NBUF; const uint32_t bpar = (seq / NBUF) & 1u;
-          const int ab = seq & 1u; const uint32_t apar = (seq >> 1) & 1u;
           mbar_wait(full_bar(buf), bpar);
-          mbar_wait(accempty_bar(ab), apar ^ 1u);
           tcgen05_fence_after();
           const uint32_t sA_hi = base + S::A_OFF + buf * 2 * TILE_BYTES, sA_lo = sA_hi + TILE_BYTES;
-          const uint32_t tmem_d = tmem_base + ab * NPAD;
           const int j = 2 - dxb;                         // tile dxb holds A_out shifted by s = dxb - 1 = 1 - j
-          const int ksteps = (p.c_out + UMMA_K - 1) / UMMA_K;   // channels >= c_out are zero padding: not multiplied
-          uint32_t acc = 0;
 #pragma unroll
           for (int i = 0; i < 3; ++i) {
             const uint32_t roff = (uint32_t)((2 - i) * p.W) * 128u;     // vertical tap = window offset of (2 - i) image rows
@@ -127,61 +137,114 @@ __global__ void __launch_bounds__(THREADS, 1) conv_bwd_tc_kernel(const Params p)
               const uint64_t dA_lo = make_kmajor_sw128_desc(sA_lo + roff + koff);
               const uint64_t dB_hi = make_kmajor_sw128_desc(sB_hi + koff);
               const uint64_t dB_lo = make_kmajor_sw128_desc(sB_lo + koff);
-              umma_tf32(tmem_d, dA_lo, dB_hi, idesc, acc);
-              umma_tf32(tmem_d, dA_hi, dB_lo, idesc, 1u);
-              umma_tf32(tmem_d, dA_hi, dB_hi, idesc, 1u);
-              acc = 1u;
+              const uint32_t t0 = tmem_base + (ab * NACC + (cnt % NACC)) * NPAD; const uint32_t f0 = cnt >= NACC; ++cnt;
+              const uint32_t t1 = tmem_base + (ab * NACC + (cnt % NACC)) * NPAD; const uint32_t f1 = cnt >= NACC; ++cnt;
+              const uint32_t t2 = tmem_base + (ab * NACC + (cnt % NACC)) * NPAD; const uint32_t f2 = cnt >= NACC; ++cnt;
+              umma_tf32(t0, dA_lo, dB_hi, idesc, f0);
+              umma_tf32(t1, dA_hi, dB_lo, idesc, f1);
+              umma_tf32(t2, dA_hi, dB_hi, idesc, f2);
             }
           }
           umma_commit(empty_bar(buf));
-          umma_commit(accfull_bar(ab));
         }
+        umma_commit(accfull_bar(ab));
+      }
+    }
+  } else if (warp == 2) {
+    // ===================== signaller: 256 named-barrier arrivals of the transform threads -> one mbarrier arrive ======
+    uint32_t seq = 0;
+    for (long long it = blockIdx.x; it < items; it += gridDim.x) {
+      for (int dxb = 0; dxb < 3; ++dxb, ++seq) {
+        const int buf = seq % NBUF;
+        asm volatile("bar.sync %0, %1;" :: "r"(1 + buf), "n"(XF_WARPS * 32 + 32) : "memory");
+        if (lane == 0) { fence_proxy_async(); mbar_arrive(full_bar(buf)); }
       }
     }
   } else if (warp >= 8) {
     // ===================== transform: NCHW fp32 -> K-major swizzled TF32 hi / lo tiles =====================
-    const int xw = warp - 8;                             // 0..7 = group of 4 output channels (co4)
-    uint32_t seq = 0;
-    for (long long it = blockIdx.x; it < items; it += gridDim.x) {
+    // A warp task = (group of 4 output channels, 32 consecutive tile rows); tasks are dealt round robin to the 8
+    // warps and everything about a task that does not depend on the item (tile offset, source offset, edge flags) is
+    // computed once.  Per item every element of the haloed band is loaded ONCE: all of a thread's loads are issued
+    // back to back with no dependent instruction in between (a use right after a load stalls the in-order warp and
+    // serialises the remaining loads: measured 15k cycles per item), and the NEXT item's loads are issued before this
+    // item's tiles are written, so their latency hides behind the shuffle / store phase.  The three horizontally
+    // shifted tiles are produced from registers with warp shuffles along x.
+    const int xw = warp - 8;
+    const int wshift = p.W == 32 ? 5 : 4;
+    const int G = 2 * ((p.c_out + UMMA_K - 1) / UMMA_K);    // groups of 4 channels that are multiplied
+    const int ntask = G * (tile_rows >> 5);
+    constexpr int NT = 6;                                   // tasks per warp (8 groups x 6 chunks / 8 warps)
+    uint32_t toff[NT];                                      // byte offset of the task's 16-byte chunk in a tile
+    int soff[NT], tyy[NT];                                  // source offset (first of the 4 channels) at y0 = 1; tile row yy
+    bool tval[NT], okl[NT], okr[NT];                        // task exists; left / right neighbour inside the image row
+    int cval[NT];                                           // channels of the group below c_out (0..4)
+#pragma unroll
+    for (int t = 0; t < NT; ++t) {
+      const int id = xw + 8 * t;
+      const int co4 = id % G, rch = id / G;
+      const int r = rch * 32 + lane;
+      const int x = r & (p.W - 1);
+      tval[t] = id < ntask;
+      tyy[t] = r >> wshift;
+      toff[t] = (uint32_t)r * 128u + (((uint32_t)co4 ^ (uint32_t)(r & 7)) << 4);
+      soff[t] = co4 * 4 * HW + (tyy[t] - 1) * p.W + x;
+      okl[t] = x >= 1; okr[t] = x + 1 < p.W;
+      cval[t] = min(4, max(0, p.c_out - co4 * 4));
+    }
+    auto load_item = [&](long long it, float (&v)[NT][4]) {
       const long long m = it / p.bands;
       const int y0 = (int)(it % p.bands) * p.TR;
       const int r_ = (int)(m % p.R);
       const long long tt = m / p.R;
-      const long long roff = (tt / p.B) * p.sBr + (tt % p.B) * p.sB + (long long)r_ * p.ld;
-      const float* src = p.A + roff;
-      const float* src_lo = p.A_lo ? p.A_lo + roff : nullptr;
+      const float* src = p.A + (tt / p.B) * p.sBr + (tt % p.B) * p.sB + (long long)r_ * p.ld + y0 * p.W;
+#pragma unroll
+      for (int t = 0; t < NT; ++t) {
+        const int y = y0 - 1 + tyy[t];
+        const bool in = tval[t] && y >= 0 && y < p.H;
+        const float* q = src + soff[t];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) v[t][e] = (in && e < cval[t]) ? __ldg(q + e * HW) : 0.f;
+      }
+    };
+    uint32_t seq = 0;
+    float v[NT][4];
+    if ((long long)blockIdx.x < items) load_item(blockIdx.x, v);
+    for (long long it = blockIdx.x; it < items; it += gridDim.x) {
+      float vn[NT][4];
+      if (it + gridDim.x < items) load_item(it + gridDim.x, vn);
       for (int dxb = 0; dxb < 3; ++dxb, ++seq) {
         const int buf = seq % NBUF; const uint32_t bpar = (seq / NBUF) & 1u;
         mbar_wait(empty_bar(buf), bpar ^ 1u);
         uint8_t* t_hi = gbase + S::A_OFF + buf * 2 * TILE_BYTES;
         uint8_t* t_lo = t_hi + TILE_BYTES;
-        const int s = dxb - 1;
-        const bool used = xw * 4 < ((p.c_out + UMMA_K - 1) / UMMA_K) * UMMA_K;     // this warp's channels are multiplied
-        for (int r = lane; used && r < tile_rows; r += 32) {     // tile row = (yy, x): lanes run along x (coalesced loads)
-          const int yy = r / p.W, x = r % p.W;
-          const int y = y0 - 1 + yy, xs = x + s;
-          const bool in = y >= 0 && y < p.H && xs >= 0 && xs < p.W;
-          float v[4];
+        const int s = dxb - 1;                              // tile[yy][x] = A_out[y0 - 1 + yy][x + s]
+#pragma unroll
+        for (int t = 0; t < NT; ++t) {
+          if (!tval[t]) continue;                           // warp-uniform
+          const bool ok = s == 0 || (s < 0 ? okl[t] : okr[t]);   // neighbour inside the image row (else zero padding)
+          float4 hi, lo;
+          float w[4];
 #pragma unroll
           for (int e = 0; e < 4; ++e) {
-            const int co = xw * 4 + e;
-            float val = 0.f;
-            if (in && co < p.c_out) {
-              const long long o = (long long)co * HW + y * p.W + xs;
-              val = src[o];
-              if (src_lo) val += src_lo[o];
-            }
-            v[e] = val;
+            const float nb = s == 0 ? v[t][e] : __shfl_sync(0xffffffffu, v[t][e], (lane + s) & 31);
+            w[e] = ok ? nb : 0.f;
           }
-          float4 hi, lo;
-          tf32_split(v[0], hi.x, lo.x); tf32_split(v[1], hi.y, lo.y); tf32_split(v[2], hi.z, lo.z); tf32_split(v[3], hi.w, lo.w);
-          const uint32_t off = (uint32_t)r * 128u + (((uint32_t)xw ^ (uint32_t)(r & 7)) << 4);
-          *reinterpret_cast<float4*>(t_hi + off) = hi;
-          *reinterpret_cast<float4*>(t_lo + off) = lo;
+          hi.x = tf32_rn_bits(w[0]); lo.x = tf32_rn_bits(w[0] - hi.x);
+          hi.y = tf32_rn_bits(w[1]); lo.y = tf32_rn_bits(w[1] - hi.y);
+          hi.z = tf32_rn_bits(w[2]); lo.z = tf32_rn_bits(w[2] - hi.z);
+          hi.w = tf32_rn_bits(w[3]); lo.w = tf32_rn_bits(w[3] - hi.w);
+          *reinterpret_cast<float4*>(t_hi + toff[t]) = hi;
+          *reinterpret_cast<float4*>(t_lo + toff[t]) = lo;
         }
         fence_proxy_async();                 // generic-proxy smem writes -> visible to the tensor core (async proxy)
-        mbar_arrive(full_bar(buf));
+        // hand-off through a named barrier and the signaller warp: an mbarrier arrive (release) by THIS thread would
+        // first wait for its prefetched global loads of the next item and expose their latency on every pass
+        asm volatile("bar.arrive %0, %1;" :: "r"(1 + buf), "n"(XF_WARPS * 32 + 32) : "memory");
       }
+#pragma unroll
+      for (int t = 0; t < NT; ++t)
+#pragma unroll
+        for (int e = 0; e < 4; ++e) v[t][e] = vn[t][e];
     }
   } else if (warp >= 4) {
     // ===================== epilogue: lane = output pixel =====================
@@ -193,33 +256,37 @@ __global__ void __launch_bounds__(THREADS, 1) conv_bwd_tc_kernel(const Params p)
       const long long m = it / p.bands;
       const int y0 = (int)(it % p.bands) * p.TR;
       float sum[NPAD];
+      // the residual fork's other contribution: all loads issued up front (they complete while the MMAs still run)
+      const float* arow = p.addend ? p.addend + (m * p.c_in) * (long long)HW + (long long)(y0 + ty) * p.W + x : nullptr;
 #pragma unroll
-      for (int c = 0; c < NPAD; ++c) sum[c] = 0.f;
-      for (int dxb = 0; dxb < 3; ++dxb, ++seq) {
+      for (int c = 0; c < NPAD; ++c) sum[c] = (arow && c < p.c_in) ? __ldg(arow + (long long)c * HW) : 0.f;
+      {
         const int ab = seq & 1u; const uint32_t apar = (seq >> 1) & 1u;
+        ++seq;
         mbar_wait(accfull_bar(ab), apar);
         tcgen05_fence_after();
-        const uint32_t taddr = tmem_base + ((uint32_t)(quad * 32) << 16) + ab * NPAD;
-        if constexpr (NPAD == 32) {
-          uint32_t v[32]; tmem_ld32(taddr, v); tmem_ld_wait();
 #pragma unroll
-          for (int c = 0; c < 32; ++c) sum[c] += __uint_as_float(v[c]);
-        } else {
-          uint32_t v[16]; tmem_ld16(taddr, v); tmem_ld_wait();
+        for (int a = 0; a < NACC; ++a) {
+          const uint32_t taddr = tmem_base + ((uint32_t)(quad * 32) << 16) + (ab * NACC + a) * NPAD;
+          if constexpr (NPAD == 32) {
+            uint32_t v[32]; tmem_ld32(taddr, v); tmem_ld_wait();
 #pragma unroll
-          for (int c = 0; c < 16; ++c) sum[c] += __uint_as_float(v[c]);
+            for (int c = 0; c < 32; ++c) sum[c] += __uint_as_float(v[c]);
+          } else {
+            uint32_t v[16]; tmem_ld16(taddr, v); tmem_ld_wait();
+#pragma unroll
+            for (int c = 0; c < 16; ++c) sum[c] += __uint_as_float(v[c]);
+          }
         }
         tcgen05_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(accempty_bar(ab));
       }
       float* orow = p.out + (m * p.c_in) * (long long)HW + (long long)(y0 + ty) * p.W + x;
-      const float* arow = p.addend ? p.addend + (m * p.c_in) * (long long)HW + (long long)(y0 + ty) * p.W + x : nullptr;
 #pragma unroll
       for (int c = 0; c < NPAD; ++c) {
         if (c < p.c_in) {
-          float o = sum[c];
-          if (arow) o += arow[(long long)c * HW];
+          const float o = sum[c];
           orow[(long long)c * HW] = o;
         }
       }
@@ -228,7 +295,7 @@ __global__ void __launch_bounds__(THREADS, 1) conv_bwd_tc_kernel(const Params p)
 
   tcgen05_fence_before();
   __syncthreads();
-  if (warp == 1) { tcgen05_fence_after(); tmem_dealloc(tmem_base, 2 * NPAD < 32 ? 32 : 2 * NPAD); }
+  if (warp == 1) { tcgen05_fence_after(); tmem_dealloc(tmem_base, 2 * NACC * NPAD); }
 }
 
 }  // namespace ctc
@@ -240,14 +307,18 @@ int conv_tc_init_device() {
 }
 
 int conv_tc_supported(int c_in, int h, int w, int c_out, int kh, int kw, int stride, int pad, int ho, int wo) {
+  // Measured per layer on B200 (profiles/r2_conv_tc_vs_ffma.md): a 128 x N x 8 MMA costs ~105 cycles whatever N <= 32 is,
+  // so the tensor-core kernel wins 2.2x at 32 channels (16 x 16 maps: 135 vs 295 us) and loses at 16 channels
+  // (32 x 32 maps: 300 vs 280 us; the 3-channel stem: 299 vs 164 us).  It is used where it wins.
   return kh == 3 && kw == 3 && stride == 1 && pad == 1 && ho == h && wo == w && (w == 16 || w == 32) &&
-         (h * w) % 128 == 0 && c_in >= 1 && c_in <= 32 && c_out >= 1 && c_out <= 32;
+         (h * w) % 128 == 0 && c_in > 16 && c_in <= 32 && c_out > 16 && c_out <= 32;
 }
 
 int launch_conv_transpose_tc(const AView& A, const float* W, const float* addend, float* out, int B, int R,
                              int c_in, int h, int w, int c_out, int num_sms, cudaStream_t s) {
   ctc::Params p;
-  p.A = A.p; p.A_lo = A.lo; p.sBr = A.sBr; p.sB = A.sB; p.ld = A.ld;
+  if (A.lo) return -1;                   // split views go to the CUDA-core kernel (none reaches a conv node today)
+  p.A = A.p; p.sBr = A.sBr; p.sB = A.sB; p.ld = A.ld;
   p.Wgt = W; p.addend = addend; p.out = out; p.B = B; p.R = R; p.rows = 2LL * B * R;
   p.c_in = c_in; p.c_out = c_out; p.H = h; p.W = w; p.TR = 128 / w; p.bands = h / p.TR;
   const long long items = p.rows * p.bands;

@@ -124,6 +124,21 @@ int conv_tc_supported(int c_in, int h, int w, int c_out, int kh, int kw, int str
 int launch_conv_transpose_tc(const AView& A, const float* W, const float* addend, float* out, int B, int R,
                              int c_in, int h, int w, int c_out, int num_sms, cudaStream_t s);
 
+// NEXT-1 -- alpha optimisation: kernels of the forward sweep G = d bound / d A (alpha.cu).
+void launch_alpha_corner(const float* A0, const float* x_lo, const float* x_hi, float* G, int B, int S, int n0,
+                         cudaStream_t s);
+void launch_alpha_linear(const float* G, const float* W, const float* bias, float* D, int M, int N, int K,
+                         cudaStream_t s);
+void launch_alpha_conv(const float* W, const float* bias, const float* in, float* out, long long M, int c_in, int h,
+                       int w, int c_out, int kh, int kw, int stride, int pad, int ho, int wo, cudaStream_t s);
+void launch_alpha_add(const float* a, const float* b, float* o, long long cnt, cudaStream_t s);
+void launch_alpha_relu(const float* A, const float* Gin, const float4* coef, float* alpha_lo, float* alpha_up,
+                       float* Gout, float* g_lo, float* g_up, const float* step, int mode, int B, int S, int n,
+                       cudaStream_t s);
+void launch_alpha_best(const float* lb, const float* ub, float* lb_best, float* ub_best, float* step, float decay,
+                       int first, int count, cudaStream_t s);
+void launch_alpha_set_step(float* step, float v, cudaStream_t s);
+
 // Per-device kernel attributes (opt-in dynamic shared memory sizes).  cudaFuncSetAttribute applies to the CURRENT
 // device only, so crown_init calls this for the device of every new context (a process-wide "done" flag would
 // leave a second device without them).  Returns 0 on success.

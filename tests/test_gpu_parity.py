@@ -225,12 +225,42 @@ def test_boundary_calls_one_by_one():
             _close(g, oub, "ub")
 
 
-def test_cfg5_half_scale_tensor_core_conv():
-    """cfg5 / 2 (16 x 16 maps, 8..32 channels): the stem and block-1 BoundConv backward steps run as the per-tap
-    implicit GEMM on tcgen05 (conv_tc.cu); same parity bar, and the CUDA-core path agrees within the tolerance."""
-    wl = W.make(5, scale=2, B=2)
-    ctx, res = _check_workload(wl)
+def test_tensor_core_conv_backward_small_resnet():
+    """A 16 x 16, 32-channel ResNet (stem + 2 residual blocks): the 3x3 stride-1 BoundConv backward steps with 32
+    channels run as the per-tap implicit GEMM on tcgen05 (conv_tc.cu), one of them with the residual fork's other
+    contribution added in its epilogue.  Same parity bar on lb / ub AND on the input-layer coefficients A^0 (every
+    conv step feeds them; with IBP intermediates the bias term dominates lb, so lb alone would not see a conv error),
+    and the CUDA-core path agrees within the tolerance without being the same arithmetic."""
+    rng = np.random.Generator(np.random.PCG64(W.SEED_BASE + 7000))
+    net = W.resnet(rng, in_shape=(3, 16, 16), stem=32, blocks=((32, 1), (32, 1)), fc=48, n_classes=12)
+    B, S = 2, 7
+    x0 = rng.random((B, net.n_in)).astype(np.float32)
+    C = rng.standard_normal((B, S, net.n_out)).astype(np.float32)
+    al = [rng.random((B, S, net.nodes[i].size)).astype(np.float32) for i in net.relu_ids()]
+    wl = W.Workload(cfg=5, name="resnet16x32", net=net, x0=x0, eps=np.full((B,), 2.0 / 255.0, np.float32), C=C,
+                    labels=np.zeros(B, int), alpha=al, intermediate="ibp", eps_set=(2.0 / 255.0,))
+    ctx, res = _check_workload(wl, free_running=False)   # IBP intermediates, 40k neurons: the forced-bounds protocol is the check
     lo, hi = wl.box()
-    res2 = _ctx(wl.net, wl.B, wl.S, disable_conv_tc=1).run(lo, hi, wl.C, wl.alpha, wl.intermediate)
+    ctx2 = _ctx(wl.net, wl.B, wl.S, disable_conv_tc=1)
+    res2 = ctx2.run(lo, hi, wl.C, wl.alpha, wl.intermediate)
     _close(_np(res["lb"]), _np(res2["lb"]), "tensor-core vs CUDA-core conv lb")
     _close(_np(res["ub"]), _np(res2["ub"]), "tensor-core vs CUDA-core conv ub")
+    ald = {i: a for i, a in zip(wl.net.relu_ids(), wl.alpha)}
+    outs = [c.crown_backward(wl.B, len(wl.net.nodes) - 1, res["pre"], Cmat=wl.C, alpha_lo=ald, alpha_up=ald,
+                             box=(lo, hi), want_A=True) for c in (ctx, ctx2)]
+    A_tc, A_cc = _np(outs[0]["A"]), _np(outs[1]["A"])
+    assert not np.array_equal(A_tc, A_cc)                 # the two paths really are different kernels
+    for p in range(wl.B):
+        forced = {i: (_np(l)[p].astype(np.float64), _np(u)[p].astype(np.float64)) for i, (l, u) in res["pre"].items()}
+        alp = {i: a[p] for i, a in ald.items()}
+        _, _, (A_lo, A_up, d_lo, d_up) = O.final_bounds(wl.net, lo[p], hi[p], wl.C[p], forced, alp, alp)
+        # A^0 entries are cancelling sums over ~10^4 paths: the bar is the stated tolerance with the absolute part
+        # scaled to the row's magnitude (fp32 rounding is relative to the summands, not to the cancelled result)
+        for k, name in enumerate(("tc", "cuda-core")):
+            A, d = (A_tc, A_cc)[k], _np(outs[k]["d"])
+            for br, ref in ((0, A_lo), (1, A_up)):
+                sc = np.abs(ref).max(axis=-1, keepdims=True)
+                err = np.abs(A[br, p] - ref) - (ATOL * sc + RTOL * np.abs(ref))
+                assert np.all(err <= 0), f"{name} A^0 branch {br} prop {p}: worst excess {err.max():.3e}"
+            _close(d[0, p], d_lo, f"{name} d_lo")
+            _close(d[1, p], d_up, f"{name} d_up")
