@@ -57,6 +57,8 @@ def parse_args():
     ap.add_argument("--no-epi-fusion", action="store_true", help="run the relaxation as its own kernel (debug)")
     ap.add_argument("--no-graph", action="store_true", help="do not replay crown_run from a CUDA graph (debug)")
     ap.add_argument("--no-conv-tc", action="store_true", help="BoundConv backward on the CUDA-core kernel everywhere (debug)")
+    ap.add_argument("--alpha-iters", type=int, default=10,
+                    help="alpha-mode configs: also time this many projected ascent steps on alpha (NEXT-1; 0 = skip)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     return ap.parse_args()
@@ -473,6 +475,32 @@ def measure_config(cfgname, args, steps, warmup, dev, local, world, tf32_peak, w
     if dom != "gemm_tc" and aw_tflops:
         roof["aw_contraction"] = {"achieved": aw_tflops, "peak": tc_peak, "frac": aw_tflops / tc_peak, "unit": "TFLOP/s"}
 
+    # ---- NEXT-1: alpha optimisation of the final bound, reported beside the step, not part of it -------
+    alpha_opt = None
+    if alpha is not None and args.alpha_iters > 0:
+        T = args.alpha_iters
+        res = {k: torch.empty(B, S, device=dev) for k in ("lb_best", "ub_best", "lb_last", "ub_last")}
+        res["verified"] = torch.empty(B, dtype=torch.uint8, device=dev)
+        step_device()                                     # (l, u) and the bound at the given alpha
+        torch.cuda.synchronize()
+        lb_start = io["lb"].clone()
+        ms_a = []
+        for it in range(3):
+            al = {i: a.clone() for i, a in alpha.items()}
+            au = {i: a.clone() for i, a in alpha.items()}
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            ctx.alpha_ascent_device(io["l"], io["u"], Cd, al, au, xlo, xhi, 0.05, 0.98, T, 1, res)
+            e1.record(); e1.synchronize()
+            ms_a.append(e0.elapsed_time(e1))
+        gain = res["lb_best"] - lb_start
+        alpha_opt = {"iters": T, "rule": "sign step, eta 0.05, decay 0.98", "ms_total": min(ms_a), "ms_per_iter": min(ms_a) / (T + 1),
+                     "mean_lb_gain": float(gain.mean().item()), "mean_abs_lb_start": float(lb_start.abs().mean().item()),
+                     "rows_tightened_frac": float((gain > 0).float().mean().item()),
+                     "verified_before": verified, "verified_after": int(res["verified"].sum().item())}
+        del res, al, au
+
     peak_ws = ctx.peak_bytes()
     peak_torch = torch.cuda.max_memory_allocated(dev)
     rc_rows = ctx.row_chunk()
@@ -490,7 +518,8 @@ def measure_config(cfgname, args, steps, warmup, dev, local, world, tf32_peak, w
         "kernel_time_shares": shares, "kernel_classes": per_class, "roofline": roof, "cpu_baseline": cpu,
         "e2e": {"value": world * B / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                 "d2h_bytes_per_step": int(d2h), "ms_per_step": ms_e2e, "steps": n_aux},
-        "gpu_launches": int(launches_per_step * steps), "gpu_launches_per_step": int(launches_per_step), "clocks": clocks}
+        "gpu_launches": int(launches_per_step * steps), "gpu_launches_per_step": int(launches_per_step), "clocks": clocks,
+        "alpha_opt": alpha_opt}
     ctx.close()
     del ctx, xlo, xhi, Cd, alpha, io, flush, wl
     gc.collect()
@@ -525,13 +554,13 @@ def run_b200(args):
             r = measure_config(c, args, st, 3, dev, local, world, tf32_peak, with_cpu)
             per[c] = {k: r[k] for k in ("value", "unit", "steps", "ms_per_step", "config", "verified_last_batch", "aw_tflops",
                                         "peak_hbm_gb", "kernel_time_shares", "kernel_classes", "roofline", "cpu_baseline",
-                                        "e2e", "gpu_launches_per_step", "clocks")}
+                                        "e2e", "gpu_launches_per_step", "clocks", "alpha_opt")}
     if rank == 0:
         line = {"metric": METRIC, "value": main["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": main["ms_per_step"], "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32 (3xTF32 products, fp32 accumulate)", "data": "synthetic"}
         for k in ("config", "verified_last_batch", "aw_tflops", "aw_flops_per_step", "peak_hbm_gb", "kernel_time_shares",
-                  "kernel_classes", "roofline", "cpu_baseline", "e2e", "gpu_launches", "gpu_launches_per_step", "clocks"):
+                  "kernel_classes", "roofline", "cpu_baseline", "e2e", "gpu_launches", "gpu_launches_per_step", "clocks", "alpha_opt"):
             line[k] = main[k]
         line["tf32_dense_peak_tflops"] = tf32_peak
         line["per_config"] = per

@@ -9,49 +9,69 @@
 namespace crownb200 {
 
 // ---- a2: IBP through Conv2d.  c' = conv(c, W) + b, r' = conv(r, |W|);  l' = c' - r', u' = c' + r'.
-// grid: (spatial tiles, c_out / 4, B); one thread per output pixel of FOUR output channels, so every (l, u) pair
-// read from global memory feeds 8 FMAs; the filters of the 4 channels sit in shared memory.
+// grid: (spatial tiles, c_out / 4, B); block: (PIX output pixels) x (CS slices of the input channels).  A thread owns
+// one output pixel of FOUR output channels for its slice of input channels, so every (l, u) pair read from global
+// memory feeds 8 FMAs and the dependent tap loop is c_in / CS * kh * kw long instead of c_in * kh * kw (the maps here
+// are 8..32 wide with 3..64 channels and B = 8 images: the kernel is latency-bound, parallelism is what it lacks);
+// the CS partial sums are added in slice order through shared memory (deterministic).
 constexpr int kIbpConvCO = 4;
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(512)
 ibp_conv_kernel(const float* __restrict__ W, const float* __restrict__ bias, const float* __restrict__ l_in,
                 const float* __restrict__ u_in, int relu_in, float* __restrict__ l_out,
                 float* __restrict__ u_out, int c_in, int h, int w, int c_out, int kh, int kw, int stride,
                 int pad, int ho, int wo) {
-  extern __shared__ float sw[];   // [kIbpConvCO][c_in*kh*kw]
+  extern __shared__ float sw[];   // [kIbpConvCO][c_in*kh*kw] filters, then [CS][PIX][2*kIbpConvCO] partial sums
   const int co0 = blockIdx.y * kIbpConvCO, b = blockIdx.z;
   const int fsz = c_in * kh * kw;
-  for (int i = threadIdx.x; i < kIbpConvCO * fsz; i += blockDim.x) {
+  const int PIX = blockDim.x, CS = blockDim.y;
+  const int tid = threadIdx.y * PIX + threadIdx.x, nthr = PIX * CS;
+  float* red = sw + kIbpConvCO * fsz;
+  for (int i = tid; i < kIbpConvCO * fsz; i += nthr) {
     const int o = i / fsz, k = i % fsz;
     sw[i] = (co0 + o < c_out) ? W[(long long)(co0 + o) * fsz + k] : 0.f;
   }
   __syncthreads();
-  const int pix = blockIdx.x * blockDim.x + threadIdx.x;
-  if (pix >= ho * wo) return;
-  const int p = pix / wo, q = pix % wo;
+  const int pix = blockIdx.x * PIX + threadIdx.x;
+  const bool live = pix < ho * wo;
+  const int p = live ? pix / wo : 0, q = live ? pix % wo : 0;
   const float* lb = l_in + (long long)b * c_in * h * w;
   const float* ub = u_in + (long long)b * c_in * h * w;
   float c[kIbpConvCO], r[kIbpConvCO];
 #pragma unroll
   for (int o = 0; o < kIbpConvCO; ++o) { c[o] = 0.f; r[o] = 0.f; }
-  for (int ci = 0; ci < c_in; ++ci)
-    for (int i = 0; i < kh; ++i) {
-      const int y = p * stride + i - pad;
-      if (y < 0 || y >= h) continue;
-      for (int j = 0; j < kw; ++j) {
-        const int x = q * stride + j - pad;
-        if (x < 0 || x >= w) continue;
-        float lo = lb[(ci * h + y) * w + x], hi = ub[(ci * h + y) * w + x];
-        if (relu_in) { lo = fmaxf(lo, 0.f); hi = fmaxf(hi, 0.f); }
-        const float xc = 0.5f * (lo + hi), xr = 0.5f * (hi - lo);
-        const int k = (ci * kh + i) * kw + j;
+  if (live)
+    for (int ci = threadIdx.y; ci < c_in; ci += CS)
+      for (int i = 0; i < kh; ++i) {
+        const int y = p * stride + i - pad;
+        if (y < 0 || y >= h) continue;
+        for (int j = 0; j < kw; ++j) {
+          const int x = q * stride + j - pad;
+          if (x < 0 || x >= w) continue;
+          float lo = lb[(ci * h + y) * w + x], hi = ub[(ci * h + y) * w + x];
+          if (relu_in) { lo = fmaxf(lo, 0.f); hi = fmaxf(hi, 0.f); }
+          const float xc = 0.5f * (lo + hi), xr = 0.5f * (hi - lo);
+          const int k = (ci * kh + i) * kw + j;
 #pragma unroll
-        for (int o = 0; o < kIbpConvCO; ++o) {
-          const float wv = sw[o * fsz + k];
-          c[o] = fmaf(wv, xc, c[o]);
-          r[o] = fmaf(fabsf(wv), xr, r[o]);
+          for (int o = 0; o < kIbpConvCO; ++o) {
+            const float wv = sw[o * fsz + k];
+            c[o] = fmaf(wv, xc, c[o]);
+            r[o] = fmaf(fabsf(wv), xr, r[o]);
+          }
         }
       }
+  if (CS > 1) {
+    float* mine = red + ((size_t)threadIdx.y * PIX + threadIdx.x) * (2 * kIbpConvCO);
+#pragma unroll
+    for (int o = 0; o < kIbpConvCO; ++o) { mine[o] = c[o]; mine[kIbpConvCO + o] = r[o]; }
+    __syncthreads();
+    if (threadIdx.y != 0) return;
+    for (int sl = 1; sl < CS; ++sl) {
+      const float* oth = red + ((size_t)sl * PIX + threadIdx.x) * (2 * kIbpConvCO);
+#pragma unroll
+      for (int o = 0; o < kIbpConvCO; ++o) { c[o] += oth[o]; r[o] += oth[kIbpConvCO + o]; }
     }
+  }
+  if (!live) return;
 #pragma unroll
   for (int o = 0; o < kIbpConvCO; ++o) {
     const int co = co0 + o;
@@ -67,12 +87,14 @@ void launch_ibp_conv(const float* W, const float* bias, const float* l_in, const
                      float* l_out, float* u_out, int B, int c_in, int h, int w, int c_out, int kh, int kw,
                      int stride, int pad, int ho, int wo, cudaStream_t s) {
   if (B <= 0) return;
-  int threads = 256;
-  while (threads > 32 && threads / 2 >= ho * wo) threads /= 2;
-  dim3 grid(ceil_div(ho * wo, threads), ceil_div(c_out, kIbpConvCO), B);
-  size_t smem = (size_t)kIbpConvCO * c_in * kh * kw * sizeof(float);
-  ibp_conv_kernel<<<grid, threads, smem, s>>>(W, bias, l_in, u_in, relu_in, l_out, u_out, c_in, h, w, c_out,
-                                              kh, kw, stride, pad, ho, wo);
+  int pix = 128;
+  while (pix > 32 && pix / 2 >= ho * wo) pix /= 2;
+  int cs = 1;
+  while (cs < 8 && cs * 2 <= c_in && pix * cs * 2 <= 512) cs *= 2;
+  dim3 grid(ceil_div(ho * wo, pix), ceil_div(c_out, kIbpConvCO), B), block(pix, cs);
+  size_t smem = ((size_t)kIbpConvCO * c_in * kh * kw + (cs > 1 ? (size_t)cs * pix * 2 * kIbpConvCO : 0)) * sizeof(float);
+  ibp_conv_kernel<<<grid, block, smem, s>>>(W, bias, l_in, u_in, relu_in, l_out, u_out, c_in, h, w, c_out,
+                                            kh, kw, stride, pad, ho, wo);
 }
 
 // ---- a6: A_in = conv^T(A_out, W) (+ addend: the other incoming A of a residual fork).

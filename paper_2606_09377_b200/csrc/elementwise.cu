@@ -50,7 +50,12 @@ struct RelaxDev {
   const float* bias; int bias_div;
   float* out; float* out_lo; float* d;
   int B, R, n;
+  int wpp;      // warps per (b, r) pair: 1, 2, 4 or 8 (all in one block); a function of n ONLY, so that the summation
+                // order of d does not depend on how the rows are chunked (chunked == unchunked bitwise)
 };
+
+// long rows with few (b, r) pairs (cfg5: 792 pairs of 16384 neurons) leave most SMs idle with one warp per pair
+static inline int warps_per_pair(int n) { return n >= 4096 ? 8 : (n >= 2048 ? 4 : (n >= 1024 ? 2 : 1)); }
 
 __device__ __forceinline__ float clip01(float a) { return fminf(fmaxf(a, 0.f), 1.f); }
 
@@ -80,8 +85,13 @@ __device__ __forceinline__ void relax_elem(float aL, float aU, const float4& c, 
 template <bool RELU, bool ALPHA, bool SPLIT, int VEC>
 __global__ void __launch_bounds__(256) relax_kernel(RelaxDev p) {
   const int lane = threadIdx.x & 31;
-  const long long pair = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  if (pair >= (long long)p.B * p.R) return;
+  const int wpp = p.wpp;
+  const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const long long pair_raw = warp / wpp;
+  const int wi = (int)(warp % wpp);                       // this warp's slice of the row
+  const bool valid = pair_raw < (long long)p.B * p.R;
+  const long long pair = valid ? pair_raw : 0;
+  const int n_eff = valid ? p.n : 0;
   const int b = (int)(pair / p.R), r = (int)(pair % p.R);
   const float* a0 = p.A + (long long)b * p.sB + (long long)r * p.ld;
   const float* a1 = a0 + p.sBr;
@@ -97,7 +107,7 @@ __global__ void __launch_bounds__(256) relax_kernel(RelaxDev p) {
   float accL = 0.f, accU = 0.f;
 
   if (VEC == 4) {
-    for (int j = lane * 4; j < p.n; j += 128) {
+    for (int j = (wi * 32 + lane) * 4; j < n_eff; j += wpp * 128) {
       float4 xL = ldg_stream4(a0 + j);
       float4 xU = ldg_stream4(a1 + j);
       float4 c0 = make_float4(0, 0, 0, 0), c1 = c0, c2 = c0, c3 = c0;
@@ -132,7 +142,7 @@ __global__ void __launch_bounds__(256) relax_kernel(RelaxDev p) {
       }
     }
   } else {
-    for (int j = lane; j < p.n; j += 32) {
+    for (int j = wi * 32 + lane; j < n_eff; j += wpp * 32) {
       float xL = a0[j], xU = a1[j];
       float4 c = RELU ? cf[j] : make_float4(0, 0, 0, 0);
       float tL = ALPHA ? alL[j] : 0.f, tU = ALPHA ? alU[j] : 0.f;
@@ -148,9 +158,22 @@ __global__ void __launch_bounds__(256) relax_kernel(RelaxDev p) {
   }
   accL = warp_sum(accL);
   accU = warp_sum(accU);
-  if (lane == 0 && p.d) {
-    p.d[pair] += accL;
-    p.d[BR + pair] += accU;
+  if (wpp == 1) {
+    if (valid && lane == 0 && p.d) {
+      p.d[pair] += accL;
+      p.d[BR + pair] += accU;
+    }
+    return;
+  }
+  __shared__ float red[8][2];
+  const int w = threadIdx.x >> 5;
+  if (lane == 0) { red[w][0] = accL; red[w][1] = accU; }
+  __syncthreads();
+  if (valid && wi == 0 && lane == 0 && p.d) {             // slices added in slice order: deterministic
+    float sL = red[w][0], sU = red[w][1];
+    for (int k = 1; k < wpp; ++k) { sL += red[w + k][0]; sU += red[w + k][1]; }
+    p.d[pair] += sL;
+    p.d[BR + pair] += sU;
   }
 }
 
@@ -169,7 +192,8 @@ void launch_relax(const RelaxArgs& a, cudaStream_t s) {
   p.out = a.out; p.out_lo = a.out_lo; p.d = a.d; p.B = a.B; p.R = a.R; p.n = a.n;
   long long pairs = (long long)a.B * a.R;
   if (pairs <= 0 || a.n <= 0) return;
-  int blocks = ceil_div(pairs * 32, 256);
+  p.wpp = warps_per_pair(a.n);
+  int blocks = ceil_div(pairs * p.wpp * 32, 256);
   auto al16 = [](const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; };
   bool vec = (a.n % 4 == 0) && (p.ld % 4 == 0) && (p.sB % 4 == 0) && (p.sBr % 4 == 0) && al16(p.A) &&
              al16(p.out) && (!p.out_lo || al16(p.out_lo)) && (!p.alpha_lo || al16(p.alpha_lo)) &&
@@ -311,11 +335,15 @@ void launch_init_d(float* d, const float* bias, int row0, int B, int R, cudaStre
 __global__ void __launch_bounds__(256) rowdot_bias_kernel(const float* __restrict__ A, const float* __restrict__ Alo,
                                                           long long sBr, long long sB, long long ld, int n,
                                                           const float* __restrict__ bias, int bias_div,
-                                                          float* d, int B, int R) {
+                                                          float* d, int B, int R, int wpp) {
   const int lane = threadIdx.x & 31;
-  const long long m = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const long long m_raw = warp / wpp;
+  const int wi = (int)(warp % wpp);
   const long long BR = (long long)B * R;
-  if (m >= 2 * BR) return;
+  const bool valid = m_raw < 2 * BR;
+  const long long m = valid ? m_raw : 0;
+  if (!valid) n = 0;
   int br = (int)(m / BR);
   long long pair = m % BR;
   int b = (int)(pair / R), r = (int)(pair % R);
@@ -324,19 +352,29 @@ __global__ void __launch_bounds__(256) rowdot_bias_kernel(const float* __restric
   float acc = 0.f;
   if (Alo) {            // view carries a TF32 lo limb: the value is hi + lo
     const float* al = Alo + off;
-    for (int j = lane; j < n; j += 32) acc = fmaf(a[j] + al[j], bias[j / bias_div], acc);
+    for (int j = wi * 32 + lane; j < n; j += wpp * 32) acc = fmaf(a[j] + al[j], bias[j / bias_div], acc);
   } else {
-    for (int j = lane; j < n; j += 32) acc = fmaf(a[j], bias[j / bias_div], acc);
+    for (int j = wi * 32 + lane; j < n; j += wpp * 32) acc = fmaf(a[j], bias[j / bias_div], acc);
   }
   acc = warp_sum(acc);
-  if (lane == 0) d[m] += acc;
+  if (wpp == 1) { if (valid && lane == 0) d[m] += acc; return; }
+  __shared__ float red[8];
+  const int w = threadIdx.x >> 5;
+  if (lane == 0) red[w] = acc;
+  __syncthreads();
+  if (valid && wi == 0 && lane == 0) {
+    float sacc = red[w];
+    for (int k = 1; k < wpp; ++k) sacc += red[w + k];
+    d[m] += sacc;
+  }
 }
 void launch_rowdot_bias(const AView& A, const float* bias, int bias_div, float* d, int B, int R,
                         cudaStream_t s) {
   long long rows = 2LL * B * R;
   if (rows <= 0 || !bias) return;
-  rowdot_bias_kernel<<<ceil_div(rows * 32, 256), 256, 0, s>>>(A.p, A.lo, A.sBr, A.sB, A.ld, A.n, bias,
-                                                             bias_div > 0 ? bias_div : 1, d, B, R);
+  const int wpp = warps_per_pair(A.n);
+  rowdot_bias_kernel<<<ceil_div(rows * wpp * 32, 256), 256, 0, s>>>(A.p, A.lo, A.sBr, A.sB, A.ld, A.n, bias,
+                                                                   bias_div > 0 ? bias_div : 1, d, B, R, wpp);
 }
 
 // out[m, :] = a[m, :] (+ b[m, :]) for the 2*B*R rows of two strided views; blockIdx.y = row, threads walk the row
