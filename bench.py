@@ -60,6 +60,9 @@ def parse_args():
     ap.add_argument("--alpha-iters", type=int, default=10,
                     help="alpha-mode configs: also time this many projected ascent steps on alpha (NEXT-1; 0 = skip)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--device-steps-only", action="store_true",
+                    help="profiling aid (ncu): only the warm-up and the timed device steps of --workload; no TF32 peak "
+                         "measurement, end-to-end leg, per-class timing leg, alpha leg, CPU baseline or per_config")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     return ap.parse_args()
 
@@ -417,6 +420,12 @@ def measure_config(cfgname, args, steps, warmup, dev, local, world, tf32_peak, w
     verified = int(io["verified"].sum().item())
     # long steps: the end-to-end and the instrumented legs run fewer steps (they re-measure the same kernels)
     n_aux = steps if ms_step < 200.0 else max(2, min(steps, int(15000.0 / ms_step)))
+    if args.device_steps_only:
+        out = {"value": world * B / (ms_step * 1e-3), "unit": UNIT, "steps": steps, "ms_per_step": ms_step,
+               "config": workload_desc(wl, cfgname), "gpu_launches_per_step": int(launches_per_step), "clocks": clocks,
+               "aw_flops_per_step": flops_step}
+        ctx.close()
+        return out
     ms_e2e = timed(step_host, n_aux, 1 if ms_step >= 200.0 else max(warmup, 1), host_clock=True)
 
     # ---- per-kernel-class device times (CUDA events around every launch; graph replay is off for this leg) ----------
@@ -541,6 +550,13 @@ def run_b200(args):
     dev = torch.device("cuda", local)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
+    if args.device_steps_only:
+        r = measure_config(args.workload, args, args.steps, args.warmup, dev, local, world, None, False)
+        if rank == 0:
+            print(json.dumps(dict(r, metric=METRIC, n_gpus=world, warmup=args.warmup, mode="device-steps-only")))
+        if world > 1:
+            dist.destroy_process_group()
+        return
     tf32_peak = measure_tf32_peak(dev)
     with_cpu = rank == 0 and world == 1 and not args.no_cpu_baseline
     main = measure_config(args.workload, args, args.steps, args.warmup, dev, local, world, tf32_peak, with_cpu)

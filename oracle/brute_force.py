@@ -18,8 +18,11 @@ from scipy.optimize import linprog
 LINEAR, RELU = "linear", "relu"
 
 
-def exact_range(net, x_lo, x_hi, C: np.ndarray) -> Tuple[np.ndarray, np.ndarray]:
-    """Exact (min, max) [S] of C.f(x) over the box for a plain MLP (linear/relu chain)."""
+def exact_range(net, x_lo, x_hi, C: np.ndarray, split=None) -> Tuple[np.ndarray, np.ndarray]:
+    """Exact (min, max) [S] of C.f(x) over the box for a plain MLP (linear/relu chain).
+    split (optional): {relu node id: s in {-1,0,+1}^n}: the BaB sub-domain that fixes pre-activation j of that ReLU to
+    >= 0 (s = +1) or <= 0 (s = -1); only activation patterns that agree with it are enumerated.
+    Returns (+inf, -inf) for an empty sub-domain."""
     x_lo = np.asarray(x_lo, np.float64).reshape(-1)
     x_hi = np.asarray(x_hi, np.float64).reshape(-1)
     C = np.asarray(C, np.float64)
@@ -38,7 +41,19 @@ def exact_range(net, x_lo, x_hi, C: np.ndarray) -> Tuple[np.ndarray, np.ndarray]
     best_min = np.full(S, np.inf)
     best_max = np.full(S, -np.inf)
     bounds = list(zip(x_lo, x_hi))
+    fixed = np.zeros(n_relu, dtype=int)          # per enumerated neuron: 0 free, +1 must be active, -1 must be inactive
+    if split is not None:
+        off, k = 0, 0
+        for i, n in enumerate(net.nodes):
+            if n.op == RELU:
+                if split.get(i) is not None:
+                    fixed[off:off + hidden[k]] = np.sign(np.asarray(split[i]).reshape(-1)).astype(int)
+                off += hidden[k]
+                k += 1
     for pattern in itertools.product((0, 1), repeat=n_relu):
+        pat = np.array(pattern)
+        if np.any((fixed > 0) & (pat == 0)) or np.any((fixed < 0) & (pat == 1)):
+            continue
         # affine map of the current layer's post-activation: z = M x + v
         M = np.eye(n0)
         v = np.zeros(n0)
