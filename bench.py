@@ -59,6 +59,8 @@ def parse_args():
     ap.add_argument("--no-conv-tc", action="store_true", help="BoundConv backward on the CUDA-core kernel everywhere (debug)")
     ap.add_argument("--alpha-iters", type=int, default=10,
                     help="alpha-mode configs: also time this many projected ascent steps on alpha (NEXT-1; 0 = skip)")
+    ap.add_argument("--bab-domains", type=int, default=4096,
+                    help="cfg2: also time the joint alpha/beta ascent (NEXT-2) on this many BaB sub-domains (0 = skip)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--device-steps-only", action="store_true",
                     help="profiling aid (ncu): only the warm-up and the timed device steps of --workload; no TF32 peak "
@@ -510,6 +512,11 @@ def measure_config(cfgname, args, steps, warmup, dev, local, world, tf32_peak, w
                      "verified_before": verified, "verified_after": int(res["verified"].sum().item())}
         del res, al, au
 
+    # ---- NEXT-2: beta-CROWN bounds of batched BaB sub-domains, reported beside the step ------------
+    bab = None
+    if cfgname == "cfg2" and alpha is not None and args.bab_domains > 0 and args.scale == 1:
+        bab = measure_bab(wl, ctx, io, args, dev, local)
+
     peak_ws = ctx.peak_bytes()
     peak_torch = torch.cuda.max_memory_allocated(dev)
     rc_rows = ctx.row_chunk()
@@ -528,12 +535,64 @@ def measure_config(cfgname, args, steps, warmup, dev, local, world, tf32_peak, w
         "e2e": {"value": world * B / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                 "d2h_bytes_per_step": int(d2h), "ms_per_step": ms_e2e, "steps": n_aux},
         "gpu_launches": int(launches_per_step * steps), "gpu_launches_per_step": int(launches_per_step), "clocks": clocks,
-        "alpha_opt": alpha_opt}
+        "alpha_opt": alpha_opt, "bab_beta": bab}
     ctx.close()
     del ctx, xlo, xhi, Cd, alpha, io, flush, wl
     gc.collect()
     torch.cuda.empty_cache()
     torch.cuda.reset_peak_memory_stats(dev)
+    return out
+
+
+def measure_bab(wl, ctx0, io0, args, dev, local):
+    """NEXT-2 leg: D sub-domains of the workload's properties (round robin), each the parent's box and intermediate bounds
+    (from the step just run, io0) plus `depth` random split decisions on unstable neurons (seeded); one call of
+    crown_beta_ascent = T + 1 bound evaluations and T joint projected steps on (alpha, beta) for all sub-domains."""
+    import torch
+    from paper_2606_09377_b200 import CrownContext
+    D, T, depth = args.bab_domains, 10, 8
+    S = wl.S
+    ctx = CrownContext(wl.net, D, S, device=f"cuda:{local}", mem_cap_bytes=8 << 30)
+    g = torch.Generator(device=dev); g.manual_seed(W.SEED_BASE + 777)
+    idx = torch.arange(D, device=dev) % wl.B
+    lo, hi = wl.box()
+    xlo = torch.from_numpy(lo).to(dev)[idx].contiguous(); xhi = torch.from_numpy(hi).to(dev)[idx].contiguous()
+    Cd = torch.from_numpy(np.ascontiguousarray(wl.C)).to(dev)[idx].contiguous()
+    l = {i: io0["l"][i][idx].contiguous() for i in ctx.relu_ids}
+    u = {i: io0["u"][i][idx].contiguous() for i in ctx.relu_ids}
+    split = {}
+    for i in ctx.relu_ids:        # `depth` splits per sub-domain spread over the layers, on unstable neurons only
+        n = ctx.sizes[i]
+        pick = torch.rand(D, n, device=dev, generator=g) < (depth / (len(ctx.relu_ids) * n))
+        sign = torch.where(torch.rand(D, n, device=dev, generator=g) < 0.5, 1, -1).to(torch.int8)
+        split[i] = torch.where(pick & (l[i] < 0) & (u[i] > 0), sign, torch.zeros_like(sign)).contiguous()
+    n_split = float(sum(int((s != 0).sum().item()) for s in split.values())) / D
+    mk = lambda v: {i: torch.full((D, S, ctx.sizes[i]), v, device=dev) for i in ctx.relu_ids}
+    res = {k: torch.empty(D, S, device=dev) for k in ("lb_best", "ub_best", "lb_last", "ub_last")}
+    res["verified"] = torch.empty(D, dtype=torch.uint8, device=dev)
+    ms = []
+    lb0 = None
+    for it in range(3):
+        al, au, bl, bu = mk(0.5), mk(0.5), mk(0.0), mk(0.0)
+        if lb0 is None:       # bounds at the start point (0 iterations)
+            ctx.beta_ascent_device(l, u, split, Cd, al, au, bl, bu, xlo, xhi, 0.05, 0.05, 0.98, 0, 1, res)
+            torch.cuda.synchronize()
+            lb0 = res["lb_best"].clone()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        ctx.beta_ascent_device(l, u, split, Cd, al, au, bl, bu, xlo, xhi, 0.05, 0.05, 0.98, T, 1, res)
+        e1.record(); e1.synchronize()
+        ms.append(e0.elapsed_time(e1))
+    gain = res["lb_best"] - lb0
+    out = {"domains": D, "iters": T, "splits_per_domain": n_split, "rule": "sign step, eta_alpha = eta_beta = 0.05, decay 0.98",
+           "ms_total": min(ms), "ms_per_iter": min(ms) / (T + 1), "domains_per_s": D / (min(ms) * 1e-3),
+           "bound_evaluations_per_s": D * (T + 1) / (min(ms) * 1e-3), "mean_lb_gain": float(gain.mean().item()),
+           "mean_abs_lb_start": float(lb0.abs().mean().item()), "rows_tightened_frac": float((gain > 0).float().mean().item()),
+           "verified_domains": int(res["verified"].sum().item()), "workspace_gb": ctx.peak_bytes() / 1e9}
+    ctx.close()
+    del ctx, al, au, bl, bu, res, split, l, u
+    torch.cuda.empty_cache()
     return out
 
 
@@ -570,13 +629,13 @@ def run_b200(args):
             r = measure_config(c, args, st, 3, dev, local, world, tf32_peak, with_cpu)
             per[c] = {k: r[k] for k in ("value", "unit", "steps", "ms_per_step", "config", "verified_last_batch", "aw_tflops",
                                         "peak_hbm_gb", "kernel_time_shares", "kernel_classes", "roofline", "cpu_baseline",
-                                        "e2e", "gpu_launches_per_step", "clocks", "alpha_opt")}
+                                        "e2e", "gpu_launches_per_step", "clocks", "alpha_opt", "bab_beta")}
     if rank == 0:
         line = {"metric": METRIC, "value": main["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": main["ms_per_step"], "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32 (3xTF32 products, fp32 accumulate)", "data": "synthetic"}
         for k in ("config", "verified_last_batch", "aw_tflops", "aw_flops_per_step", "peak_hbm_gb", "kernel_time_shares",
-                  "kernel_classes", "roofline", "cpu_baseline", "e2e", "gpu_launches", "gpu_launches_per_step", "clocks", "alpha_opt"):
+                  "kernel_classes", "roofline", "cpu_baseline", "e2e", "gpu_launches", "gpu_launches_per_step", "clocks", "alpha_opt", "bab_beta"):
             line[k] = main[k]
         line["tf32_dense_peak_tflops"] = tf32_peak
         line["per_config"] = per

@@ -210,6 +210,51 @@ int crown_alpha_ascent(crown_ctx* ctx, int B, const float* C_dev, int S,
                        float* lb_best_dev, float* ub_best_dev, float* lb_last_dev, float* ub_last_dev,
                        uint8_t* verified_dev, void* scratch_dev, size_t scratch_bytes);
 
+/* NEXT-2 -- beta-CROWN bounds of batched branch-and-bound sub-domains (sec. 2.1.1: BaB fixes "a ReLU state
+ * x >= 0 or x < 0" and bounds are recomputed per sub-region; sec. 2.2: the split constraints enter the
+ * bound-propagation pass "via Lagrangian dual variables beta ... bounds for thousands of sub-problems are evaluated in
+ * parallel on GPU as batched matrix multiplications, and alpha/beta parameters are jointly optimised by gradient
+ * descent"; PAPER.md:96 batch BaB).  A sub-domain is one entry of the batch: its box, its (parent's) intermediate bounds
+ * l_dev/u_dev and, per ReLU i, split_dev[i] (array of n_nodes pointers; entry = int8 [B, size_i], 4-byte aligned, or NULL):
+ * +1 fixes the pre-activation z >= 0, -1 fixes z <= 0, 0 = not split.  Readings G26-G28:
+ *   - the interval of a split neuron is clamped inside the library (l <- max(l,0) resp. u <- min(u,0)); l_dev/u_dev are
+ *     not modified;
+ *   - right after the relaxation of ReLU i (A w.r.t. its pre-activation):  lower branch A -= max(beta_lo_i, 0) * s_i,
+ *     upper branch A += max(beta_up_i, 0) * s_i  with beta [B, rows, size_i]; sound for every beta >= 0 (weak duality);
+ *     beta arrays / entries may be NULL (= 0); values on unsplit neurons are ignored.
+ * crown_backward_split: crown_backward with these two additions (same outputs, same errors). */
+int crown_backward_split(crown_ctx* ctx, int B, int start, int row0, int rows, const float* C_dev,
+                         const float* const* l_dev, const float* const* u_dev, const int8_t* const* split_dev,
+                         const float* const* alpha_lo_dev, const float* const* alpha_up_dev,
+                         const float* const* beta_lo_dev, const float* const* beta_up_dev,
+                         float* A_dev, float* d_dev,
+                         const float* x_lo_dev, const float* x_hi_dev, float* lb_dev, float* ub_dev);
+
+/* crown_alpha_grad for a batch of sub-domains: additionally gb_lo_dev[i] = d lb / d beta_lo[i] = -s_i * z_i(x*) and
+ * gb_up_dev[i] = d ub / d beta_up[i] = +s_i * z_i(x*)  ([B,S,size_i]; z_i(x*) = the pre-activation at the bound-attaining
+ * corner through the selected lines, i.e. the forward sweep of crown_alpha_grad); zero on unsplit neurons.  Written only
+ * for ReLUs with a split entry.  Scratch as for crown_alpha_grad. */
+int crown_beta_grad(crown_ctx* ctx, int B, const float* C_dev, int S,
+                    const float* const* l_dev, const float* const* u_dev, const int8_t* const* split_dev,
+                    const float* const* alpha_lo_dev, const float* const* alpha_up_dev,
+                    const float* const* beta_lo_dev, const float* const* beta_up_dev,
+                    const float* x_lo_dev, const float* x_hi_dev,
+                    float* const* g_lo_dev, float* const* g_up_dev, float* const* gb_lo_dev, float* const* gb_up_dev,
+                    float* lb_dev, float* ub_dev, void* scratch_dev, size_t scratch_bytes);
+
+/* Joint projected ascent on (alpha, beta), in place (reading G28): alpha as in crown_alpha_ascent with step eta_alpha;
+ *   beta_lo <- max(max(beta_lo,0) + eta_beta * dir(gb_lo), 0),  beta_up <- max(max(beta_up,0) - eta_beta * dir(gb_up), 0);
+ * both steps decay by `decay` per iteration.  Every iterate is sound; outputs as crown_alpha_ascent (best over iterates).
+ * Every ReLU with a split entry needs DISTINCT beta_lo / beta_up tensors (CROWN_EINVAL otherwise). */
+int crown_beta_ascent(crown_ctx* ctx, int B, const float* C_dev, int S,
+                      const float* const* l_dev, const float* const* u_dev, const int8_t* const* split_dev,
+                      float* const* alpha_lo_dev, float* const* alpha_up_dev,
+                      float* const* beta_lo_dev, float* const* beta_up_dev,
+                      const float* x_lo_dev, const float* x_hi_dev,
+                      float eta_alpha, float eta_beta, float decay, int iters, int mode,
+                      float* lb_best_dev, float* ub_best_dev, float* lb_last_dev, float* ub_last_dev,
+                      uint8_t* verified_dev, void* scratch_dev, size_t scratch_bytes);
+
 /* D[M,N] = A[M,K] . W[K,N] (row-major fp32) through the same contraction kernel the backward
  * pass uses (scheme: 0 = 3xTF32 tcgen05 on prepared limbs, 2 = FFMA; 1 -- reserved in SURVEY.md for a split-bf16
  * scheme -- is intentionally absent); exposed for parity tests and roofline

@@ -19,7 +19,7 @@ OP_CODES = {"linear": 1, "conv": 2, "relu": 3, "add": 4, "flatten": 5}
 K_CLASSES = ["ibp", "coeff", "relax", "gemm_tc", "gemm_ffma", "concretize", "conv", "misc"]
 
 EXPORTS = ["crown_h2d_bytes", "crown_workspace_bytes", "crown_init", "ibp_forward", "crown_backward", "concretize", "crown_run",
-           "crown_run_host", "crown_alpha_scratch_bytes", "crown_alpha_grad", "crown_alpha_ascent", "crown_gemm", "crown_split_tf32", "crown_peak_bytes", "crown_row_chunk", "crown_launch_count", "crown_graph_replays",
+           "crown_run_host", "crown_alpha_scratch_bytes", "crown_alpha_grad", "crown_alpha_ascent", "crown_backward_split", "crown_beta_grad", "crown_beta_ascent", "crown_gemm", "crown_split_tf32", "crown_peak_bytes", "crown_row_chunk", "crown_launch_count", "crown_graph_replays",
            "crown_gemm_flops", "crown_timing", "crown_timing_read", "crown_last_error", "crown_destroy",
            "crown_version"]
 
@@ -75,6 +75,11 @@ def load_library() -> C.CDLL:
                                      C.POINTER(vp), C.POINTER(vp), vp, vp, vp, C.c_size_t]
     lib.crown_alpha_ascent.argtypes = [vp, i32, vp, i32, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), vp, vp,
                                        C.c_float, C.c_float, i32, i32, vp, vp, vp, vp, vp, vp, C.c_size_t]
+    pp = C.POINTER(vp)
+    lib.crown_backward_split.argtypes = [vp, i32, i32, i32, i32, vp, pp, pp, pp, pp, pp, pp, pp, vp, vp, vp, vp, vp, vp]
+    lib.crown_beta_grad.argtypes = [vp, i32, vp, i32, pp, pp, pp, pp, pp, pp, pp, vp, vp, pp, pp, pp, pp, vp, vp, vp, C.c_size_t]
+    lib.crown_beta_ascent.argtypes = [vp, i32, vp, i32, pp, pp, pp, pp, pp, pp, pp, vp, vp, C.c_float, C.c_float, C.c_float,
+                                      i32, i32, vp, vp, vp, vp, vp, vp, C.c_size_t]
     lib.crown_gemm.argtypes = [vp, i32, i32, i32, i32, vp, vp, vp, vp, vp]
     lib.crown_split_tf32.argtypes = [vp, vp, i32, i32, i32, vp, vp]
     lib.crown_peak_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
@@ -348,6 +353,89 @@ class CrownContext:
         self.alpha_ascent_device(l, u, Cmat, al, au, x_lo, x_hi, eta, decay, iters, {"plain": 0, "sign": 1}[mode], out)
         self.stream.synchronize()
         out["alpha_lo"], out["alpha_up"] = al, au
+        return out
+
+    # ---- NEXT-2: beta-CROWN bounds of BaB sub-domains -------------------------------------
+    def _split_dev(self, split):
+        return None if split is None else {i: self._dev(v, torch.int8) for i, v in split.items()}
+
+    def backward_split(self, B: int, start: int, pre: Dict[int, tuple], split, Cmat=None, row0: int = 0,
+                       rows: Optional[int] = None, alpha_lo=None, alpha_up=None, beta_lo=None, beta_up=None, box=None,
+                       want_A: bool = True):
+        """crown_backward_split: O3 for a batch of sub-domains.  split {relu id: int8 [B, n]}; beta {relu id: [B,R,n]}."""
+        if Cmat is not None:
+            Cmat = self._dev(Cmat)
+            rows = Cmat.shape[1]
+        l = {i: self._dev(v[0]) for i, v in pre.items()}
+        u = {i: self._dev(v[1]) for i, v in pre.items()}
+        dev = lambda d: None if d is None else {i: self._dev(v) for i, v in d.items()}
+        al, au, bl, bu, sp = dev(alpha_lo), dev(alpha_up), dev(beta_lo), dev(beta_up), self._split_dev(split)
+        A = torch.empty(2, B, rows, self.n0, device=self.device) if want_A else None
+        d = torch.empty(2, B, rows, device=self.device)
+        x_lo = x_hi = lb = ub = None
+        if box is not None:
+            x_lo, x_hi = self._dev(box[0]), self._dev(box[1])
+            lb = torch.empty(B, rows, device=self.device)
+            ub = torch.empty(B, rows, device=self.device)
+        arr = lambda d_: self._ptr_array(d_) if d_ else None
+        self._check(self.lib.crown_backward_split(self.h, B, start, row0, rows, _ptr(Cmat), self._ptr_array(l),
+                                                  self._ptr_array(u), arr(sp), arr(al), arr(au), arr(bl), arr(bu),
+                                                  _ptr(A), _ptr(d), _ptr(x_lo), _ptr(x_hi), _ptr(lb), _ptr(ub)), self.h)
+        self.stream.synchronize()
+        return {"A": A, "d": d, "lb": lb, "ub": ub}
+
+    def beta_grad(self, pre, split, Cmat, alpha_lo, alpha_up, beta_lo, beta_up, box):
+        """crown_beta_grad: bounds and their derivatives w.r.t. alpha and beta for a batch of sub-domains."""
+        Cmat = self._dev(Cmat)
+        B, S = Cmat.shape[0], Cmat.shape[1]
+        l = {i: self._dev(v[0]) for i, v in pre.items()}
+        u = {i: self._dev(v[1]) for i, v in pre.items()}
+        dev = lambda d: {i: self._dev(v) for i, v in d.items()}
+        al, au, bl, bu, sp = dev(alpha_lo), dev(alpha_up), dev(beta_lo), dev(beta_up), self._split_dev(split)
+        x_lo, x_hi = self._dev(box[0]), self._dev(box[1])
+        mk = lambda: {i: torch.zeros(B, S, self.sizes[i], device=self.device) for i in self.relu_ids}
+        g_lo, g_up, gb_lo, gb_up = mk(), mk(), mk(), mk()
+        lb = torch.empty(B, S, device=self.device)
+        ub = torch.empty(B, S, device=self.device)
+        scr = self._alpha_scratch(B, S)
+        self._check(self.lib.crown_beta_grad(self.h, B, Cmat.data_ptr(), S, self._ptr_array(l), self._ptr_array(u),
+                                             self._ptr_array(sp), self._ptr_array(al), self._ptr_array(au),
+                                             self._ptr_array(bl), self._ptr_array(bu), x_lo.data_ptr(), x_hi.data_ptr(),
+                                             self._ptr_array(g_lo), self._ptr_array(g_up), self._ptr_array(gb_lo),
+                                             self._ptr_array(gb_up), lb.data_ptr(), ub.data_ptr(), scr.data_ptr(),
+                                             scr.numel()), self.h)
+        self.stream.synchronize()
+        return {"lb": lb, "ub": ub, "g_lo": g_lo, "g_up": g_up, "gb_lo": gb_lo, "gb_up": gb_up}
+
+    def beta_ascent_device(self, l, u, split, Cmat, alpha_lo, alpha_up, beta_lo, beta_up, x_lo, x_hi, eta_alpha, eta_beta,
+                           decay, iters, mode, out) -> None:
+        """crown_beta_ascent on device tensors (asynchronous); alpha / beta are updated in place."""
+        B, S = Cmat.shape[0], Cmat.shape[1]
+        scr = self._alpha_scratch(B, S)
+        self._check(self.lib.crown_beta_ascent(self.h, B, Cmat.data_ptr(), S, self._ptr_array(l), self._ptr_array(u),
+                                               self._ptr_array(split), self._ptr_array(alpha_lo), self._ptr_array(alpha_up),
+                                               self._ptr_array(beta_lo), self._ptr_array(beta_up), x_lo.data_ptr(),
+                                               x_hi.data_ptr(), float(eta_alpha), float(eta_beta), float(decay), int(iters),
+                                               int(mode), out["lb_best"].data_ptr(), out["ub_best"].data_ptr(),
+                                               out["lb_last"].data_ptr(), out["ub_last"].data_ptr(),
+                                               out["verified"].data_ptr(), scr.data_ptr(), scr.numel()), self.h)
+
+    def beta_ascent(self, pre, split, Cmat, alpha_lo, alpha_up, beta_lo, beta_up, box, eta_alpha: float, eta_beta: float,
+                    iters: int, mode: str = "sign", decay: float = 1.0):
+        """Joint projected ascent on (alpha, beta) for a batch of sub-domains; returns optimised copies and bounds."""
+        Cmat = self._dev(Cmat)
+        B, S = Cmat.shape[0], Cmat.shape[1]
+        l = {i: self._dev(v[0]) for i, v in pre.items()}
+        u = {i: self._dev(v[1]) for i, v in pre.items()}
+        cl = lambda d: {i: self._dev(v).clone() for i, v in d.items()}
+        al, au, bl, bu, sp = cl(alpha_lo), cl(alpha_up), cl(beta_lo), cl(beta_up), self._split_dev(split)
+        x_lo, x_hi = self._dev(box[0]), self._dev(box[1])
+        out = {k: torch.empty(B, S, device=self.device) for k in ("lb_best", "ub_best", "lb_last", "ub_last")}
+        out["verified"] = torch.empty(B, dtype=torch.uint8, device=self.device)
+        self.beta_ascent_device(l, u, sp, Cmat, al, au, bl, bu, x_lo, x_hi, eta_alpha, eta_beta, decay, iters,
+                                {"plain": 0, "sign": 1}[mode], out)
+        self.stream.synchronize()
+        out.update(alpha_lo=al, alpha_up=au, beta_lo=bl, beta_up=bu)
         return out
 
     # ---- kernel 1 on its own ---------------------------------------------------------------------

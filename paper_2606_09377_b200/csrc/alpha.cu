@@ -189,7 +189,9 @@ __device__ __forceinline__ float sgnf(float a) { return a > 0.f ? 1.f : (a < 0.f
 __global__ void __launch_bounds__(256)
 alpha_relu_kernel(const float* __restrict__ A, const float* __restrict__ Gin, const float4* __restrict__ coef,
                   float* alpha_lo, float* alpha_up, float* __restrict__ Gout, float* __restrict__ g_lo,
-                  float* __restrict__ g_up, const float* __restrict__ step, int mode, int B, int S, int n) {
+                  float* __restrict__ g_up, const float* __restrict__ step, int mode, int B, int S, int n,
+                  const int8_t* __restrict__ split, float* beta_lo, float* beta_up, float* __restrict__ gb_lo,
+                  float* __restrict__ gb_up) {
   const long long per_br = (long long)B * S * n;
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= per_br) return;
@@ -213,15 +215,29 @@ alpha_relu_kernel(const float* __restrict__ A, const float* __restrict__ Gin, co
     if (g_lo) g_lo[i] = dl;
     if (g_up) g_up[i] = du;
   }
+  if (split) {
+    // NEXT-2 (reading G28): the split term -beta_lo * s (lower) / +beta_up * s (upper) is added to A w.r.t. this ReLU's
+    // INPUT, whose derivative is Gin: d lb / d beta_lo = -s * Gin, d ub / d beta_up = +s * Gin
+    const float sg = (float)split[(long long)b * n + j];
+    const float bl = -sg * gL, bu = sg * gU;
+    if (step) {
+      const float eb = step[1];
+      if (beta_lo) beta_lo[i] = fmaxf(fmaxf(beta_lo[i], 0.f) + eb * (mode ? sgnf(bl) : bl), 0.f);    // ascent on lb
+      if (beta_up) beta_up[i] = fmaxf(fmaxf(beta_up[i], 0.f) - eb * (mode ? sgnf(bu) : bu), 0.f);    // descent on ub
+    } else {
+      if (gb_lo) gb_lo[i] = bl;
+      if (gb_up) gb_up[i] = bu;
+    }
+  }
 }
 
 void launch_alpha_relu(const float* A, const float* Gin, const float4* coef, float* alpha_lo, float* alpha_up,
                        float* Gout, float* g_lo, float* g_up, const float* step, int mode, int B, int S, int n,
-                       cudaStream_t s) {
+                       cudaStream_t s, const int8_t* split, float* beta_lo, float* beta_up, float* gb_lo, float* gb_up) {
   const long long cnt = (long long)B * S * n;
   if (cnt <= 0) return;
   alpha_relu_kernel<<<ceil_div(cnt, 256), 256, 0, s>>>(A, Gin, coef, alpha_lo, alpha_up, Gout, g_lo, g_up, step, mode,
-                                                      B, S, n);
+                                                      B, S, n, split, beta_lo, beta_up, gb_lo, gb_up);
 }
 
 // ---- best-so-far bounds over the iterates (every iterate is sound): lb_best = max, ub_best = min; the step size
@@ -236,7 +252,7 @@ alpha_best_kernel(const float* __restrict__ lb, const float* __restrict__ ub, fl
     lb_best[i] = first ? l : ((l > lb_best[i] || l != l) ? l : lb_best[i]);
     ub_best[i] = first ? u : ((u < ub_best[i] || u != u) ? u : ub_best[i]);
   }
-  if (i == 0 && step && !first) step[0] *= decay;
+  if (i == 0 && step && !first) { step[0] *= decay; step[1] *= decay; }
 }
 
 void launch_alpha_best(const float* lb, const float* ub, float* lb_best, float* ub_best, float* step, float decay,
@@ -245,7 +261,7 @@ void launch_alpha_best(const float* lb, const float* ub, float* lb_best, float* 
   alpha_best_kernel<<<ceil_div(count, 256), 256, 0, s>>>(lb, ub, lb_best, ub_best, step, decay, first, count);
 }
 
-__global__ void alpha_set_step_kernel(float* step, float v) { step[0] = v; }
-void launch_alpha_set_step(float* step, float v, cudaStream_t s) { alpha_set_step_kernel<<<1, 1, 0, s>>>(step, v); }
+__global__ void alpha_set_step_kernel(float* step, float v, float vb) { step[0] = v; step[1] = vb; }
+void launch_alpha_set_step(float* step, float v, cudaStream_t s, float v_beta) { alpha_set_step_kernel<<<1, 1, 0, s>>>(step, v, v_beta); }
 
 }  // namespace crownb200

@@ -5,6 +5,14 @@
 
 namespace {
 
+// NEXT-2: split constraints of a BaB sub-domain and their Lagrange multipliers (arrays of n_nodes pointers, entries for
+// ReLU nodes; nullptr arrays / entries = no split / beta = 0)
+struct SplitSpec {
+  const int8_t* const* split = nullptr;     // [B, size_i] in {-1, 0, +1}
+  const float* const* beta_lo = nullptr;    // [B, R, size_i]
+  const float* const* beta_up = nullptr;
+};
+
 struct Pass {
   crown_ctx* ctx;
   int B, R;
@@ -103,7 +111,8 @@ int tc_contract(crown_ctx* ctx, const NodeInfo& ni, const float* hi, const float
 int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_dev,
              const float* const* l_dev, const float* const* u_dev, const float* const* alpha_lo,
              const float* const* alpha_up, float* A_dev, float* d_dev, const float* x_lo, const float* x_hi,
-             float* lb, float* ub, int out_stride, std::vector<char>* coef_ready, float* const* A_save = nullptr) {
+             float* lb, float* ub, int out_stride, std::vector<char>* coef_ready, float* const* A_save = nullptr,
+             const SplitSpec* sp = nullptr) {
   const int n = (int)ctx->nodes.size();
   cudaStream_t s = ctx->stream;
   if (B <= 0 || B > ctx->B_max || R <= 0 || R > ctx->plan.rows_cap || start < 0 || start >= n)
@@ -118,7 +127,8 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
     if (!l_dev || !u_dev || !l_dev[i] || !u_dev[i]) return fail(ctx, CROWN_EINVAL, "crown_backward: bounds of a ReLU below start are missing");
     if (!coef_ready || !(*coef_ready)[i]) {
       Scope sc(ctx, CROWN_K_COEFF, 24.0 * B * ctx->nodes[i].size);
-      launch_relax_coeffs(l_dev[i], u_dev[i], coef_ptr(ctx, i), (long long)B * ctx->nodes[i].size, ctx->opts.slope_rule, s);
+      launch_relax_coeffs(l_dev[i], u_dev[i], coef_ptr(ctx, i), (long long)B * ctx->nodes[i].size, ctx->opts.slope_rule, s,
+                          (sp && sp->split) ? sp->split[i] : nullptr);
       if (coef_ready) (*coef_ready)[i] = 1;
     }
     return CROWN_OK;
@@ -173,6 +183,11 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
         ra.bias = lin_below ? ctx->nodes[j].n.b_dev : nullptr;
         ra.bias_div = (lin_below && ctx->nodes[j].n.op == CROWN_CONV2D) ? ctx->nodes[j].h * ctx->nodes[j].w : 1;
         ra.d = ctx->d_buf; ra.B = B; ra.R = R; ra.n = ni.size;
+        if (sp && sp->split && sp->split[i]) {
+          ra.split = sp->split[i];
+          ra.beta_lo = sp->beta_lo ? sp->beta_lo[i] : nullptr;
+          ra.beta_up = sp->beta_up ? sp->beta_up[i] : nullptr;
+        }
         Pending out;
         out.buf = new_buf(ps, ra.out);
         if (out.buf < 0) return fail(ctx, CROWN_ENOMEM, "backward: A-buffer pool exhausted");
@@ -183,7 +198,8 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
         const double in_rows = (double)(cur.v.sBr ? 2 : 1) * (cur.v.sB ? B : 1) * R;
         const double out_rows = 2.0 * B * R;
         { Scope sc(ctx, CROWN_K_RELAX, 4.0 * ni.size * (in_rows + out_rows * (tc ? 2.0 : 1.0)) +
-                                       ((ra.alpha_lo || ra.alpha_up) ? 4.0 * B * R * ni.size : 0.0));
+                                       ((ra.alpha_lo || ra.alpha_up) ? 4.0 * B * R * ni.size : 0.0) +
+                                       ((ra.beta_lo ? 4.0 : 0.0) + (ra.beta_up && ra.beta_up != ra.beta_lo ? 4.0 : 0.0)) * B * R * ni.size);
           launch_relax(ra, s); }
         out.v = canon_view(ra.out, B, R, ni.size); out.v.lo = ra.out_lo;
         out.bias_done_for = lin_below ? j : -2;
@@ -220,7 +236,8 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
           bool fr = false;
           if (!fc && r >= 0 && ctx->nodes[r].n.op == CROWN_RELU && ctx->nodes[r].n_consumers == 1 &&
               ps.pend.find(r) == ps.pend.end() && !ctx->opts.disable_epi_fusion && single && (R % 32) == 0 &&
-              !(alpha_lo && alpha_lo[r]) && !(alpha_up && alpha_up[r]) && (size_t)M_full * parts * 4 <= ctx->plan.part_bytes) {
+              !(alpha_lo && alpha_lo[r]) && !(alpha_up && alpha_up[r]) && !(sp && sp->split && sp->split[r]) &&
+              (size_t)M_full * parts * 4 <= ctx->plan.part_bytes) {
             j = ctx->nodes[r].n.in0;
             fr = j >= 0 && ctx->nodes[j].n.op == CROWN_LINEAR && ctx->nodes[j].tc_ok &&
                  (ctx->nodes[j].streamed || gemm_tc_supported(M_full, ctx->nodes[j].n.n_in, ctx->nodes[j].n.n_out));
@@ -593,7 +610,7 @@ void alpha_layout(crown_ctx* ctx, int B, int S, uint8_t* base, AlphaScratch& sc)
     else sc.G[i] = take(rows * ni.size);
   }
   sc.lb = take((size_t)B * S); sc.ub = take((size_t)B * S);
-  sc.step = take(1);
+  sc.step = take(2);                 // {alpha step, beta step}
   sc.bytes = off;
 }
 
@@ -620,15 +637,22 @@ int alpha_check(crown_ctx* ctx, int B, int S, const float* C_dev, const float* c
 // final pass at the current alpha (keeping A at every ReLU and at the input), bounds into sc.lb / sc.ub
 int alpha_backward(crown_ctx* ctx, int B, int S, const float* C_dev, const float* const* l_dev, const float* const* u_dev,
                    const float* const* alpha_lo, const float* const* alpha_up, const float* x_lo, const float* x_hi,
-                   const AlphaScratch& sc, std::vector<char>* coef_ready) {
+                   const AlphaScratch& sc, std::vector<char>* coef_ready, const SplitSpec* sp = nullptr) {
   return run_pass(ctx, B, (int)ctx->nodes.size() - 1, 0, S, C_dev, l_dev, u_dev, alpha_lo, alpha_up, sc.A0, nullptr, x_lo, x_hi,
-                  sc.lb, sc.ub, S, coef_ready, sc.Asave.data());
+                  sc.lb, sc.ub, S, coef_ready, sc.Asave.data(), sp);
 }
+
+// what the forward sweep does with beta (NEXT-2): gradients out, or the projected step in place (with `step`)
+struct BetaSweep {
+  const int8_t* const* split = nullptr;
+  float* const* beta_lo = nullptr; float* const* beta_up = nullptr;
+  float* const* gb_lo = nullptr; float* const* gb_up = nullptr;
+};
 
 // forward sweep of G; step == nullptr: gradients into g_lo / g_up, else the projected step on alpha in place
 int alpha_forward(crown_ctx* ctx, int B, int S, const AlphaScratch& sc, const float* x_lo, const float* x_hi,
                   float* const* alpha_lo, float* const* alpha_up, float* const* g_lo, float* const* g_up,
-                  const float* step, int mode) {
+                  const float* step, int mode, const BetaSweep* bs = nullptr) {
   cudaStream_t s = ctx->stream;
   const long long M = 2LL * B * S;
   { Scope scp(ctx, CROWN_K_MISC, 4.0 * M * ctx->n0 * 2); launch_alpha_corner(sc.A0, x_lo, x_hi, sc.Gin, B, S, ctx->n0, s); }
@@ -656,9 +680,13 @@ int alpha_forward(crown_ctx* ctx, int B, int S, const AlphaScratch& sc, const fl
       case CROWN_FLATTEN:
         break;                                  // aliases its producer
       case CROWN_RELU: {
-        Scope scp(ctx, CROWN_K_RELAX, 4.0 * ni.size * (3.0 * M + 2.0 * B * S));
+        const bool sp = bs && bs->split && bs->split[i];
+        Scope scp(ctx, CROWN_K_RELAX, 4.0 * ni.size * (3.0 * M + 2.0 * B * S + (sp ? 2.0 * B * S : 0.0)));
         launch_alpha_relu(sc.Asave[i], gin, coef_ptr(ctx, i), alpha_lo[i], alpha_up[i], sc.G[i],
-                          g_lo ? g_lo[i] : nullptr, g_up ? g_up[i] : nullptr, step, mode, B, S, ni.size, s);
+                          g_lo ? g_lo[i] : nullptr, g_up ? g_up[i] : nullptr, step, mode, B, S, ni.size, s,
+                          sp ? bs->split[i] : nullptr, sp && bs->beta_lo ? bs->beta_lo[i] : nullptr,
+                          sp && bs->beta_up ? bs->beta_up[i] : nullptr, sp && bs->gb_lo ? bs->gb_lo[i] : nullptr,
+                          sp && bs->gb_up ? bs->gb_up[i] : nullptr);
         break; }
       default:
         return fail(ctx, CROWN_EUNSUPPORTED, "crown_alpha: unsupported op");
@@ -678,23 +706,78 @@ extern "C" int crown_alpha_scratch_bytes(crown_ctx* ctx, int B, int S, size_t* o
   return CROWN_OK;
 }
 
+static int beta_grad_impl(crown_ctx* ctx, int B, const float* C_dev, int S, const float* const* l_dev,
+                          const float* const* u_dev, const int8_t* const* split_dev, const float* const* alpha_lo_dev,
+                          const float* const* alpha_up_dev, const float* const* beta_lo_dev, const float* const* beta_up_dev,
+                          const float* x_lo_dev, const float* x_hi_dev, float* const* g_lo_dev, float* const* g_up_dev,
+                          float* const* gb_lo_dev, float* const* gb_up_dev, float* lb_dev, float* ub_dev,
+                          void* scratch_dev, size_t scratch_bytes) {
+  AlphaScratch sc;
+  int rc = alpha_check(ctx, B, S, C_dev, l_dev, u_dev, alpha_lo_dev, alpha_up_dev, x_lo_dev, x_hi_dev, scratch_dev,
+                       scratch_bytes, false, sc);
+  if (rc) return rc;
+  CK(ctx, cudaMemsetAsync(scratch_dev, 0, sc.bytes, ctx->stream));
+  SplitSpec sp; sp.split = split_dev; sp.beta_lo = beta_lo_dev; sp.beta_up = beta_up_dev;
+  rc = alpha_backward(ctx, B, S, C_dev, l_dev, u_dev, alpha_lo_dev, alpha_up_dev, x_lo_dev, x_hi_dev, sc, nullptr,
+                      split_dev ? &sp : nullptr);
+  if (rc) return rc;
+  if (lb_dev) CK(ctx, cudaMemcpyAsync(lb_dev, sc.lb, (size_t)B * S * 4, cudaMemcpyDeviceToDevice, ctx->stream));
+  if (ub_dev) CK(ctx, cudaMemcpyAsync(ub_dev, sc.ub, (size_t)B * S * 4, cudaMemcpyDeviceToDevice, ctx->stream));
+  BetaSweep bs; bs.split = split_dev; bs.gb_lo = gb_lo_dev; bs.gb_up = gb_up_dev;
+  return alpha_forward(ctx, B, S, sc, x_lo_dev, x_hi_dev, const_cast<float* const*>(reinterpret_cast<const float* const*>(alpha_lo_dev)),
+                       const_cast<float* const*>(reinterpret_cast<const float* const*>(alpha_up_dev)), g_lo_dev, g_up_dev, nullptr, 0,
+                       split_dev ? &bs : nullptr);
+}
+
+static int beta_ascent_impl(crown_ctx* ctx, int B, const float* C_dev, int S, const float* const* l_dev,
+                            const float* const* u_dev, const int8_t* const* split_dev, float* const* alpha_lo_dev,
+                            float* const* alpha_up_dev, float* const* beta_lo_dev, float* const* beta_up_dev,
+                            const float* x_lo_dev, const float* x_hi_dev, float eta_alpha, float eta_beta, float decay,
+                            int iters, int mode, float* lb_best_dev, float* ub_best_dev, float* lb_last_dev,
+                            float* ub_last_dev, uint8_t* verified_dev, void* scratch_dev, size_t scratch_bytes,
+                            const char* who) {
+  if (iters < 0 || (mode != 0 && mode != 1) || !(eta_alpha >= 0.f) || !(eta_beta >= 0.f) || !(decay > 0.f) || !lb_best_dev || !ub_best_dev)
+    return fail(ctx, CROWN_EINVAL, std::string(who) + ": bad arguments");
+  AlphaScratch sc;
+  const float* const* al = reinterpret_cast<const float* const*>(alpha_lo_dev);
+  const float* const* au = reinterpret_cast<const float* const*>(alpha_up_dev);
+  int rc = alpha_check(ctx, B, S, C_dev, l_dev, u_dev, al, au, x_lo_dev, x_hi_dev, scratch_dev, scratch_bytes, true, sc);
+  if (rc) return rc;
+  if (split_dev)
+    for (size_t i = 0; i < ctx->nodes.size(); ++i)
+      if (split_dev[i] && (!beta_lo_dev || !beta_up_dev || !beta_lo_dev[i] || !beta_up_dev[i] || beta_lo_dev[i] == beta_up_dev[i]))
+        return fail(ctx, CROWN_EINVAL, std::string(who) + ": every split ReLU needs distinct beta_lo and beta_up tensors");
+  cudaStream_t s = ctx->stream;
+  CK(ctx, cudaMemsetAsync(scratch_dev, 0, sc.bytes, s));
+  { Scope scp(ctx, CROWN_K_MISC); launch_alpha_set_step(sc.step, eta_alpha, s, eta_beta); }
+  SplitSpec sp; sp.split = split_dev;
+  sp.beta_lo = reinterpret_cast<const float* const*>(beta_lo_dev); sp.beta_up = reinterpret_cast<const float* const*>(beta_up_dev);
+  BetaSweep bs; bs.split = split_dev; bs.beta_lo = beta_lo_dev; bs.beta_up = beta_up_dev;
+  std::vector<char> coef_ready(ctx->nodes.size(), 0);      // the intermediate bounds and the split are fixed: coefficients once
+  for (int t = 0; t <= iters; ++t) {
+    rc = alpha_backward(ctx, B, S, C_dev, l_dev, u_dev, al, au, x_lo_dev, x_hi_dev, sc, &coef_ready, split_dev ? &sp : nullptr);
+    if (rc) return rc;
+    { Scope scp(ctx, CROWN_K_MISC); launch_alpha_best(sc.lb, sc.ub, lb_best_dev, ub_best_dev, sc.step, decay, t == 0, B * S, s); }
+    if (t == iters) break;
+    rc = alpha_forward(ctx, B, S, sc, x_lo_dev, x_hi_dev, alpha_lo_dev, alpha_up_dev, nullptr, nullptr, sc.step, mode,
+                       split_dev ? &bs : nullptr);
+    if (rc) return rc;
+  }
+  if (lb_last_dev) CK(ctx, cudaMemcpyAsync(lb_last_dev, sc.lb, (size_t)B * S * 4, cudaMemcpyDeviceToDevice, s));
+  if (ub_last_dev) CK(ctx, cudaMemcpyAsync(ub_last_dev, sc.ub, (size_t)B * S * 4, cudaMemcpyDeviceToDevice, s));
+  if (verified_dev) { Scope scp(ctx, CROWN_K_MISC); launch_verdict(lb_best_dev, verified_dev, B, S, s); }
+  CK(ctx, cudaGetLastError());
+  return CROWN_OK;
+}
+
 extern "C" int crown_alpha_grad(crown_ctx* ctx, int B, const float* C_dev, int S, const float* const* l_dev,
                                 const float* const* u_dev, const float* const* alpha_lo_dev,
                                 const float* const* alpha_up_dev, const float* x_lo_dev, const float* x_hi_dev,
                                 float* const* g_lo_dev, float* const* g_up_dev, float* lb_dev, float* ub_dev,
                                 void* scratch_dev, size_t scratch_bytes) {
   if (!ctx) return CROWN_EINVAL;
-  AlphaScratch sc;
-  int rc = alpha_check(ctx, B, S, C_dev, l_dev, u_dev, alpha_lo_dev, alpha_up_dev, x_lo_dev, x_hi_dev, scratch_dev,
-                       scratch_bytes, false, sc);
-  if (rc) return rc;
-  CK(ctx, cudaMemsetAsync(scratch_dev, 0, sc.bytes, ctx->stream));
-  rc = alpha_backward(ctx, B, S, C_dev, l_dev, u_dev, alpha_lo_dev, alpha_up_dev, x_lo_dev, x_hi_dev, sc, nullptr);
-  if (rc) return rc;
-  if (lb_dev) CK(ctx, cudaMemcpyAsync(lb_dev, sc.lb, (size_t)B * S * 4, cudaMemcpyDeviceToDevice, ctx->stream));
-  if (ub_dev) CK(ctx, cudaMemcpyAsync(ub_dev, sc.ub, (size_t)B * S * 4, cudaMemcpyDeviceToDevice, ctx->stream));
-  return alpha_forward(ctx, B, S, sc, x_lo_dev, x_hi_dev, const_cast<float* const*>(reinterpret_cast<const float* const*>(alpha_lo_dev)),
-                       const_cast<float* const*>(reinterpret_cast<const float* const*>(alpha_up_dev)), g_lo_dev, g_up_dev, nullptr, 0);
+  return beta_grad_impl(ctx, B, C_dev, S, l_dev, u_dev, nullptr, alpha_lo_dev, alpha_up_dev, nullptr, nullptr, x_lo_dev,
+                        x_hi_dev, g_lo_dev, g_up_dev, nullptr, nullptr, lb_dev, ub_dev, scratch_dev, scratch_bytes);
 }
 
 extern "C" int crown_alpha_ascent(crown_ctx* ctx, int B, const float* C_dev, int S, const float* const* l_dev,
@@ -703,30 +786,50 @@ extern "C" int crown_alpha_ascent(crown_ctx* ctx, int B, const float* C_dev, int
                                   int mode, float* lb_best_dev, float* ub_best_dev, float* lb_last_dev,
                                   float* ub_last_dev, uint8_t* verified_dev, void* scratch_dev, size_t scratch_bytes) {
   if (!ctx) return CROWN_EINVAL;
-  if (iters < 0 || (mode != 0 && mode != 1) || !(eta >= 0.f) || !(decay > 0.f) || !lb_best_dev || !ub_best_dev)
-    return fail(ctx, CROWN_EINVAL, "crown_alpha_ascent: bad arguments");
-  AlphaScratch sc;
-  const float* const* al = reinterpret_cast<const float* const*>(alpha_lo_dev);
-  const float* const* au = reinterpret_cast<const float* const*>(alpha_up_dev);
-  int rc = alpha_check(ctx, B, S, C_dev, l_dev, u_dev, al, au, x_lo_dev, x_hi_dev, scratch_dev, scratch_bytes, true, sc);
-  if (rc) return rc;
-  cudaStream_t s = ctx->stream;
-  CK(ctx, cudaMemsetAsync(scratch_dev, 0, sc.bytes, s));
-  { Scope scp(ctx, CROWN_K_MISC); launch_alpha_set_step(sc.step, eta, s); }
-  std::vector<char> coef_ready(ctx->nodes.size(), 0);      // the intermediate bounds are fixed: coefficients once
-  for (int t = 0; t <= iters; ++t) {
-    rc = alpha_backward(ctx, B, S, C_dev, l_dev, u_dev, al, au, x_lo_dev, x_hi_dev, sc, &coef_ready);
-    if (rc) return rc;
-    { Scope scp(ctx, CROWN_K_MISC); launch_alpha_best(sc.lb, sc.ub, lb_best_dev, ub_best_dev, sc.step, decay, t == 0, B * S, s); }
-    if (t == iters) break;
-    rc = alpha_forward(ctx, B, S, sc, x_lo_dev, x_hi_dev, alpha_lo_dev, alpha_up_dev, nullptr, nullptr, sc.step, mode);
-    if (rc) return rc;
-  }
-  if (lb_last_dev) CK(ctx, cudaMemcpyAsync(lb_last_dev, sc.lb, (size_t)B * S * 4, cudaMemcpyDeviceToDevice, s));
-  if (ub_last_dev) CK(ctx, cudaMemcpyAsync(ub_last_dev, sc.ub, (size_t)B * S * 4, cudaMemcpyDeviceToDevice, s));
-  if (verified_dev) { Scope scp(ctx, CROWN_K_MISC); launch_verdict(lb_best_dev, verified_dev, B, S, s); }
-  CK(ctx, cudaGetLastError());
-  return CROWN_OK;
+  return beta_ascent_impl(ctx, B, C_dev, S, l_dev, u_dev, nullptr, alpha_lo_dev, alpha_up_dev, nullptr, nullptr, x_lo_dev,
+                          x_hi_dev, eta, 0.f, decay, iters, mode, lb_best_dev, ub_best_dev, lb_last_dev, ub_last_dev,
+                          verified_dev, scratch_dev, scratch_bytes, "crown_alpha_ascent");
+}
+
+// ================================================================================================
+// NEXT-2 -- beta-CROWN bounds of batched BaB sub-domains
+// ================================================================================================
+extern "C" int crown_backward_split(crown_ctx* ctx, int B, int start, int row0, int rows, const float* C_dev,
+                                    const float* const* l_dev, const float* const* u_dev,
+                                    const int8_t* const* split_dev, const float* const* alpha_lo_dev,
+                                    const float* const* alpha_up_dev, const float* const* beta_lo_dev,
+                                    const float* const* beta_up_dev, float* A_dev, float* d_dev,
+                                    const float* x_lo_dev, const float* x_hi_dev, float* lb_dev, float* ub_dev) {
+  if (!ctx) return CROWN_EINVAL;
+  if (!A_dev && !d_dev && !lb_dev) return fail(ctx, CROWN_EINVAL, "crown_backward_split: no output requested");
+  SplitSpec sp; sp.split = split_dev; sp.beta_lo = beta_lo_dev; sp.beta_up = beta_up_dev;
+  return run_pass(ctx, B, start, row0, rows, C_dev, l_dev, u_dev, alpha_lo_dev, alpha_up_dev, A_dev, d_dev,
+                  x_lo_dev, x_hi_dev, lb_dev, ub_dev, rows, nullptr, nullptr, split_dev ? &sp : nullptr);
+}
+
+extern "C" int crown_beta_grad(crown_ctx* ctx, int B, const float* C_dev, int S, const float* const* l_dev,
+                               const float* const* u_dev, const int8_t* const* split_dev,
+                               const float* const* alpha_lo_dev, const float* const* alpha_up_dev,
+                               const float* const* beta_lo_dev, const float* const* beta_up_dev,
+                               const float* x_lo_dev, const float* x_hi_dev, float* const* g_lo_dev,
+                               float* const* g_up_dev, float* const* gb_lo_dev, float* const* gb_up_dev,
+                               float* lb_dev, float* ub_dev, void* scratch_dev, size_t scratch_bytes) {
+  if (!ctx) return CROWN_EINVAL;
+  return beta_grad_impl(ctx, B, C_dev, S, l_dev, u_dev, split_dev, alpha_lo_dev, alpha_up_dev, beta_lo_dev, beta_up_dev,
+                        x_lo_dev, x_hi_dev, g_lo_dev, g_up_dev, gb_lo_dev, gb_up_dev, lb_dev, ub_dev, scratch_dev, scratch_bytes);
+}
+
+extern "C" int crown_beta_ascent(crown_ctx* ctx, int B, const float* C_dev, int S, const float* const* l_dev,
+                                 const float* const* u_dev, const int8_t* const* split_dev,
+                                 float* const* alpha_lo_dev, float* const* alpha_up_dev, float* const* beta_lo_dev,
+                                 float* const* beta_up_dev, const float* x_lo_dev, const float* x_hi_dev,
+                                 float eta_alpha, float eta_beta, float decay, int iters, int mode,
+                                 float* lb_best_dev, float* ub_best_dev, float* lb_last_dev, float* ub_last_dev,
+                                 uint8_t* verified_dev, void* scratch_dev, size_t scratch_bytes) {
+  if (!ctx) return CROWN_EINVAL;
+  return beta_ascent_impl(ctx, B, C_dev, S, l_dev, u_dev, split_dev, alpha_lo_dev, alpha_up_dev, beta_lo_dev, beta_up_dev,
+                          x_lo_dev, x_hi_dev, eta_alpha, eta_beta, decay, iters, mode, lb_best_dev, ub_best_dev,
+                          lb_last_dev, ub_last_dev, verified_dev, scratch_dev, scratch_bytes, "crown_beta_ascent");
 }
 
 // ================================================================================================

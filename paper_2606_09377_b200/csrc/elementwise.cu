@@ -11,10 +11,15 @@ namespace crownb200 {
 // (reading G3); adaptive rule lambda = 1 iff u > -l (reading G4).
 // ------------------------------------------------------------------------------------------------
 __global__ void relax_coeffs_kernel(const float* __restrict__ l, const float* __restrict__ u,
-                                    float4* __restrict__ coef, long long count, int rule) {
+                                    float4* __restrict__ coef, long long count, int rule,
+                                    const int8_t* __restrict__ split) {
   long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= count) return;
   float lo = l[i], hi = u[i];
+  if (split) {                      // BaB sub-domain (reading G26): the fixed state clamps the interval
+    const int sg = split[i];
+    if (sg > 0) lo = fmaxf(lo, 0.f); else if (sg < 0) hi = fminf(hi, 0.f);
+  }
   float4 c;
   if (lo >= 0.f) {
     c = make_float4(1.f, 0.f, 1.f, 0.f);
@@ -30,10 +35,11 @@ __global__ void relax_coeffs_kernel(const float* __restrict__ l, const float* __
   coef[i] = c;
 }
 
-void launch_relax_coeffs(const float* l, const float* u, float4* coef, long long count, int rule, cudaStream_t s) {
+void launch_relax_coeffs(const float* l, const float* u, float4* coef, long long count, int rule, cudaStream_t s,
+                         const int8_t* split) {
   if (count <= 0) return;
   int threads = 256;
-  relax_coeffs_kernel<<<ceil_div(count, threads), threads, 0, s>>>(l, u, coef, count, rule);
+  relax_coeffs_kernel<<<ceil_div(count, threads), threads, 0, s>>>(l, u, coef, count, rule, split);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -50,6 +56,7 @@ struct RelaxDev {
   const float* bias; int bias_div;
   float* out; float* out_lo; float* d;
   int B, R, n;
+  const int8_t* split; const float* beta_lo; const float* beta_up;   // NEXT-2 (BETA instantiations only)
   int wpp;      // warps per (b, r) pair: 1, 2, 4 or 8 (all in one block); a function of n ONLY, so that the summation
                 // order of d does not depend on how the rows are chunked (chunked == unchunked bitwise)
 };
@@ -60,9 +67,11 @@ static inline int warps_per_pair(int n) { return n >= 4096 ? 8 : (n >= 2048 ? 4 
 __device__ __forceinline__ float clip01(float a) { return fminf(fmaxf(a, 0.f), 1.f); }
 
 // one element, both branches.  Returns contributions to d.
+// btL / btU: the beta-CROWN terms max(beta_lo, 0) * s and max(beta_up, 0) * s of this element (0 without a split)
 template <bool RELU, bool ALPHA>
 __device__ __forceinline__ void relax_elem(float aL, float aU, const float4& c, float alL, float alU,
-                                           float bias, float& oL, float& oU, float& dLacc, float& dUacc) {
+                                           float bias, float& oL, float& oU, float& dLacc, float& dUacc,
+                                           float btL = 0.f, float btU = 0.f) {
   if (RELU) {
     float dU = c.x, bU = c.y;
     float sL = c.z, sU = c.z;
@@ -71,8 +80,8 @@ __device__ __forceinline__ void relax_elem(float aL, float aU, const float4& c, 
     }
     float pL = fmaxf(aL, 0.f), mL = fminf(aL, 0.f);
     float pU = fmaxf(aU, 0.f), mU = fminf(aU, 0.f);
-    oL = pL * sL + mL * dU;
-    oU = pU * dU + mU * sU;
+    oL = pL * sL + mL * dU - btL;
+    oU = pU * dU + mU * sU + btU;
     dLacc = fmaf(mL, bU, dLacc);
     dUacc = fmaf(pU, bU, dUacc);
   } else {
@@ -82,7 +91,7 @@ __device__ __forceinline__ void relax_elem(float aL, float aU, const float4& c, 
   dUacc = fmaf(oU, bias, dUacc);
 }
 
-template <bool RELU, bool ALPHA, bool SPLIT, int VEC>
+template <bool RELU, bool ALPHA, bool SPLIT, int VEC, bool BETA = false>
 __global__ void __launch_bounds__(256) relax_kernel(RelaxDev p) {
   const int lane = threadIdx.x & 31;
   const int wpp = p.wpp;
@@ -99,6 +108,9 @@ __global__ void __launch_bounds__(256) relax_kernel(RelaxDev p) {
   const long long arow = ((long long)b * p.R + r) * p.n;
   const float* alL = ALPHA ? p.alpha_lo + arow : nullptr;
   const float* alU = ALPHA ? p.alpha_up + arow : nullptr;
+  const int8_t* sp = BETA ? p.split + (long long)b * p.n : nullptr;
+  const float* btL = (BETA && p.beta_lo) ? p.beta_lo + arow : nullptr;
+  const float* btU = (BETA && p.beta_up) ? p.beta_up + arow : nullptr;
   const long long BR = (long long)p.B * p.R;
   float* o0 = p.out + (pair) * (long long)p.n;
   float* o1 = p.out + (BR + pair) * (long long)p.n;
@@ -124,10 +136,18 @@ __global__ void __launch_bounds__(256) relax_kernel(RelaxDev p) {
                bs.z = __ldg(p.bias + (j + 2) / p.bias_div); bs.w = __ldg(p.bias + (j + 3) / p.bias_div); }
       }
       float4 yL, yU;
-      relax_elem<RELU, ALPHA>(xL.x, xU.x, c0, tL.x, tU.x, bs.x, yL.x, yU.x, accL, accU);
-      relax_elem<RELU, ALPHA>(xL.y, xU.y, c1, tL.y, tU.y, bs.y, yL.y, yU.y, accL, accU);
-      relax_elem<RELU, ALPHA>(xL.z, xU.z, c2, tL.z, tU.z, bs.z, yL.z, yU.z, accL, accU);
-      relax_elem<RELU, ALPHA>(xL.w, xU.w, c3, tL.w, tU.w, bs.w, yL.w, yU.w, accL, accU);
+      float4 eL = make_float4(0, 0, 0, 0), eU = eL;
+      if (BETA) {
+        const char4 sg = *reinterpret_cast<const char4*>(sp + j);
+        if (btL) { const float4 v = ldg_stream4(btL + j);
+                   eL = make_float4(fmaxf(v.x, 0.f) * sg.x, fmaxf(v.y, 0.f) * sg.y, fmaxf(v.z, 0.f) * sg.z, fmaxf(v.w, 0.f) * sg.w); }
+        if (btU) { const float4 v = (btU == btL) ? ldg_stream4(btL + j) : ldg_stream4(btU + j);
+                   eU = make_float4(fmaxf(v.x, 0.f) * sg.x, fmaxf(v.y, 0.f) * sg.y, fmaxf(v.z, 0.f) * sg.z, fmaxf(v.w, 0.f) * sg.w); }
+      }
+      relax_elem<RELU, ALPHA>(xL.x, xU.x, c0, tL.x, tU.x, bs.x, yL.x, yU.x, accL, accU, eL.x, eU.x);
+      relax_elem<RELU, ALPHA>(xL.y, xU.y, c1, tL.y, tU.y, bs.y, yL.y, yU.y, accL, accU, eL.y, eU.y);
+      relax_elem<RELU, ALPHA>(xL.z, xU.z, c2, tL.z, tU.z, bs.z, yL.z, yU.z, accL, accU, eL.z, eU.z);
+      relax_elem<RELU, ALPHA>(xL.w, xU.w, c3, tL.w, tU.w, bs.w, yL.w, yU.w, accL, accU, eL.w, eU.w);
       if (SPLIT) {
         float4 hL, lL, hU, lU;
         tf32_split(yL.x, hL.x, lL.x); tf32_split(yL.y, hL.y, lL.y);
@@ -148,7 +168,13 @@ __global__ void __launch_bounds__(256) relax_kernel(RelaxDev p) {
       float tL = ALPHA ? alL[j] : 0.f, tU = ALPHA ? alU[j] : 0.f;
       float bs = p.bias ? p.bias[j / p.bias_div] : 0.f;
       float yL, yU;
-      relax_elem<RELU, ALPHA>(xL, xU, c, tL, tU, bs, yL, yU, accL, accU);
+      float eL = 0.f, eU = 0.f;
+      if (BETA) {
+        const float sg = (float)sp[j];
+        if (btL) eL = fmaxf(btL[j], 0.f) * sg;
+        if (btU) eU = fmaxf(btU[j], 0.f) * sg;
+      }
+      relax_elem<RELU, ALPHA>(xL, xU, c, tL, tU, bs, yL, yU, accL, accU, eL, eU);
       if (SPLIT) {
         float h, l2;
         tf32_split(yL, h, l2); o0[j] = h; q0[j] = l2;
@@ -179,6 +205,11 @@ __global__ void __launch_bounds__(256) relax_kernel(RelaxDev p) {
 
 template <bool RELU, bool ALPHA, bool SPLIT>
 static void relax_dispatch_vec(const RelaxDev& p, bool vec, int blocks, cudaStream_t s) {
+  if (RELU && p.split) {          // beta-CROWN term (NEXT-2)
+    if (vec) relax_kernel<RELU, ALPHA, SPLIT, 4, RELU><<<blocks, 256, 0, s>>>(p);
+    else relax_kernel<RELU, ALPHA, SPLIT, 1, RELU><<<blocks, 256, 0, s>>>(p);
+    return;
+  }
   if (vec) relax_kernel<RELU, ALPHA, SPLIT, 4><<<blocks, 256, 0, s>>>(p);
   else relax_kernel<RELU, ALPHA, SPLIT, 1><<<blocks, 256, 0, s>>>(p);
 }
@@ -190,6 +221,7 @@ void launch_relax(const RelaxArgs& a, cudaStream_t s) {
   if (!p.alpha_lo) p.alpha_lo = p.alpha_up;
   p.bias = a.bias; p.bias_div = a.bias_div > 0 ? a.bias_div : 1;
   p.out = a.out; p.out_lo = a.out_lo; p.d = a.d; p.B = a.B; p.R = a.R; p.n = a.n;
+  p.split = (a.coef && (a.beta_lo || a.beta_up)) ? a.split : nullptr; p.beta_lo = a.beta_lo; p.beta_up = a.beta_up;
   long long pairs = (long long)a.B * a.R;
   if (pairs <= 0 || a.n <= 0) return;
   p.wpp = warps_per_pair(a.n);
@@ -197,7 +229,9 @@ void launch_relax(const RelaxArgs& a, cudaStream_t s) {
   auto al16 = [](const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; };
   bool vec = (a.n % 4 == 0) && (p.ld % 4 == 0) && (p.sB % 4 == 0) && (p.sBr % 4 == 0) && al16(p.A) &&
              al16(p.out) && (!p.out_lo || al16(p.out_lo)) && (!p.alpha_lo || al16(p.alpha_lo)) &&
-             (!p.alpha_up || al16(p.alpha_up)) && (!p.bias || p.bias_div != 1 || al16(p.bias));
+             (!p.alpha_up || al16(p.alpha_up)) && (!p.bias || p.bias_div != 1 || al16(p.bias)) &&
+             (!p.split || ((reinterpret_cast<uintptr_t>(p.split) & 3) == 0 && (!p.beta_lo || al16(p.beta_lo)) &&
+                           (!p.beta_up || al16(p.beta_up))));
   bool relu = a.coef != nullptr, alpha = relu && p.alpha_lo != nullptr, split = a.out_lo != nullptr;
 #define CROWN_RELAX_CASE(R_, A_, S_) relax_dispatch_vec<R_, A_, S_>(p, vec, blocks, s)
   if (relu) {

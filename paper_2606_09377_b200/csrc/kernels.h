@@ -18,7 +18,10 @@ struct AView {
 
 // a3 -- relaxation coefficients of a ReLU from its pre-activation bounds.
 // coef[b*n+j] = {dU, bU, dL_fixed, unstable?1:0}.  rule: 0 adaptive, 1 zero, 2 one.
-void launch_relax_coeffs(const float* l, const float* u, float4* coef, long long count, int rule, cudaStream_t s);
+// split (NEXT-2; reading G26), int8 [count] or nullptr: +1 clamps l to max(l, 0), -1 clamps u to min(u, 0)
+// before the classification, so a split neuron gets the exact line of its fixed state.
+void launch_relax_coeffs(const float* l, const float* u, float4* coef, long long count, int rule, cudaStream_t s,
+                         const int8_t* split = nullptr);
 
 // a4 -- fused relaxation of A through a ReLU, both branches, with the bias
 // accumulation of the ReLU (bU through the sign-selected part of A) and of the linear layer below
@@ -34,6 +37,11 @@ struct RelaxArgs {
   float* out_lo;             // TF32 lo part or nullptr
   float* d;                  // [2,B,R] in/out: d += ...
   int B, R, n;
+  // NEXT-2 -- beta-CROWN split constraints (reading G27): after the relaxation,
+  // lower: Abar -= max(beta_lo, 0) * s, upper: Abar += max(beta_up, 0) * s  (the bias term d += Abar . b sees the sum)
+  const int8_t* split = nullptr;   // [B, n] in {-1, 0, +1} or nullptr
+  const float* beta_lo = nullptr;  // [B, R, n] or nullptr (= 0)
+  const float* beta_up = nullptr;
 };
 void launch_relax(const RelaxArgs& a, cudaStream_t s);
 
@@ -132,12 +140,15 @@ void launch_alpha_linear(const float* G, const float* W, const float* bias, floa
 void launch_alpha_conv(const float* W, const float* bias, const float* in, float* out, long long M, int c_in, int h,
                        int w, int c_out, int kh, int kw, int stride, int pad, int ho, int wo, cudaStream_t s);
 void launch_alpha_add(const float* a, const float* b, float* o, long long cnt, cudaStream_t s);
+// split / beta_lo / beta_up / gb_lo / gb_up (NEXT-2, reading G28; all nullptr = alpha only): d lb / d beta_lo = -s * Gin,
+// d ub / d beta_up = +s * Gin; step mode: beta <- max(max(beta, 0) +/- step[1] * dir, 0) in place.
 void launch_alpha_relu(const float* A, const float* Gin, const float4* coef, float* alpha_lo, float* alpha_up,
                        float* Gout, float* g_lo, float* g_up, const float* step, int mode, int B, int S, int n,
-                       cudaStream_t s);
+                       cudaStream_t s, const int8_t* split = nullptr, float* beta_lo = nullptr, float* beta_up = nullptr,
+                       float* gb_lo = nullptr, float* gb_up = nullptr);
 void launch_alpha_best(const float* lb, const float* ub, float* lb_best, float* ub_best, float* step, float decay,
                        int first, int count, cudaStream_t s);
-void launch_alpha_set_step(float* step, float v, cudaStream_t s);
+void launch_alpha_set_step(float* step, float v, cudaStream_t s, float v_beta = 0.f);   // step[0] = alpha step, step[1] = beta step
 
 // Per-device kernel attributes (opt-in dynamic shared memory sizes).  cudaFuncSetAttribute applies to the CURRENT
 // device only, so crown_init calls this for the device of every new context (a process-wide "done" flag would
