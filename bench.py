@@ -61,6 +61,9 @@ def parse_args():
                     help="alpha-mode configs: also time this many projected ascent steps on alpha (NEXT-1; 0 = skip)")
     ap.add_argument("--bab-domains", type=int, default=4096,
                     help="cfg2: also time the joint alpha/beta ascent (NEXT-2) on this many BaB sub-domains (0 = skip)")
+    ap.add_argument("--shard-rows", action="store_true",
+                    help="NEXT-4 (opt-in, torchrun): all ranks work on the SAME batch; the identity rows of every intermediate "
+                         "pass are sharded across ranks, one AllGather of (l_k, u_k) per layer (strong scaling)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--device-steps-only", action="store_true",
                     help="profiling aid (ncu): only the warm-up and the timed device steps of --workload; no TF32 peak "
@@ -361,6 +364,10 @@ def measure_config(cfgname, args, steps, warmup, dev, local, world, tf32_peak, w
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
 
     def step_device():
+        if args.shard_rows:
+            r = multi.crown_run_row_sharded(ctx, xlo, xhi, Cd, alpha, int(os.environ.get("RANK", "0")), world)
+            io["lb"], io["ub"], io["verified"] = r["lb"], r["ub"], r["verified"]
+            return
         ctx.run_device(xlo, xhi, Cd, alpha, inter, io)
 
     # ---- pinned host buffers for the end-to-end leg ---------------------------------------------------
@@ -422,8 +429,8 @@ def measure_config(cfgname, args, steps, warmup, dev, local, world, tf32_peak, w
     verified = int(io["verified"].sum().item())
     # long steps: the end-to-end and the instrumented legs run fewer steps (they re-measure the same kernels)
     n_aux = steps if ms_step < 200.0 else max(2, min(steps, int(15000.0 / ms_step)))
-    if args.device_steps_only:
-        out = {"value": world * B / (ms_step * 1e-3), "unit": UNIT, "steps": steps, "ms_per_step": ms_step,
+    if args.device_steps_only or args.shard_rows:
+        out = {"value": (B if args.shard_rows else world * B) / (ms_step * 1e-3), "unit": UNIT, "steps": steps, "ms_per_step": ms_step,
                "config": workload_desc(wl, cfgname), "gpu_launches_per_step": int(launches_per_step), "clocks": clocks,
                "aw_flops_per_step": flops_step}
         ctx.close()
@@ -609,10 +616,12 @@ def run_b200(args):
     dev = torch.device("cuda", local)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
-    if args.device_steps_only:
+    if args.device_steps_only or args.shard_rows:
         r = measure_config(args.workload, args, args.steps, args.warmup, dev, local, world, None, False)
         if rank == 0:
-            print(json.dumps(dict(r, metric=METRIC, n_gpus=world, warmup=args.warmup, mode="device-steps-only")))
+            print(json.dumps(dict(r, metric=METRIC, n_gpus=world, warmup=args.warmup, higher_is_better=True,
+                                  scaling="strong" if args.shard_rows else "weak", data="synthetic",
+                                  mode="row-sharded (NEXT-4)" if args.shard_rows else "device-steps-only")))
         if world > 1:
             dist.destroy_process_group()
         return

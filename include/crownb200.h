@@ -124,8 +124,10 @@ int ibp_forward(crown_ctx* ctx, int B, const float* x_lo_dev, const float* x_hi_
 /* O3 -- one CROWN backward pass (PAPER.md:64-68 Eq. 1, :128 A <- A.Lambda_i W_i) from node
  * `start` down to the input, for `rows` start-spec rows per property.
  *   C_dev == NULL : start matrix = rows [row0, row0+rows) of the identity on node `start`'s
- *                   output (intermediate bounds); `start` must be a Linear node
- *                   (CROWN_EUNSUPPORTED otherwise: identity starts on conv maps are NEXT-3).
+ *                   output (intermediate bounds).  `start` is any non-ReLU node: for a Linear node
+ *                   the rows of W are read in place; for a conv-shaped node (Conv2d / Add / Flatten output; full-CROWN
+ *                   intermediate bounds of a conv net) the rows are materialised
+ *                   one-hot and the sweep starts at the node itself.
  *   C_dev != NULL : [B, rows, size_start] start matrix (row0 ignored).
  *   l_dev/u_dev   : arrays of n_nodes pointers; for every ReLU node i below `start`, the
  *                   pre-activation bounds of its INPUT, [B, size_i].
@@ -151,9 +153,14 @@ int concretize(crown_ctx* ctx, int B, int rows, const float* A_dev, const float*
                const float* x_lo_dev, const float* x_hi_dev,
                float* lb_dev, float* ub_dev, int out_stride);
 
+/* a9 on its own -- verdict: verified_dev[b] = 1 iff every lb_dev[b, s] > 0 (a NaN bound fails
+ * closed), lb_dev [B, S], verified_dev [B] uint8.  For callers that assemble the path from the calls above. */
+int crown_verdict(crown_ctx* ctx, int B, int S, const float* lb_dev, uint8_t* verified_dev);
+
 /* The whole hot path for a batch (O4 then O5 then the verdict):
  *   intermediate = 0: CROWN intermediate bounds for every ReLU in topological order (first
- *                     layer by IBP, which coincides), row-chunked under mem_cap;
+ *                     layer by IBP, which coincides), row-chunked under mem_cap; Linear AND
+ *                     conv-shaped pre-activations (conv nets: dense A, chunks of crown_row_chunk rows);
  *   intermediate = 1: IBP for every pre-activation (cfg5, reading G22);
  *   then the final pass from the last node with C_dev [B,S,n_L] and alpha (array of n_nodes
  *   pointers, entry i = [B,S,size_i] for ReLU i, or NULL array/entries = slope rule).

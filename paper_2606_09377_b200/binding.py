@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libcrownb200.so")
 OP_CODES = {"linear": 1, "conv": 2, "relu": 3, "add": 4, "flatten": 5}
 K_CLASSES = ["ibp", "coeff", "relax", "gemm_tc", "gemm_ffma", "concretize", "conv", "misc"]
 
-EXPORTS = ["crown_h2d_bytes", "crown_workspace_bytes", "crown_init", "ibp_forward", "crown_backward", "concretize", "crown_run",
+EXPORTS = ["crown_h2d_bytes", "crown_workspace_bytes", "crown_init", "ibp_forward", "crown_backward", "concretize", "crown_verdict", "crown_run",
            "crown_run_host", "crown_alpha_scratch_bytes", "crown_alpha_grad", "crown_alpha_ascent", "crown_backward_split", "crown_beta_grad", "crown_beta_ascent", "crown_gemm", "crown_split_tf32", "crown_peak_bytes", "crown_row_chunk", "crown_launch_count", "crown_graph_replays",
            "crown_gemm_flops", "crown_timing", "crown_timing_read", "crown_last_error", "crown_destroy",
            "crown_version"]
@@ -68,6 +68,7 @@ def load_library() -> C.CDLL:
     lib.crown_backward.argtypes = [vp, i32, i32, i32, i32, vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp),
                                    C.POINTER(vp), vp, vp, vp, vp, vp, vp]
     lib.concretize.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp, vp, i32]
+    lib.crown_verdict.argtypes = [vp, i32, i32, vp, vp]
     lib.crown_run.argtypes = [vp, i32, vp, vp, vp, i32, C.POINTER(vp), i32, C.POINTER(vp), C.POINTER(vp), vp, vp, vp]
     lib.crown_run_host.argtypes = [vp, i32, vp, vp, vp, i32, C.POINTER(vp), i32, vp, vp, vp]
     lib.crown_alpha_scratch_bytes.argtypes = [vp, i32, i32, C.POINTER(C.c_size_t)]
@@ -249,6 +250,13 @@ class CrownContext:
         self._check(self.lib.concretize(self.h, B, R, A.data_ptr(), d.data_ptr(), x_lo.data_ptr(), x_hi.data_ptr(),
                                         lb.data_ptr(), ub.data_ptr(), R), self.h)
         return lb, ub
+
+    def verdict(self, lb: torch.Tensor) -> torch.Tensor:
+        """a9: verified[b] = 1 iff every lb[b, s] > 0 (device kernel)."""
+        B, S = lb.shape
+        v = torch.empty(B, dtype=torch.uint8, device=self.device)
+        self._check(self.lib.crown_verdict(self.h, B, S, lb.data_ptr(), v.data_ptr()), self.h)
+        return v
 
     # ---- whole path ----------------------------------------------------------------------------
     def alloc_io(self, B: int, S: int):

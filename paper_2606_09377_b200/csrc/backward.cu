@@ -137,9 +137,22 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
     { Scope sc(ctx, CROWN_K_MISC); launch_init_d(ctx->d_buf, nullptr, 0, B, R, s); }
     Pending p; p.v.p = C_dev; p.v.ld = sn.size; p.v.n = sn.size; p.v.sB = (long long)R * sn.size; p.v.sBr = 0;
     ps.pend[start] = p;
+  } else if (sn.n.op != CROWN_LINEAR) {
+    // NEXT-3: rows [row0, row0+R) of the identity on a conv-shaped node (Conv2d / Add / Flatten
+    // output).  The start matrix is materialised once as R one-hot rows shared by all branches and properties
+    // (zero-stride view) and the sweep begins AT the start node: its conv-transpose turns the rows into the 3x3xC_in
+    // patches of the layer, the rest of the pass is the dense recursion, row-chunked like every identity pass.
+    if (sn.n.op == CROWN_RELU) return fail(ctx, CROWN_EUNSUPPORTED, "crown_backward: identity start on a ReLU node");
+    if (row0 < 0 || row0 + R > sn.size) return fail(ctx, CROWN_EINVAL, "crown_backward: row range outside the start node");
+    { Scope sc(ctx, CROWN_K_MISC); launch_init_d(ctx->d_buf, nullptr, 0, B, R, s); }
+    float* oh = nullptr;
+    Pending p; p.buf = new_buf(ps, oh);
+    if (p.buf < 0) return fail(ctx, CROWN_ENOMEM, "backward: A-buffer pool exhausted");
+    { Scope sc(ctx, CROWN_K_MISC, 4.0 * R * sn.size); launch_onehot(oh, row0, R, sn.size, s); }
+    p.v.p = oh; p.v.ld = sn.size; p.v.n = sn.size; p.v.sB = 0; p.v.sBr = 0;
+    ps.pend[start] = p;
   } else {
     // rows [row0, row0+R) of the identity on a Linear node: I.W = those rows of W, I.b = those biases
-    if (sn.n.op != CROWN_LINEAR) return fail(ctx, CROWN_EUNSUPPORTED, "crown_backward: identity start needs a Linear node");
     if (row0 < 0 || row0 + R > sn.size) return fail(ctx, CROWN_EINVAL, "crown_backward: row range outside the start node");
     { Scope sc(ctx, CROWN_K_MISC); launch_init_d(ctx->d_buf, sn.n.b_dev, row0, B, R, s); }
     Pending p; p.v.ld = sn.n.n_in; p.v.n = sn.n.n_in; p.v.sB = 0; p.v.sBr = 0;
@@ -393,6 +406,14 @@ extern "C" int concretize(crown_ctx* ctx, int B, int rows, const float* A_dev, c
   return CROWN_OK;
 }
 
+extern "C" int crown_verdict(crown_ctx* ctx, int B, int S, const float* lb_dev, uint8_t* verified_dev) {
+  if (!ctx) return CROWN_EINVAL;
+  if (B <= 0 || S <= 0 || !lb_dev || !verified_dev) return fail(ctx, CROWN_EINVAL, "crown_verdict: bad arguments");
+  { Scope sc(ctx, CROWN_K_MISC); launch_verdict(lb_dev, verified_dev, B, S, ctx->stream); }
+  CK(ctx, cudaGetLastError());
+  return CROWN_OK;
+}
+
 // ================================================================================================
 // O4 + O5 + verdict: the whole hot path for one batch
 // ================================================================================================
@@ -433,8 +454,6 @@ static int crown_run_enqueue(crown_ctx* ctx, int B, const float* x_lo_dev, const
       const int src = ctx->nodes[i].n.in0;
       const crown_node& sn = ctx->nodes[src].n;
       if ((sn.op == CROWN_LINEAR || sn.op == CROWN_CONV2D) && sn.in0 < 0) continue;   // first layer: O1 (exact)
-      if (sn.op != CROWN_LINEAR)
-        return fail(ctx, CROWN_EUNSUPPORTED, "crown_run: CROWN intermediate bounds need Linear pre-activations (use intermediate=1)");
       const int size = ctx->nodes[src].size;
       for (int row0 = 0; row0 < size; row0 += ctx->plan.rc) {
         const int rows = std::min(ctx->plan.rc, size - row0);

@@ -381,9 +381,90 @@ static bool conv_bwd_set_attr() {
          cudaFuncSetAttribute(conv_bwd_tiled_kernel<KH, KW, S, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) == cudaSuccess &&
          cudaFuncSetAttribute(conv_bwd_tiled_kernel<KH, KW, S, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) == cudaSuccess;
 }
-int conv_init_device() {
-  return (conv_bwd_set_attr<3, 3, 1>() && conv_bwd_set_attr<3, 3, 2>() && conv_bwd_set_attr<1, 1, 1>() &&
-          conv_bwd_set_attr<1, 1, 2>()) ? 0 : -1;
+
+// ---- a6, 1x1 convolutions (the stride-2 skip connections of a ResNet; pad 0).  conv^T of a 1x1 kernel is a per-pixel
+// matrix product: A_in[m, ci, s*p, s*q] = sum_co W[co, ci] * A_out[m, co, p, q], every other pixel a structural zero.
+// Block = one spec row x PIX output pixels; A_out[m, :, tile] and W^T sit in shared memory; a thread owns one pixel x
+// CIP input channels and writes its s x s block of the input map (value + zeros) so that the stores of a warp are contiguous.
+// The generic tiled kernel walked the zero pixels as if they were work: 151 + 127 us for 0.84 GFLOP on cfg5 (profiles/r2_conv.md).
+template <int CIP>
+__global__ void __launch_bounds__(256)
+conv_bwd_1x1_kernel(const float* __restrict__ A, long long sBr, long long sB, long long ld, int B, int R,
+                    const float* __restrict__ W, const float* __restrict__ addend, float* __restrict__ out,
+                    int c_in, int h, int w, int c_out, int stride, int ho, int wo, int PIX) {
+  extern __shared__ __align__(16) float sm[];
+  float* Ws = sm;                          // [c_out][c_in]
+  float* As = sm + c_out * c_in;           // [c_out][PIX]
+  const long long m = blockIdx.y;
+  const int pix0 = blockIdx.x * PIX;
+  const int npix = ho * wo;
+  for (int i = threadIdx.x; i < c_out * c_in; i += blockDim.x) Ws[i] = __ldg(W + i);     // W [c_out, c_in, 1, 1]
+  {
+    const int r = (int)(m % R);
+    const long long tt = m / R;
+    const float* a = A + (tt / B) * sBr + (tt % B) * sB + (long long)r * ld;
+    for (int i = threadIdx.x; i < c_out * PIX; i += blockDim.x) {
+      const int co = i / PIX, p = i % PIX;
+      As[i] = (pix0 + p < npix) ? __ldg(a + (long long)co * npix + pix0 + p) : 0.f;
+    }
+  }
+  __syncthreads();
+  const int p = threadIdx.x % PIX, cg = threadIdx.x / PIX;
+  const int ci0 = cg * CIP;
+  if (ci0 >= c_in || pix0 + p >= npix) return;
+  float acc[CIP];
+#pragma unroll
+  for (int c = 0; c < CIP; ++c) acc[c] = 0.f;
+  for (int co = 0; co < c_out; ++co) {
+    const float a = As[co * PIX + p];
+    const float* wr = Ws + co * c_in + ci0;
+#pragma unroll
+    for (int c = 0; c < CIP; ++c) acc[c] = fmaf(a, (ci0 + c < c_in) ? wr[c] : 0.f, acc[c]);
+  }
+  const int py = (pix0 + p) / wo, px = (pix0 + p) % wo;
+#pragma unroll
+  for (int c = 0; c < CIP; ++c) {
+    const int ci = ci0 + c;
+    if (ci >= c_in) break;
+    const long long base = (m * c_in + ci) * (long long)(h * w);
+    for (int dy = 0; dy < stride; ++dy) {
+      const int y = py * stride + dy;
+      if (y >= h) break;
+      for (int dx = 0; dx < stride; ++dx) {
+        const int x = px * stride + dx;
+        if (x >= w) break;
+        const long long o = base + (long long)y * w + x;
+        const float v = (dy == 0 && dx == 0) ? acc[c] : 0.f;
+        out[o] = addend ? v + __ldg(addend + o) : v;
+      }
+    }
+  }
+}
+
+// rows / columns of the input map that no output pixel reaches (h > stride * ho) are zero-filled by this launcher's caller
+// contract: supported only when stride * ho >= h and stride * wo >= w, i.e. every input pixel belongs to some s x s block
+static bool launch_conv_bwd_1x1(const AView& A, const float* W, const float* addend, float* out, int B, int R,
+                                int c_in, int h, int w, int c_out, int stride, int pad, int ho, int wo, cudaStream_t s) {
+  if (pad != 0 || stride < 1 || stride * ho < h || stride * wo < w || c_in > 64 || c_out > 64) return false;
+  const long long rows = 2LL * B * R;
+  if (rows > 65535) return false;
+  const int npix = ho * wo;
+  int PIX = 256;
+  while (PIX > 32 && PIX / 2 >= npix) PIX /= 2;
+  const int groups = 256 / PIX;                                   // channel groups per block
+  int cip = (c_in + groups - 1) / groups;
+  cip = cip <= 4 ? 4 : (cip <= 8 ? 8 : 16);
+  if ((long long)cip * groups < c_in) return false;
+  const size_t smem = ((size_t)c_out * c_in + (size_t)c_out * PIX) * sizeof(float);
+  if (smem > 96 * 1024) return false;
+  dim3 grid((unsigned)((npix + PIX - 1) / PIX), (unsigned)rows);
+  auto go = [&](auto kern) {
+    kern<<<grid, 256, smem, s>>>(A.p, A.sBr, A.sB, A.ld, B, R, W, addend, out, c_in, h, w, c_out, stride, ho, wo, PIX);
+  };
+  if (cip == 4) go(conv_bwd_1x1_kernel<4>);
+  else if (cip == 8) go(conv_bwd_1x1_kernel<8>);
+  else go(conv_bwd_1x1_kernel<16>);
+  return true;
 }
 
 void launch_conv_transpose(const AView& A, const float* W, const float* addend, float* out, int B, int R,
@@ -395,6 +476,7 @@ void launch_conv_transpose(const AView& A, const float* W, const float* addend, 
       launch_conv_transpose_tc(A, W, addend, out, B, R, c_in, h, w, c_out, num_sms, s) == 0) return;
   if ((A.sB % 1 == 0) && rows < (1LL << 31)) {
     bool done = false;
+    if (kh == 1 && kw == 1 && launch_conv_bwd_1x1(A, W, addend, out, B, R, c_in, h, w, c_out, stride, pad, ho, wo, s)) return;
     if (kh == 3 && kw == 3 && stride == 1) done = launch_conv_bwd_ct<3, 3, 1>(A, W, addend, out, B, R, c_in, h, w, c_out, pad, ho, wo, s);
     else if (kh == 3 && kw == 3 && stride == 2) done = launch_conv_bwd_ct<3, 3, 2>(A, W, addend, out, B, R, c_in, h, w, c_out, pad, ho, wo, s);
     else if (kh == 1 && kw == 1 && stride == 1) done = launch_conv_bwd_ct<1, 1, 1>(A, W, addend, out, B, R, c_in, h, w, c_out, pad, ho, wo, s);
@@ -407,6 +489,15 @@ void launch_conv_transpose(const AView& A, const float* W, const float* addend, 
   size_t smem = (size_t)c_out * kh * kw * sizeof(float);
   conv_transpose_kernel<<<grid, threads, smem, s>>>(A.p, A.sBr, A.sB, A.ld, B, R, W, addend, out, c_in, h, w,
                                                     c_out, kh, kw, stride, pad, ho, wo);
+}
+
+int conv_init_device() {
+  const int b1 = 96 * 1024;
+  if (cudaFuncSetAttribute(conv_bwd_1x1_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1) != cudaSuccess ||
+      cudaFuncSetAttribute(conv_bwd_1x1_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1) != cudaSuccess ||
+      cudaFuncSetAttribute(conv_bwd_1x1_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1) != cudaSuccess) return -1;
+  return (conv_bwd_set_attr<3, 3, 1>() && conv_bwd_set_attr<3, 3, 2>() && conv_bwd_set_attr<1, 1, 1>() &&
+          conv_bwd_set_attr<1, 1, 2>()) ? 0 : -1;
 }
 
 }  // namespace crownb200

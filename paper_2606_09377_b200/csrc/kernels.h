@@ -61,6 +61,8 @@ void launch_ibp_relu(const float* l, const float* u, float* lo, float* uo, long 
 void launch_ibp_add(const float* l0, const float* u0, const float* l1, const float* u1,
                     float* lo, float* uo, long long count, cudaStream_t s);
 
+// out[r, :] = e_{row0 + r} for r < R (row-major [R, n]): identity rows of a start node without a weight matrix (NEXT-3)
+void launch_onehot(float* out, int row0, int R, int n, cudaStream_t s);
 // d[br,b,r] = bias[row0 + r] (start of an identity pass: d = I . b_k), or 0 when bias == nullptr.
 void launch_init_d(float* d, const float* bias, int row0, int B, int R, cudaStream_t s);
 // d[br,b,r] += sum_j A[br,b,r,j] * bias[j / bias_div]   (unfused bias of a Linear / Conv2d layer)
