@@ -64,6 +64,7 @@ def parse_args():
     ap.add_argument("--shard-rows", action="store_true",
                     help="NEXT-4 (opt-in, torchrun): all ranks work on the SAME batch; the identity rows of every intermediate "
                          "pass are sharded across ranks, one AllGather of (l_k, u_k) per layer (strong scaling)")
+    ap.add_argument("--no-conv-crown", action="store_true", help="cfg5: skip the CROWN-intermediate-bounds leg (NEXT-3)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--device-steps-only", action="store_true",
                     help="profiling aid (ncu): only the warm-up and the timed device steps of --workload; no TF32 peak "
@@ -82,11 +83,11 @@ def peaks():
     return {"hbm": 6650.0, "bf16": 1590.0, "bf16_sustained": 1400.0, "src": "fallback"}
 
 
-def kernel_source_sha1():
-    """sha1 over the CUDA sources: a committed ncu traffic figure is only quoted while the kernels are unchanged."""
+def kernel_source_sha1(files):
+    """sha1 over the CUDA sources a kernel is built from: a committed ncu traffic figure is only quoted while they are unchanged."""
     h = hashlib.sha1()
     d = os.path.join(ROOT, "paper_2606_09377_b200", "csrc")
-    for f in sorted(os.listdir(d)):
+    for f in sorted(files):
         with open(os.path.join(d, f), "rb") as fh:
             h.update(fh.read())
     return h.hexdigest()[:16]
@@ -94,14 +95,15 @@ def kernel_source_sha1():
 
 def profiled_traffic(cfgname, kernel):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed ncu --set full capture of
-    this workload (profiles/traffic.json), or None when there is none for the current kernel sources."""
+    this workload (profiles/traffic.json: {"cfgN:kernel": {dram_bytes_per_launch, src_files, src_sha1, profile}}), or None
+    when there is none for the current sources of that kernel."""
     p = os.path.join(ROOT, "profiles", "traffic.json")
     if not os.path.exists(p):
         return None
     with open(p) as f:
         tab = json.load(f)
     e = tab.get(f"{cfgname}:{kernel}")
-    if not e or e.get("src_sha1") != kernel_source_sha1():
+    if not e or e.get("src_sha1") != kernel_source_sha1(e.get("src_files", [])):
         return None
     return e["dram_bytes_per_launch"]
 
@@ -524,6 +526,23 @@ def measure_config(cfgname, args, steps, warmup, dev, local, world, tf32_peak, w
     if cfgname == "cfg2" and alpha is not None and args.bab_domains > 0 and args.scale == 1:
         bab = measure_bab(wl, ctx, io, args, dev, local)
 
+    # ---- NEXT-3: the same batch with full-CROWN intermediate bounds through the conv layers --------
+    conv_crown = None
+    if cfgname == "cfg5" and args.scale == 1 and not args.no_conv_crown:
+        io2 = ctx.alloc_io(B, S)
+        ms_c = []
+        for it in range(3):
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); ctx.run_device(xlo, xhi, Cd, alpha, 0, io2); e1.record(); e1.synchronize()
+            ms_c.append(e0.elapsed_time(e1))
+        w_ibp = (io["ub"] - io["lb"]).abs()
+        w_cr = (io2["ub"] - io2["lb"]).abs()
+        conv_crown = {"ms_per_step": min(ms_c), "properties_per_s": B / (min(ms_c) * 1e-3), "row_chunk": ctx.row_chunk(),
+                      "median_final_width_ratio_vs_ibp_intermediates": float((w_cr / w_ibp).median().item()),
+                      "verified": int(io2["verified"].sum().item())}
+        del io2
+
     peak_ws = ctx.peak_bytes()
     peak_torch = torch.cuda.max_memory_allocated(dev)
     rc_rows = ctx.row_chunk()
@@ -542,7 +561,7 @@ def measure_config(cfgname, args, steps, warmup, dev, local, world, tf32_peak, w
         "e2e": {"value": world * B / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                 "d2h_bytes_per_step": int(d2h), "ms_per_step": ms_e2e, "steps": n_aux},
         "gpu_launches": int(launches_per_step * steps), "gpu_launches_per_step": int(launches_per_step), "clocks": clocks,
-        "alpha_opt": alpha_opt, "bab_beta": bab}
+        "alpha_opt": alpha_opt, "bab_beta": bab, "conv_crown": conv_crown}
     ctx.close()
     del ctx, xlo, xhi, Cd, alpha, io, flush, wl
     gc.collect()
@@ -638,13 +657,13 @@ def run_b200(args):
             r = measure_config(c, args, st, 3, dev, local, world, tf32_peak, with_cpu)
             per[c] = {k: r[k] for k in ("value", "unit", "steps", "ms_per_step", "config", "verified_last_batch", "aw_tflops",
                                         "peak_hbm_gb", "kernel_time_shares", "kernel_classes", "roofline", "cpu_baseline",
-                                        "e2e", "gpu_launches_per_step", "clocks", "alpha_opt", "bab_beta")}
+                                        "e2e", "gpu_launches_per_step", "clocks", "alpha_opt", "bab_beta", "conv_crown")}
     if rank == 0:
         line = {"metric": METRIC, "value": main["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": main["ms_per_step"], "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32 (3xTF32 products, fp32 accumulate)", "data": "synthetic"}
         for k in ("config", "verified_last_batch", "aw_tflops", "aw_flops_per_step", "peak_hbm_gb", "kernel_time_shares",
-                  "kernel_classes", "roofline", "cpu_baseline", "e2e", "gpu_launches", "gpu_launches_per_step", "clocks", "alpha_opt", "bab_beta"):
+                  "kernel_classes", "roofline", "cpu_baseline", "e2e", "gpu_launches", "gpu_launches_per_step", "clocks", "alpha_opt", "bab_beta", "conv_crown"):
             line[k] = main[k]
         line["tf32_dense_peak_tflops"] = tf32_peak
         line["per_config"] = per

@@ -441,6 +441,129 @@ conv_bwd_1x1_kernel(const float* __restrict__ A, long long sBr, long long sB, lo
   }
 }
 
+// ---- a6, 3x3 / stride 2 / pad 1 (the down-sampling convolutions of a ResNet; h = 2 ho, w = 2 wo).
+// A thread owns the 2 x 2 block of INPUT pixels (2p..2p+1, 2q..2q+1) x CT input channels, i.e. one pixel of each of the four
+// stride-parity classes, so every thread runs the same 9 taps on the same 4 values of A_out:
+//   in(2p  ,2q  ) += W11 a(p,q)                          in(2p  ,2q+1) += W10 a(p,q+1) + W12 a(p,q)
+//   in(2p+1,2q  ) += W01 a(p+1,q) + W21 a(p,q)           in(2p+1,2q+1) += W00 a(p+1,q+1) + W02 a(p+1,q) + W20 a(p,q+1) + W22 a(p,q)
+// (y = 2p' + i - 1).  The generic tiled kernel gives a thread four pixels of ONE class: classes need 1, 2, 2 and 4 taps, so
+// with 16-thread classes half the lanes of every FFMA were idle (ncu: 16.0 active threads per FFMA on 32 -> 64 @ 8x8) and
+// with warp-sized classes the block waited for its 4-tap warps (profiles/r2_conv.md: 8 and 12.6 TFLOP/s).
+// Block = RB rows x CG channel groups x (ho * wo) pixel threads; A_out tiles (zero halo right / below) and the filter slice
+// [co][tap][ci] are staged COC output channels at a time.
+template <int CT>
+__global__ void __launch_bounds__(256, 2)
+conv_bwd_3x3s2_kernel(const float* __restrict__ A, long long sBr, long long sB, long long ld, int B, int R,
+                      const float* __restrict__ W, const float* __restrict__ addend, float* __restrict__ out,
+                      int c_in, int c_out, int ho, int wo, int COC, int CG, int RB) {
+  extern __shared__ __align__(16) float sm[];
+  const int cgct = CG * CT;
+  const int PT = ho * wo, PW = wo + 1, tile = (ho + 1) * PW;
+  float* Ws = sm;                                  // [COC][9][cgct]
+  float* As = sm + COC * 9 * cgct;                 // [RB][COC][tile]
+  const int tid = threadIdx.x;
+  const int pt = tid % PT, cg = (tid / PT) % CG, rb = tid / (PT * CG);
+  const bool active = rb < RB;
+  const long long rows = 2LL * B * R;
+  const long long m_base = (long long)blockIdx.x * RB;
+  const int ci_base = blockIdx.y * cgct;
+  const int p = pt / wo, q = pt % wo;
+  const int a_off = p * PW + q;
+  float acc[4][CT];
+#pragma unroll
+  for (int k = 0; k < 4; ++k)
+#pragma unroll
+    for (int c = 0; c < CT; ++c) acc[k][c] = 0.f;
+  for (int co0 = 0; co0 < c_out; co0 += COC) {
+    const int cc = min(COC, c_out - co0);
+    __syncthreads();                               // the previous chunk has been consumed
+    for (int idx = tid; idx < cc * 9 * cgct; idx += blockDim.x) {
+      const int c = idx % cgct, t2 = idx / cgct;
+      const int tap = t2 % 9, co = t2 / 9;
+      const int ci = ci_base + c;
+      Ws[idx] = ci < c_in ? __ldg(W + ((long long)(co0 + co) * c_in + ci) * 9 + tap) : 0.f;
+    }
+    for (int r_ = 0; r_ < RB; ++r_) {
+      const long long m = m_base + r_;
+      const float* base = nullptr;
+      if (m < rows) {
+        const int r = (int)(m % R);
+        const long long tt = m / R;
+        base = A + (tt / B) * sBr + (tt % B) * sB + (long long)r * ld + (long long)co0 * PT;
+      }
+      float* dst = As + (long long)r_ * COC * tile;
+      for (int idx = tid; idx < cc * tile; idx += blockDim.x) {
+        const int co = idx / tile, e = idx % tile;
+        const int y = e / PW, x = e % PW;
+        dst[idx] = (base && y < ho && x < wo) ? __ldg(base + (long long)co * PT + y * wo + x) : 0.f;
+      }
+    }
+    __syncthreads();
+    if (active) {
+      const float* ap = As + (long long)rb * COC * tile + a_off;
+      const float* wp = Ws + cg * CT;
+      for (int co = 0; co < cc; ++co, ap += tile, wp += 9 * cgct) {
+        const float a00 = ap[0], a01 = ap[1], a10 = ap[PW], a11 = ap[PW + 1];
+#pragma unroll
+        for (int c4 = 0; c4 < CT; c4 += 4) {
+          float4 w[9];
+#pragma unroll
+          for (int t = 0; t < 9; ++t) w[t] = *reinterpret_cast<const float4*>(wp + t * cgct + c4);
+#define CROWN_S2_STEP(C_, F_) \
+          acc[0][c4 + C_] = fmaf(w[4].F_, a00, acc[0][c4 + C_]); \
+          acc[1][c4 + C_] = fmaf(w[3].F_, a01, fmaf(w[5].F_, a00, acc[1][c4 + C_])); \
+          acc[2][c4 + C_] = fmaf(w[1].F_, a10, fmaf(w[7].F_, a00, acc[2][c4 + C_])); \
+          acc[3][c4 + C_] = fmaf(w[0].F_, a11, fmaf(w[2].F_, a10, fmaf(w[6].F_, a01, fmaf(w[8].F_, a00, acc[3][c4 + C_]))));
+          CROWN_S2_STEP(0, x) CROWN_S2_STEP(1, y) CROWN_S2_STEP(2, z) CROWN_S2_STEP(3, w)
+#undef CROWN_S2_STEP
+        }
+      }
+    }
+  }
+  const long long m = m_base + rb;
+  if (!active || m >= rows) return;
+  const int h = 2 * ho, w_ = 2 * wo;
+#pragma unroll
+  for (int c = 0; c < CT; ++c) {
+    const int ci = ci_base + cg * CT + c;
+    if (ci >= c_in) continue;
+    const long long o = ((m * c_in + ci) * h + 2 * p) * (long long)w_ + 2 * q;     // even: 8-byte aligned
+    float2 r0 = make_float2(acc[0][c], acc[1][c]), r1 = make_float2(acc[2][c], acc[3][c]);
+    if (addend) {
+      const float2 e0 = __ldg(reinterpret_cast<const float2*>(addend + o)), e1 = __ldg(reinterpret_cast<const float2*>(addend + o + w_));
+      r0.x += e0.x; r0.y += e0.y; r1.x += e1.x; r1.y += e1.y;
+    }
+    *reinterpret_cast<float2*>(out + o) = r0;
+    *reinterpret_cast<float2*>(out + o + w_) = r1;
+  }
+}
+
+static bool launch_conv_bwd_3x3s2(const AView& A, const float* W, const float* addend, float* out, int B, int R,
+                                  int c_in, int h, int w, int c_out, int pad, int ho, int wo, cudaStream_t s) {
+  if (pad != 1 || h != 2 * ho || w != 2 * wo || ho * wo > 256 || ho * wo < 16) return false;
+  if ((reinterpret_cast<uintptr_t>(out) & 7) || (addend && (reinterpret_cast<uintptr_t>(addend) & 7))) return false;
+  const int CT = (c_in % 16 == 0) ? 16 : 8;
+  const int PT = ho * wo;
+  const int groups = (c_in + CT - 1) / CT;
+  int CG = 256 / PT < groups ? 256 / PT : groups;
+  if (CG < 1) CG = 1;
+  int RB = 256 / (PT * CG);
+  if (RB < 1) RB = 1;
+  if (RB > 4) RB = 4;
+  const int tile = (ho + 1) * (wo + 1);
+  const size_t per_co = ((size_t)9 * CG * CT + (size_t)RB * tile) * sizeof(float);
+  int COC = (int)((44 * 1024) / per_co);
+  if (COC < 1) return false;
+  if (COC > c_out) COC = c_out;
+  const size_t smem = per_co * COC;
+  const long long rows = 2LL * B * R;
+  const int threads = ((PT * CG * RB + 31) / 32) * 32;
+  dim3 grid((unsigned)((rows + RB - 1) / RB), (unsigned)((groups + CG - 1) / CG));
+  if (CT == 16) conv_bwd_3x3s2_kernel<16><<<grid, threads, smem, s>>>(A.p, A.sBr, A.sB, A.ld, B, R, W, addend, out, c_in, c_out, ho, wo, COC, CG, RB);
+  else conv_bwd_3x3s2_kernel<8><<<grid, threads, smem, s>>>(A.p, A.sBr, A.sB, A.ld, B, R, W, addend, out, c_in, c_out, ho, wo, COC, CG, RB);
+  return true;
+}
+
 // rows / columns of the input map that no output pixel reaches (h > stride * ho) are zero-filled by this launcher's caller
 // contract: supported only when stride * ho >= h and stride * wo >= w, i.e. every input pixel belongs to some s x s block
 static bool launch_conv_bwd_1x1(const AView& A, const float* W, const float* addend, float* out, int B, int R,
@@ -478,6 +601,7 @@ void launch_conv_transpose(const AView& A, const float* W, const float* addend, 
     bool done = false;
     if (kh == 1 && kw == 1 && launch_conv_bwd_1x1(A, W, addend, out, B, R, c_in, h, w, c_out, stride, pad, ho, wo, s)) return;
     if (kh == 3 && kw == 3 && stride == 1) done = launch_conv_bwd_ct<3, 3, 1>(A, W, addend, out, B, R, c_in, h, w, c_out, pad, ho, wo, s);
+    else if (kh == 3 && kw == 3 && stride == 2 && launch_conv_bwd_3x3s2(A, W, addend, out, B, R, c_in, h, w, c_out, pad, ho, wo, s)) done = true;
     else if (kh == 3 && kw == 3 && stride == 2) done = launch_conv_bwd_ct<3, 3, 2>(A, W, addend, out, B, R, c_in, h, w, c_out, pad, ho, wo, s);
     else if (kh == 1 && kw == 1 && stride == 1) done = launch_conv_bwd_ct<1, 1, 1>(A, W, addend, out, B, R, c_in, h, w, c_out, pad, ho, wo, s);
     else if (kh == 1 && kw == 1 && stride == 2) done = launch_conv_bwd_ct<1, 1, 2>(A, W, addend, out, B, R, c_in, h, w, c_out, pad, ho, wo, s);
