@@ -232,12 +232,17 @@ conv_bwd_tiled_kernel(const float* __restrict__ A, long long sBr, long long sB, 
       if (base == nullptr) continue;
       base += (long long)co0 * g.ho * g.wo;
       float* dst = As + r_ * g.COC * tile;
-      for (int co = 0; co < cc; ++co) {
+      if (tile <= (int)blockDim.x) {      // small maps (8x8: 100 elements): one slot per thread, not six predicated ones
+        for (int co = 0; co < cc; ++co, base += g.ho * g.wo, dst += tile)
+          if (soff[0] >= 0) cp_async4(dst + doff[0], base + soff[0]);
+      } else {
+        for (int co = 0; co < cc; ++co) {
 #pragma unroll
-        for (int k = 0; k < kConvFillMax; ++k)
-          if (soff[k] >= 0) cp_async4(dst + doff[k], base + soff[k]);
-        base += g.ho * g.wo;
-        dst += tile;
+          for (int k = 0; k < kConvFillMax; ++k)
+            if (soff[k] >= 0) cp_async4(dst + doff[k], base + soff[k]);
+          base += g.ho * g.wo;
+          dst += tile;
+        }
       }
     }
     cp_async_commit();
@@ -391,9 +396,9 @@ template <int CIP>
 __global__ void __launch_bounds__(256)
 conv_bwd_1x1_kernel(const float* __restrict__ A, long long sBr, long long sB, long long ld, int B, int R,
                     const float* __restrict__ W, const float* __restrict__ addend, float* __restrict__ out,
-                    int c_in, int h, int w, int c_out, int stride, int ho, int wo, int PIX) {
+                    int c_in, int h, int w, int c_out, int stride, int ho, int wo, int PIX, int vec) {
   extern __shared__ __align__(16) float sm[];
-  float* Ws = sm;                          // [c_out][c_in]
+  float* Ws = sm;                          // [c_out][c_in]  (c_out * c_in is a multiple of 4 when vec: As stays 16-byte aligned)
   float* As = sm + c_out * c_in;           // [c_out][PIX]
   const long long m = blockIdx.y;
   const int pix0 = blockIdx.x * PIX;
@@ -403,9 +408,25 @@ conv_bwd_1x1_kernel(const float* __restrict__ A, long long sBr, long long sB, lo
     const int r = (int)(m % R);
     const long long tt = m / R;
     const float* a = A + (tt / B) * sBr + (tt % B) * sB + (long long)r * ld;
-    for (int i = threadIdx.x; i < c_out * PIX; i += blockDim.x) {
-      const int co = i / PIX, p = i % PIX;
-      As[i] = (pix0 + p < npix) ? __ldg(a + (long long)co * npix + pix0 + p) : 0.f;
+    if (vec) {       // 16-byte asynchronous copies, all in flight at once (the tile is c_out contiguous runs of PIX floats)
+      const int q4 = PIX >> 2;
+      for (int i = threadIdx.x; i < c_out * q4; i += blockDim.x) {
+        const int co = i / q4, p4 = (i % q4) << 2;
+        float* dst = As + co * PIX + p4;
+        if (pix0 + p4 < npix) {
+          const uint32_t d = static_cast<uint32_t>(__cvta_generic_to_shared(dst));
+          asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(d), "l"(a + (long long)co * npix + pix0 + p4) : "memory");
+        } else {
+          *reinterpret_cast<float4*>(dst) = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+      }
+      cp_async_commit();
+      cp_async_wait<0>();
+    } else {
+      for (int i = threadIdx.x; i < c_out * PIX; i += blockDim.x) {
+        const int co = i / PIX, p = i % PIX;
+        As[i] = (pix0 + p < npix) ? __ldg(a + (long long)co * npix + pix0 + p) : 0.f;
+      }
     }
   }
   __syncthreads();
@@ -455,12 +476,12 @@ template <int CT>
 __global__ void __launch_bounds__(256, 2)
 conv_bwd_3x3s2_kernel(const float* __restrict__ A, long long sBr, long long sB, long long ld, int B, int R,
                       const float* __restrict__ W, const float* __restrict__ addend, float* __restrict__ out,
-                      int c_in, int c_out, int ho, int wo, int COC, int CG, int RB) {
+                      int c_in, int c_out, int ho, int wo, int COC, int CG, int RB, int stage_floats) {
   extern __shared__ __align__(16) float sm[];
+  __shared__ const float* rowp[4];
   const int cgct = CG * CT;
   const int PT = ho * wo, PW = wo + 1, tile = (ho + 1) * PW;
-  float* Ws = sm;                                  // [COC][9][cgct]
-  float* As = sm + COC * 9 * cgct;                 // [RB][COC][tile]
+  const int w_floats = COC * 9 * cgct;             // stage layout: Ws [COC][9][cgct], then As [RB][COC][tile]
   const int tid = threadIdx.x;
   const int pt = tid % PT, cg = (tid / PT) % CG, rb = tid / (PT * CG);
   const bool active = rb < RB;
@@ -469,38 +490,66 @@ conv_bwd_3x3s2_kernel(const float* __restrict__ A, long long sBr, long long sB, 
   const int ci_base = blockIdx.y * cgct;
   const int p = pt / wo, q = pt % wo;
   const int a_off = p * PW + q;
+  if (tid < RB) {
+    const long long m = m_base + tid;
+    const float* ptr = nullptr;
+    if (m < rows) {
+      const int r = (int)(m % R);
+      const long long tt = m / R;
+      ptr = A + (tt / B) * sBr + (tt % B) * sB + (long long)r * ld;
+    }
+    rowp[tid] = ptr;
+  }
+  // both stages zeroed once: the halo column / row (and rows past the end) stay zero, the copies touch the interior only
+  for (int i = tid; i < 2 * stage_floats; i += blockDim.x) sm[i] = 0.f;
+  int soff[2];                                      // this thread's (up to two) elements of a (row, co) tile
+#pragma unroll
+  for (int k = 0; k < 2; ++k) {
+    const int e = tid + k * (int)blockDim.x;
+    const int y = e / PW, x = e % PW;
+    soff[k] = (e < tile && y < ho && x < wo) ? y * wo + x : -1;
+  }
+  __syncthreads();
+  // asynchronous staging (cp.async, 4-byte copies: the halo shifts alignment), double-buffered
+  auto fill = [&](int co0, int stage) {
+    float* Ws = sm + stage * stage_floats;
+    float* As = Ws + w_floats;
+    const int cc = min(COC, c_out - co0);
+    for (int idx = tid; idx < cc * 9 * cgct; idx += blockDim.x) {
+      const int c = idx % cgct, t2 = idx / cgct;
+      const int tap = t2 % 9, co = t2 / 9;
+      const int ci = ci_base + c;
+      if (ci < c_in) cp_async4(Ws + idx, W + ((long long)(co0 + co) * c_in + ci) * 9 + tap);
+    }
+    for (int r_ = 0; r_ < RB; ++r_) {
+      const float* base = rowp[r_];
+      if (base == nullptr) continue;
+      base += (long long)co0 * PT;
+      float* dst = As + r_ * COC * tile;
+      for (int co = 0; co < cc; ++co, base += PT, dst += tile) {
+#pragma unroll
+        for (int k = 0; k < 2; ++k)
+          if (soff[k] >= 0) cp_async4(dst + tid + k * (int)blockDim.x, base + soff[k]);
+      }
+    }
+    cp_async_commit();
+  };
   float acc[4][CT];
 #pragma unroll
   for (int k = 0; k < 4; ++k)
 #pragma unroll
     for (int c = 0; c < CT; ++c) acc[k][c] = 0.f;
-  for (int co0 = 0; co0 < c_out; co0 += COC) {
-    const int cc = min(COC, c_out - co0);
-    __syncthreads();                               // the previous chunk has been consumed
-    for (int idx = tid; idx < cc * 9 * cgct; idx += blockDim.x) {
-      const int c = idx % cgct, t2 = idx / cgct;
-      const int tap = t2 % 9, co = t2 / 9;
-      const int ci = ci_base + c;
-      Ws[idx] = ci < c_in ? __ldg(W + ((long long)(co0 + co) * c_in + ci) * 9 + tap) : 0.f;
-    }
-    for (int r_ = 0; r_ < RB; ++r_) {
-      const long long m = m_base + r_;
-      const float* base = nullptr;
-      if (m < rows) {
-        const int r = (int)(m % R);
-        const long long tt = m / R;
-        base = A + (tt / B) * sBr + (tt % B) * sB + (long long)r * ld + (long long)co0 * PT;
-      }
-      float* dst = As + (long long)r_ * COC * tile;
-      for (int idx = tid; idx < cc * tile; idx += blockDim.x) {
-        const int co = idx / tile, e = idx % tile;
-        const int y = e / PW, x = e % PW;
-        dst[idx] = (base && y < ho && x < wo) ? __ldg(base + (long long)co * PT + y * wo + x) : 0.f;
-      }
-    }
+  const int nchunks = (c_out + COC - 1) / COC;
+  fill(0, 0);
+  for (int ch = 0; ch < nchunks; ++ch) {
+    const int stage = ch & 1;
+    if (ch + 1 < nchunks) { fill((ch + 1) * COC, stage ^ 1); cp_async_wait<1>(); }
+    else cp_async_wait<0>();
     __syncthreads();
     if (active) {
-      const float* ap = As + (long long)rb * COC * tile + a_off;
+      const int cc = min(COC, c_out - ch * COC);
+      const float* Ws = sm + stage * stage_floats;
+      const float* ap = Ws + w_floats + rb * COC * tile + a_off;
       const float* wp = Ws + cg * CT;
       for (int co = 0; co < cc; ++co, ap += tile, wp += 9 * cgct) {
         const float a00 = ap[0], a01 = ap[1], a10 = ap[PW], a11 = ap[PW + 1];
@@ -519,6 +568,7 @@ conv_bwd_3x3s2_kernel(const float* __restrict__ A, long long sBr, long long sB, 
         }
       }
     }
+    __syncthreads();      // the stage is refilled by the next iteration's fill
   }
   const long long m = m_base + rb;
   if (!active || m >= rows) return;
@@ -551,16 +601,18 @@ static bool launch_conv_bwd_3x3s2(const AView& A, const float* W, const float* a
   if (RB < 1) RB = 1;
   if (RB > 4) RB = 4;
   const int tile = (ho + 1) * (wo + 1);
+  if (tile > 2 * 256) return false;
   const size_t per_co = ((size_t)9 * CG * CT + (size_t)RB * tile) * sizeof(float);
-  int COC = (int)((44 * 1024) / per_co);
+  int COC = (int)((44 * 1024) / per_co);           // two stages of <= 44 KB, two blocks per SM
   if (COC < 1) return false;
   if (COC > c_out) COC = c_out;
-  const size_t smem = per_co * COC;
+  const int stage_floats = (int)((per_co * COC / sizeof(float) + 3) / 4 * 4);
+  const size_t smem = (size_t)2 * stage_floats * sizeof(float);
   const long long rows = 2LL * B * R;
-  const int threads = ((PT * CG * RB + 31) / 32) * 32;
+  const int threads = 256;                          // the element -> thread map of the staging assumes blockDim = 256
   dim3 grid((unsigned)((rows + RB - 1) / RB), (unsigned)((groups + CG - 1) / CG));
-  if (CT == 16) conv_bwd_3x3s2_kernel<16><<<grid, threads, smem, s>>>(A.p, A.sBr, A.sB, A.ld, B, R, W, addend, out, c_in, c_out, ho, wo, COC, CG, RB);
-  else conv_bwd_3x3s2_kernel<8><<<grid, threads, smem, s>>>(A.p, A.sBr, A.sB, A.ld, B, R, W, addend, out, c_in, c_out, ho, wo, COC, CG, RB);
+  if (CT == 16) conv_bwd_3x3s2_kernel<16><<<grid, threads, smem, s>>>(A.p, A.sBr, A.sB, A.ld, B, R, W, addend, out, c_in, c_out, ho, wo, COC, CG, RB, stage_floats);
+  else conv_bwd_3x3s2_kernel<8><<<grid, threads, smem, s>>>(A.p, A.sBr, A.sB, A.ld, B, R, W, addend, out, c_in, c_out, ho, wo, COC, CG, RB, stage_floats);
   return true;
 }
 
@@ -581,8 +633,10 @@ static bool launch_conv_bwd_1x1(const AView& A, const float* W, const float* add
   const size_t smem = ((size_t)c_out * c_in + (size_t)c_out * PIX) * sizeof(float);
   if (smem > 96 * 1024) return false;
   dim3 grid((unsigned)((npix + PIX - 1) / PIX), (unsigned)rows);
+  const int vec = (npix % 4 == 0) && (PIX % 4 == 0) && ((c_out * c_in) % 4 == 0) && (A.ld % 4 == 0) && (A.sB % 4 == 0) &&
+                  (A.sBr % 4 == 0) && ((reinterpret_cast<uintptr_t>(A.p) & 15) == 0);
   auto go = [&](auto kern) {
-    kern<<<grid, 256, smem, s>>>(A.p, A.sBr, A.sB, A.ld, B, R, W, addend, out, c_in, h, w, c_out, stride, ho, wo, PIX);
+    kern<<<grid, 256, smem, s>>>(A.p, A.sBr, A.sB, A.ld, B, R, W, addend, out, c_in, h, w, c_out, stride, ho, wo, PIX, vec);
   };
   if (cip == 4) go(conv_bwd_1x1_kernel<4>);
   else if (cip == 8) go(conv_bwd_1x1_kernel<8>);
@@ -617,6 +671,8 @@ void launch_conv_transpose(const AView& A, const float* W, const float* addend, 
 
 int conv_init_device() {
   const int b1 = 96 * 1024;
+  if (cudaFuncSetAttribute(conv_bwd_3x3s2_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1) != cudaSuccess ||
+      cudaFuncSetAttribute(conv_bwd_3x3s2_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1) != cudaSuccess) return -1;
   if (cudaFuncSetAttribute(conv_bwd_1x1_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1) != cudaSuccess ||
       cudaFuncSetAttribute(conv_bwd_1x1_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1) != cudaSuccess ||
       cudaFuncSetAttribute(conv_bwd_1x1_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1) != cudaSuccess) return -1;
