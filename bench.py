@@ -55,6 +55,7 @@ def parse_args():
     ap.add_argument("--stream-weights", action="store_true",
                     help="layers with >= 2^28 weights are streamed from pinned host memory (a7), not resident")
     ap.add_argument("--no-epi-fusion", action="store_true", help="run the relaxation as its own kernel (debug)")
+    ap.add_argument("--k-drain", type=int, default=0, help="3xTF32 drain chunk (debug; 0 = library default)")
     ap.add_argument("--no-graph", action="store_true", help="do not replay crown_run from a CUDA graph (debug)")
     ap.add_argument("--no-conv-tc", action="store_true", help="BoundConv backward on the CUDA-core kernel everywhere (debug)")
     ap.add_argument("--alpha-iters", type=int, default=10,
@@ -355,7 +356,7 @@ def measure_config(cfgname, args, steps, warmup, dev, local, world, tf32_peak, w
     free0, _ = torch.cuda.mem_get_info(dev)
     ctx = CrownContext(wl.net, B, S, device=f"cuda:{local}", mem_cap_bytes=cap,
                        stream_weights=int(args.stream_weights), disable_epi_fusion=int(args.no_epi_fusion),
-                       disable_graph=int(args.no_graph), disable_conv_tc=int(args.no_conv_tc))
+                       disable_graph=int(args.no_graph), disable_conv_tc=int(args.no_conv_tc), k_drain=args.k_drain)
     inter = 1 if wl.intermediate == "ibp" else 0
 
     # ---- inputs resident in HBM -------------------------------------------------------------------

@@ -123,6 +123,7 @@ extern "C" int crown_destroy(crown_ctx* ctx) {
   for (auto e : ctx->free_events) cudaEventDestroy(e);
   for (auto& ni : ctx->nodes) { if (ni.hWt_hi) cudaFreeHost(ni.hWt_hi); if (ni.hWt_lo) cudaFreeHost(ni.hWt_lo); }
   for (int b = 0; b < 2; ++b) { if (ctx->ev_copied[b]) cudaEventDestroy(ctx->ev_copied[b]); if (ctx->ev_free[b]) cudaEventDestroy(ctx->ev_free[b]); }
+  if (ctx->hpack) cudaFreeHost(ctx->hpack);
   if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
   for (auto& g : ctx->graphs) if (g.exec) cudaGraphExecDestroy(g.exec);
   if (ctx->ev_gin) cudaEventDestroy(ctx->ev_gin);

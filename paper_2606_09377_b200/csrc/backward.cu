@@ -331,7 +331,9 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
           // kernel it measured the same as the separate sum pass
           const bool tc_conv = ctx->opts.mma_scheme == 0 && !ctx->opts.disable_conv_tc && !cur.v.lo &&
                                conv_tc_supported(nd.c_in, nd.h_in, nd.w_in, nd.c_out, nd.kh, nd.kw, nd.stride, nd.pad, ni.h, ni.w);
-          if (itp != ps.pend.end() && plain_node && tc_conv && !itp->second.v.lo && itp->second.v.n == in_size && itp->second.v.ld == in_size &&
+          const bool s2_conv = !cur.v.lo && conv_s2_supported(nd.c_in, nd.h_in, nd.w_in, nd.c_out, nd.kh, nd.kw, nd.stride, nd.pad, ni.h, ni.w) &&
+                               (2LL * B * R * in_size) % 2 == 0;
+          if (itp != ps.pend.end() && plain_node && (tc_conv || s2_conv) && !itp->second.v.lo && itp->second.v.n == in_size && itp->second.v.ld == in_size &&
               itp->second.v.sB == (long long)R * in_size && itp->second.v.sBr == (long long)B * R * in_size) {
             other = itp->second; addend = other.v.p; ps.pend.erase(itp);
           }
@@ -561,34 +563,79 @@ extern "C" int crown_run_host(crown_ctx* ctx, int B, const float* x_lo_host, con
   for (size_t k = 0; k < (size_t)B * ctx->n0; ++k)
     if (x_lo_host[k] > x_hi_host[k]) return fail(ctx, CROWN_EINVAL, "crown_run_host: x_lo > x_hi");
   cudaStream_t s = ctx->stream;
-  uint8_t* cur = ctx->io_base;
-  auto take = [&](size_t bytes) { uint8_t* p = cur; cur += align_up(bytes); return p; };
+  // staging layout inside the workspace: [inputs: alpha per ReLU, x_lo, x_hi, C] [l, u per ReLU] [outputs: lb, ub, verified]
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
+  std::vector<size_t> a_off(n, 0), l_off(n, 0), u_off(n, 0);
+  for (int i = 0; i < n; ++i)
+    if (ctx->nodes[i].n.op == CROWN_RELU) a_off[i] = take((size_t)ctx->B_max * ctx->S_max * ctx->nodes[i].size * 4);
+  const size_t nL = ctx->nodes.back().size;
+  const size_t xl_off = take((size_t)ctx->B_max * ctx->n0 * 4), xh_off = take((size_t)ctx->B_max * ctx->n0 * 4);
+  const size_t C_off = take((size_t)ctx->B_max * ctx->S_max * nL * 4);
+  const size_t in_bytes = off;
+  for (int i = 0; i < n; ++i)
+    if (ctx->nodes[i].n.op == CROWN_RELU) {
+      l_off[i] = take((size_t)ctx->B_max * ctx->nodes[i].size * 4);
+      u_off[i] = take((size_t)ctx->B_max * ctx->nodes[i].size * 4);
+    }
+  const size_t out0 = off;
+  const size_t lb_off = take((size_t)ctx->B_max * ctx->S_max * 4), ub_off = take((size_t)ctx->B_max * ctx->S_max * 4);
+  const size_t ver_off = take((size_t)ctx->B_max);
+  const size_t out_bytes = off - out0;
+  if (off > ctx->plan.io_bytes) return fail(ctx, CROWN_ENOMEM, "crown_run_host: staging region too small");
+  uint8_t* io = ctx->io_base;
+  // Small problems (cfg1: 25 KB in, 73 B out) are latency-bound on the NUMBER of copies: everything is packed into one
+  // pinned mirror of the staging region (allocated once) and moved by ONE copy per direction instead of 4 + 2 per ReLU.
+  constexpr size_t kPackMax = (size_t)1 << 20;
+  const bool pack = in_bytes + out_bytes <= kPackMax;
+  if (pack && !ctx->hpack) {
+    if (cudaHostAlloc(reinterpret_cast<void**>(&ctx->hpack), in_bytes + out_bytes, cudaHostAllocDefault) != cudaSuccess) {
+      (void)cudaGetLastError();
+      ctx->hpack = nullptr;
+    }
+  }
+  const bool packed = pack && ctx->hpack != nullptr;
   std::vector<float*> l(n, nullptr), u(n, nullptr);
   std::vector<const float*> al(n, nullptr);
   bool any_alpha = false;
   for (int i = 0; i < n; ++i) {
     if (ctx->nodes[i].n.op != CROWN_RELU) continue;
     const size_t sz = ctx->nodes[i].size;
-    float* a = reinterpret_cast<float*>(take((size_t)ctx->B_max * ctx->S_max * sz * 4));
-    l[i] = reinterpret_cast<float*>(take((size_t)ctx->B_max * sz * 4));
-    u[i] = reinterpret_cast<float*>(take((size_t)ctx->B_max * sz * 4));
+    l[i] = reinterpret_cast<float*>(io + l_off[i]);
+    u[i] = reinterpret_cast<float*>(io + u_off[i]);
     if (alpha_host && alpha_host[i]) {
-      CK(ctx, cudaMemcpyAsync(a, alpha_host[i], (size_t)B * S * sz * 4, cudaMemcpyHostToDevice, s));
-      al[i] = a; any_alpha = true;
+      if (packed) std::memcpy(ctx->hpack + a_off[i], alpha_host[i], (size_t)B * S * sz * 4);
+      else CK(ctx, cudaMemcpyAsync(io + a_off[i], alpha_host[i], (size_t)B * S * sz * 4, cudaMemcpyHostToDevice, s));
+      al[i] = reinterpret_cast<const float*>(io + a_off[i]); any_alpha = true;
     }
   }
-  float* xl = reinterpret_cast<float*>(take((size_t)ctx->B_max * ctx->n0 * 4));
-  float* xh = reinterpret_cast<float*>(take((size_t)ctx->B_max * ctx->n0 * 4));
-  const size_t nL = ctx->nodes.back().size;
-  float* C = reinterpret_cast<float*>(take((size_t)ctx->B_max * ctx->S_max * nL * 4));
-  float* lb = reinterpret_cast<float*>(take((size_t)ctx->B_max * ctx->S_max * 4));
-  float* ub = reinterpret_cast<float*>(take((size_t)ctx->B_max * ctx->S_max * 4));
-  uint8_t* ver = take((size_t)ctx->B_max);
-  CK(ctx, cudaMemcpyAsync(xl, x_lo_host, (size_t)B * ctx->n0 * 4, cudaMemcpyHostToDevice, s));
-  CK(ctx, cudaMemcpyAsync(xh, x_hi_host, (size_t)B * ctx->n0 * 4, cudaMemcpyHostToDevice, s));
-  CK(ctx, cudaMemcpyAsync(C, C_host, (size_t)B * S * nL * 4, cudaMemcpyHostToDevice, s));
+  float* xl = reinterpret_cast<float*>(io + xl_off);
+  float* xh = reinterpret_cast<float*>(io + xh_off);
+  float* C = reinterpret_cast<float*>(io + C_off);
+  float* lb = reinterpret_cast<float*>(io + lb_off);
+  float* ub = reinterpret_cast<float*>(io + ub_off);
+  uint8_t* ver = io + ver_off;
+  if (packed) {
+    std::memcpy(ctx->hpack + xl_off, x_lo_host, (size_t)B * ctx->n0 * 4);
+    std::memcpy(ctx->hpack + xh_off, x_hi_host, (size_t)B * ctx->n0 * 4);
+    std::memcpy(ctx->hpack + C_off, C_host, (size_t)B * S * nL * 4);
+    CK(ctx, cudaMemcpyAsync(io, ctx->hpack, in_bytes, cudaMemcpyHostToDevice, s));
+  } else {
+    CK(ctx, cudaMemcpyAsync(xl, x_lo_host, (size_t)B * ctx->n0 * 4, cudaMemcpyHostToDevice, s));
+    CK(ctx, cudaMemcpyAsync(xh, x_hi_host, (size_t)B * ctx->n0 * 4, cudaMemcpyHostToDevice, s));
+    CK(ctx, cudaMemcpyAsync(C, C_host, (size_t)B * S * nL * 4, cudaMemcpyHostToDevice, s));
+  }
   int rc = crown_run(ctx, B, xl, xh, C, S, any_alpha ? al.data() : nullptr, intermediate, l.data(), u.data(), lb, ub, ver);
   if (rc) return rc;
+  if (packed) {
+    uint8_t* ho = ctx->hpack + in_bytes;          // mirror of [out0, out0 + out_bytes)
+    CK(ctx, cudaMemcpyAsync(ho, io + out0, out_bytes, cudaMemcpyDeviceToHost, s));
+    CK(ctx, cudaStreamSynchronize(s));
+    std::memcpy(lb_host, ho + (lb_off - out0), (size_t)B * S * 4);
+    std::memcpy(ub_host, ho + (ub_off - out0), (size_t)B * S * 4);
+    if (verified_host) std::memcpy(verified_host, ho + (ver_off - out0), (size_t)B);
+    return CROWN_OK;
+  }
   CK(ctx, cudaMemcpyAsync(lb_host, lb, (size_t)B * S * 4, cudaMemcpyDeviceToHost, s));
   CK(ctx, cudaMemcpyAsync(ub_host, ub, (size_t)B * S * 4, cudaMemcpyDeviceToHost, s));
   if (verified_host) CK(ctx, cudaMemcpyAsync(verified_host, ver, (size_t)B, cudaMemcpyDeviceToHost, s));

@@ -588,9 +588,15 @@ conv_bwd_3x3s2_kernel(const float* __restrict__ A, long long sBr, long long sB, 
   }
 }
 
+int conv_s2_supported(int c_in, int h, int w, int c_out, int kh, int kw, int stride, int pad, int ho, int wo) {
+  (void)c_in; (void)c_out;
+  return kh == 3 && kw == 3 && stride == 2 && pad == 1 && h == 2 * ho && w == 2 * wo && ho * wo <= 256 && ho * wo >= 16 &&
+         (ho + 1) * (wo + 1) <= 512;
+}
+
 static bool launch_conv_bwd_3x3s2(const AView& A, const float* W, const float* addend, float* out, int B, int R,
                                   int c_in, int h, int w, int c_out, int pad, int ho, int wo, cudaStream_t s) {
-  if (pad != 1 || h != 2 * ho || w != 2 * wo || ho * wo > 256 || ho * wo < 16) return false;
+  if (!conv_s2_supported(c_in, h, w, c_out, 3, 3, 2, pad, ho, wo)) return false;
   if ((reinterpret_cast<uintptr_t>(out) & 7) || (addend && (reinterpret_cast<uintptr_t>(addend) & 7))) return false;
   const int CT = (c_in % 16 == 0) ? 16 : 8;
   const int PT = ho * wo;

@@ -67,6 +67,7 @@ struct crown_ctx {
   float* d_buf = nullptr;
   float* part_buf = nullptr;
   uint8_t* io_base = nullptr;
+  uint8_t* hpack = nullptr;        // pinned mirror of the host-call staging region (small problems only, crown_run_host)
   uint8_t* pool_base = nullptr;
   std::vector<int> pool_ref;
   size_t peak = 0;
@@ -190,6 +191,10 @@ int make_plan(const std::vector<NodeInfo>& nodes, int n0, int B, int S, const cr
         gemm_tc_single_panel(ni.n.n_out)) any_epi = true;
     nmax = std::max(nmax, ni.size);
     if (ni.n.op == CROWN_LINEAR && ni.n.in0 >= 0) max_start = std::max(max_start, ni.size);
+    // conv-shaped pre-activations (NEXT-3 identity passes) are chunked too; they ask for at most 512 rows per chunk so that
+    // a conv net whose CROWN intermediate bounds are never requested (cfg5 benchmark: IBP ones) does not pay for them
+    if (ni.n.op == CROWN_RELU && ni.n.in0 >= 0 && nodes[ni.n.in0].n.op != CROWN_LINEAR && nodes[ni.n.in0].n.in0 >= 0)
+      max_start = std::max(max_start, std::min(nodes[ni.n.in0].size, 512));
     if (is_streamed(ni.n, o)) {
       // staging must hold 128 rows of the prepacked operand (2 limbs x n_out) and 128 raw rows (n_in)
       size_t need = std::max((size_t)2 * 128 * ni.n.n_out * 4, (size_t)128 * ni.n.n_in * 4);

@@ -131,6 +131,8 @@ void launch_conv_transpose(const AView& A, const float* W, const float* addend, 
                            int B, int R, int c_in, int h, int w, int c_out, int kh, int kw,
                            int stride, int pad, int ho, int wo, cudaStream_t s, int allow_tc = 0, int num_sms = 148);
 int conv_tc_supported(int c_in, int h, int w, int c_out, int kh, int kw, int stride, int pad, int ho, int wo);
+// 3x3 / stride 2 / pad 1 layers with h = 2 ho take the specialised kernel of conv.cu, whose epilogue adds `addend` for free
+int conv_s2_supported(int c_in, int h, int w, int c_out, int kh, int kw, int stride, int pad, int ho, int wo);
 int launch_conv_transpose_tc(const AView& A, const float* W, const float* addend, float* out, int B, int R,
                              int c_in, int h, int w, int c_out, int num_sms, cudaStream_t s);
 

@@ -216,6 +216,27 @@ def test_host_entry_rejects_an_inverted_box():
         ctx.run_host(bad, hi, wl.C, wl.alpha, wl.intermediate, lb, ub, ver)
 
 
+@pytest.mark.parametrize("which", ["cfg1", "cfg2", "small_B1of3"])
+def test_host_entry_equals_device_entry_bitwise(which):
+    """crown_run_host (H2D / D2H inside; one packed copy per direction for small problems, direct copies above 1 MiB)
+    returns exactly what crown_run returns on resident tensors, also for B below B_max and on repeated calls"""
+    if which == "cfg1":
+        wl = W.make(1); Bmax = wl.B                      # 25 KB of inputs: packed path
+    elif which == "cfg2":
+        wl = W.make(2, B=24); Bmax = wl.B                # 1.4 MB of alpha: direct copies
+    else:
+        wl = W.small_mlp([6, 9, 7, 3], seed=43, B=1, eps=0.1); Bmax = 3
+    lo, hi = wl.box()
+    ctx = _ctx(wl.net, Bmax, wl.S)
+    ref = ctx.run(lo, hi, wl.C, wl.alpha, wl.intermediate)
+    for rep in range(2):
+        lb = np.full((wl.B, wl.S), np.nan, np.float32); ub = np.full_like(lb, np.nan); ver = np.full(wl.B, 7, np.uint8)
+        ctx.run_host(lo, hi, wl.C, wl.alpha, wl.intermediate, lb, ub, ver)
+        assert np.array_equal(lb, ref["lb"].cpu().numpy()) and np.array_equal(ub, ref["ub"].cpu().numpy())
+        assert np.array_equal(ver, ref["verified"].cpu().numpy())
+    ctx.close()
+
+
 # ------------------------------------------------------------------------------------------ graph shapes
 def _graph_workload(net, seed, B=2, eps=0.05, S=5):
     rng = np.random.Generator(np.random.PCG64(W.SEED_BASE + 5000 + seed))
