@@ -106,7 +106,7 @@ def profiled_traffic(cfgname, kernel):
     e = tab.get(f"{cfgname}:{kernel}")
     if not e or e.get("src_sha1") != kernel_source_sha1(e.get("src_files", [])):
         return None
-    return e["dram_bytes_per_launch"]
+    return {"dram_bytes_per_launch": e["dram_bytes_per_launch"], "launch": e.get("launch"), "profile": e.get("profile")}
 
 
 def workload_desc(wl, cfgname):
@@ -490,6 +490,10 @@ def measure_config(cfgname, args, steps, warmup, dev, local, world, tf32_peak, w
         ach = d["bytes"] / (d["ms"] * 1e-3) / 1e9
         roof = {"kernel": dom, "bound": "hbm", "achieved": ach, "peak": pk["hbm"], "unit": "GB/s",
                 "frac": ach / pk["hbm"], "traffic": profiled_traffic(cfgname, dom), "peak_source": f"{pk['src']} copy bandwidth"}
+    tr = roof.get("traffic")
+    if isinstance(tr, dict):          # numeric per-launch DRAM bytes of the committed ncu capture + which launch it was
+        roof["traffic"] = tr["dram_bytes_per_launch"]
+        roof["traffic_from"] = {"launch": tr["launch"], "profile": tr["profile"]}
     roof["avg_launch_ms"] = avg_ms
     roof["launches_per_step"] = d["launches"] / n_aux
     roof["share_of_kernel_time"] = shares.get(dom)

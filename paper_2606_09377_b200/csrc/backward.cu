@@ -338,6 +338,19 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
             other = itp->second; addend = other.v.p; ps.pend.erase(itp);
           }
         }
+        // rows still shared by all branches and properties (the first hops of an identity pass on a conv map, NEXT-3) are
+        // transposed ONCE: the R rows run as a B = 1 problem whose "upper branch" is the second half of the rows
+        const bool shared_rows = cur.v.sB == 0 && cur.v.sBr == 0 && !cur.v.lo && !addend && (R % 2) == 0 && B * 2 > 1;
+        if (shared_rows) {
+          AView v2 = cur.v; v2.sBr = (long long)(R / 2) * cur.v.ld;
+          { Scope sc(ctx, CROWN_K_CONV, 4.0 * R * ((double)ni.size + in_size), 2.0 * R * (double)ni.size * nd.c_in * nd.kh * nd.kw);
+            launch_conv_transpose(v2, nd.W_dev, nullptr, D, 1, R / 2, nd.c_in, nd.h_in, nd.w_in, nd.c_out, nd.kh, nd.kw,
+                                  nd.stride, nd.pad, ni.h, ni.w, s, ctx->opts.mma_scheme == 0 && !ctx->opts.disable_conv_tc, ctx->num_sms); }
+          out.v.p = D; out.v.ld = in_size; out.v.n = in_size; out.v.sB = 0; out.v.sBr = 0;
+          release(ctx, cur);
+          rc = contribute(ps, nd.in0, out);
+          break;
+        }
         { Scope sc(ctx, CROWN_K_CONV, 4.0 * 2 * B * R * ((double)ni.size + in_size * (addend ? 2.0 : 1.0)),
                    2.0 * 2 * B * R * (double)ni.size * nd.c_in * nd.kh * nd.kw);
           launch_conv_transpose(cur.v, nd.W_dev, addend, D, B, R, nd.c_in, nd.h_in, nd.w_in, nd.c_out, nd.kh, nd.kw,

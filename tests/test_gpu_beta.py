@@ -273,3 +273,68 @@ def test_beta_errors():
         ctx.beta_ascent_device(l, u, ctx._split_dev(sd["split"]), ctx._dev(sd["C"]), t(sd["al"]), t(sd["au"]), bl, bl,
                                ctx._dev(sd["lo"]), ctx._dev(sd["hi"]), 0.1, 0.1, 1.0, 2, 1, o)
     ctx.close()
+
+
+def test_branch_and_bound_loop_with_gpu_bounds_against_brute_force():
+    """The batched sub-domain bounding inside an actual BaB loop (split, re-bound, repeat).  The loop itself
+    (which neuron to split, the domain list) is host logic of the TEST; every bound comes from crown_beta_ascent on the
+    whole frontier as ONE batch.  On nets small enough for brute force: every leaf's bound is sound against the exact minimum
+    over that leaf, the global lower bound (min over the leaves, which cover the box) is sound at every depth, and a leaf is
+    only ever declared verified when the exact minimum over it is positive.  (Tightness is not asserted: with a finite number
+    of ascent steps from beta = 0 a child can start below its parent; weak duality is what must always hold.)"""
+    from oracle import brute_force as BF
+    n_leaves = []
+    for seed in (51, 52, 53):
+        wl = W.small_mlp([2, 6, 5, 2], seed=seed, B=1, eps=0.7, S=2)
+        lo, hi = wl.box()
+        net, C = wl.net, wl.C[0]
+        exact_min, _ = BF.exact_range(net, lo[0], hi[0], C)
+        relus = net.relu_ids()
+        Bmax = 64
+        ctx = _ctx(net, Bmax, wl.S)
+        root = ctx.run(lo, hi, wl.C, None, wl.intermediate)
+        pre0 = {i: (_np(root["pre"][i][0])[0], _np(root["pre"][i][1])[0]) for i in relus}
+        frontier = [{i: np.zeros(net.nodes[i].size, np.int8) for i in relus}]      # split vectors of the open leaves
+        glb_hist = []
+        for depth in range(5):
+            nb = len(frontier)
+            assert nb <= Bmax
+            rep = lambda v: np.repeat(v[None], nb, axis=0)
+            pre = {i: (rep(pre0[i][0]), rep(pre0[i][1])) for i in relus}
+            split = {i: np.stack([f[i] for f in frontier]) for i in relus}
+            mk = lambda v: {i: np.full((nb, wl.S, net.nodes[i].size), v, np.float32) for i in relus}
+            out = ctx.beta_ascent(pre, split, rep(C), mk(0.5), mk(0.5), mk(0.0), mk(0.0), (rep(lo[0]), rep(hi[0])),
+                                  0.05, 0.1, 40, "sign", 0.97)
+            lbb = _np(out["lb_best"]).astype(np.float64)
+            ver = _np(out["verified"]).astype(bool)
+            # soundness of every leaf bound against the exact minimum over that leaf (skip empty leaves)
+            for e, f in enumerate(frontier):
+                mn, _ = BF.exact_range(net, lo[0], hi[0], C, split=f)
+                if np.all(np.isfinite(mn)):
+                    assert np.all(lbb[e] <= mn + 1e-5 + 1e-4 * np.abs(mn)), (seed, depth, e, lbb[e], mn)
+                    if ver[e]:
+                        assert np.all(mn > 0)
+            glb = lbb.min(axis=0)                      # a valid lower bound of the whole box: the leaves cover it
+            assert np.all(glb <= exact_min + 1e-5 + 1e-4 * np.abs(exact_min))
+            glb_hist.append(glb)
+            # branch: every open leaf splits its unstable, unsplit neuron with the widest relaxation gap (-l u / (u - l))
+            nxt = []
+            for e, f in enumerate(frontier):
+                best, score = None, 0.0
+                for i in relus:
+                    l, u = pre0[i]
+                    gap = np.where((l < 0) & (u > 0) & (f[i] == 0), -l * u / np.maximum(u - l, 1e-30), 0.0)
+                    j = int(np.argmax(gap))
+                    if gap[j] > score:
+                        best, score = (i, j), float(gap[j])
+                if best is None or ver[e]:
+                    nxt.append(f)                      # fully split or verified: stays a leaf
+                    continue
+                for sg in (1, -1):
+                    c = {i: v.copy() for i, v in f.items()}
+                    c[best[0]][best[1]] = sg
+                    nxt.append(c)
+            frontier = nxt
+        n_leaves.append(len(frontier))
+        ctx.close()
+    assert max(n_leaves) >= 16            # the frontier really grew into a batch of sub-domains
