@@ -72,7 +72,12 @@ extern "C" int crown_init(crown_ctx** out, const crown_node* nodes, int n_nodes,
           cudaEventCreateWithFlags(&ctx->ev_free[b], cudaEventDisableTiming) != cudaSuccess) return bail(CROWN_ECUDA);
   }
   ctx->coef_base = cur; ctx->coef_off.assign(n_nodes, 0);
-  { size_t off = 0; for (int i = 0; i < n_nodes; ++i) if (ctx->nodes[i].n.op == CROWN_RELU) { ctx->coef_off[i] = off; off += align_up((size_t)B_max * ctx->nodes[i].size * 16); } cur += ctx->plan.coef_bytes; }
+  { size_t off = 0;
+    for (int i = 0; i < n_nodes; ++i) {
+      if (ctx->nodes[i].n.op == CROWN_RELU) { ctx->coef_off[i] = off; off += align_up((size_t)B_max * ctx->nodes[i].size * 16); }
+      if (ctx->nodes[i].n.op == CROWN_ADD) { ctx->coef_off[i] = off; off += align_up((size_t)ctx->nodes[i].c * 4); }
+    }
+    cur += ctx->plan.coef_bytes; }
   ctx->ibp_base = cur; ctx->ibp_off.assign(n_nodes, 0);
   { size_t off = 0; for (int i = 0; i < n_nodes; ++i) { ctx->ibp_off[i] = off; off += 2 * align_up((size_t)B_max * ctx->nodes[i].size * 4); } cur += ctx->plan.ibp_bytes; }
   ctx->d_buf = reinterpret_cast<float*>(cur); cur += ctx->plan.d_bytes;
@@ -81,6 +86,28 @@ extern "C" int crown_init(crown_ctx** out, const crown_node* nodes, int n_nodes,
   ctx->pool_base = cur;
   ctx->pool_ref.assign(ctx->plan.nbuf, 0);
   ctx->peak = (size_t)(ctx->pool_base - ctx->ws);
+  // residual Add nodes fed by convolutions: the sum of the operands' biases per channel, so that the relaxation kernel of
+  // the ReLU above the Add accumulates d += Abar . (b_in0 + b_in1) in the pass it makes anyway (a6: the Add fans the same A
+  // out to both operands) instead of one extra pass over A per conv operand
+  ctx->add_bias_ok.assign(n_nodes, 0);
+  for (int i = 0; i < n_nodes; ++i) {
+    const NodeInfo& ni = ctx->nodes[i];
+    if (ni.n.op != CROWN_ADD || ni.h * ni.w <= 0) continue;
+    const float* b0 = nullptr; const float* b1 = nullptr;
+    bool any = false, ok = true;
+    for (int k = 0; k < 2; ++k) {
+      const int src = k == 0 ? ni.n.in0 : ni.n.in1;
+      if (src < 0) continue;
+      const NodeInfo& sn = ctx->nodes[src];
+      if (sn.n.op == CROWN_CONV2D) { (k == 0 ? b0 : b1) = sn.n.b_dev; any = true; if (sn.c != ni.c || sn.h != ni.h || sn.w != ni.w) ok = false; }
+      else if (sn.n.op == CROWN_LINEAR) ok = false;         // Linear operands keep their own bias pass
+    }
+    if (ni.n.in0 == ni.n.in1) ok = false;
+    if (!any || !ok) continue;
+    Scope sc(ctx, CROWN_K_MISC);
+    launch_bias_sum(b0, b1, reinterpret_cast<float*>(ctx->coef_base + ctx->coef_off[i]), ni.c, ctx->stream);
+    ctx->add_bias_ok[i] = 1;
+  }
   // prepack: transpose + TF32 split of every GEMM weight operand (one pass over W)
   for (auto& ni : ctx->nodes) {
     if (!ni.tc_ok || ni.streamed) continue;

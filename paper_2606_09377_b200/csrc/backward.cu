@@ -195,6 +195,14 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
         ra.alpha_up = alpha_up ? alpha_up[i] : nullptr;
         ra.bias = lin_below ? ctx->nodes[j].n.b_dev : nullptr;
         ra.bias_div = (lin_below && ctx->nodes[j].n.op == CROWN_CONV2D) ? ctx->nodes[j].h * ctx->nodes[j].w : 1;
+        // ReLU over a residual Add of convolutions: the Add hands the same A to both operands, so their biases are
+        // accumulated here as one summed vector (crown_init) and the operands' own bias passes are skipped
+        const bool add_below = j >= 0 && ctx->nodes[j].n.op == CROWN_ADD && ctx->add_bias_ok[j] && ctx->nodes[j].n_consumers == 1 &&
+                               ps.pend.find(j) == ps.pend.end();
+        if (add_below) {
+          ra.bias = reinterpret_cast<const float*>(ctx->coef_base + ctx->coef_off[j]);
+          ra.bias_div = ctx->nodes[j].h * ctx->nodes[j].w;
+        }
         ra.d = ctx->d_buf; ra.B = B; ra.R = R; ra.n = ni.size;
         if (sp && sp->split && sp->split[i]) {
           ra.split = sp->split[i];
@@ -215,7 +223,7 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
                                        ((ra.beta_lo ? 4.0 : 0.0) + (ra.beta_up && ra.beta_up != ra.beta_lo ? 4.0 : 0.0)) * B * R * ni.size);
           launch_relax(ra, s); }
         out.v = canon_view(ra.out, B, R, ni.size); out.v.lo = ra.out_lo;
-        out.bias_done_for = lin_below ? j : -2;
+        out.bias_done_for = (lin_below || add_below) ? j : -2;
         release(ctx, cur);
         rc = contribute(ps, j, out);
         break; }
@@ -363,6 +371,13 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
       case CROWN_ADD: {
         Pending second = cur;
         pool_retain(ctx, second.buf); pool_retain(ctx, second.buf_lo);
+        {
+          // the summed bias of the conv operands went into d with the relaxation above this Add (see CROWN_RELU)
+          const bool done = cur.bias_done_for == i && ctx->add_bias_ok[i];
+          auto mark = [&](int src) { return (done && src >= 0 && ctx->nodes[src].n.op == CROWN_CONV2D) ? src : -2; };
+          cur.bias_done_for = mark(nd.in0);
+          second.bias_done_for = mark(nd.in1);
+        }
         rc = contribute(ps, nd.in0, cur);
         if (rc == CROWN_OK) rc = contribute(ps, nd.in1, second);
         break; }

@@ -62,7 +62,8 @@ struct crown_ctx {
   size_t ws_bytes = 0;
   Plan plan;
   // carved regions
-  uint8_t* coef_base = nullptr; std::vector<size_t> coef_off;   // per node (ReLU only)
+  uint8_t* coef_base = nullptr; std::vector<size_t> coef_off;   // per node: ReLU coefficient records; Add: summed conv biases
+  std::vector<char> add_bias_ok;                                // per node: the Add's operands' biases are in its vector
   uint8_t* ibp_base = nullptr;  std::vector<size_t> ibp_off;    // per node: l then u
   float* d_buf = nullptr;
   float* part_buf = nullptr;
@@ -202,6 +203,7 @@ int make_plan(const std::vector<NodeInfo>& nodes, int n0, int B, int S, const cr
       p.stage_bytes = std::max(p.stage_bytes, std::max(need, std::min(full, o.stream_stage_bytes ? (size_t)o.stream_stage_bytes : kStageBytesMax)));
     } else if (wants_prepack(ni, o)) p.prepack_bytes += 2 * align_up((size_t)ni.n.n_in * ni.n.n_out * 4);
     if (ni.n.op == CROWN_RELU) p.coef_bytes += align_up((size_t)B * ni.size * 16);   // float4 records {dU, bU, dL, unstable}
+    if (ni.n.op == CROWN_ADD) p.coef_bytes += align_up((size_t)ni.c * 4);            // summed biases of its conv operands
     p.ibp_bytes += 2 * align_up((size_t)B * ni.size * 4);
     if (ni.n.op == CROWN_RELU) p.io_bytes += align_up((size_t)B * S * ni.size * 4) + 2 * align_up((size_t)B * ni.size * 4);
   }

@@ -500,6 +500,15 @@ void launch_onehot(float* out, int row0, int R, int n, cudaStream_t s) {
   else onehot_scalar_kernel<<<ceil_div(cnt, 256), 256, 0, s>>>(out, row0, R, n);
 }
 
+__global__ void bias_sum_kernel(const float* a, const float* b, float* out, int n) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) out[i] = (a ? a[i] : 0.f) + (b ? b[i] : 0.f);
+}
+void launch_bias_sum(const float* a, const float* b, float* out, int n, cudaStream_t s) {
+  if (n <= 0) return;
+  bias_sum_kernel<<<ceil_div(n, 128), 128, 0, s>>>(a, b, out, n);
+}
+
 void launch_verdict(const float* lb, uint8_t* verified, int B, int S, cudaStream_t s) {
   if (B <= 0) return;
   verdict_kernel<<<ceil_div(B, 128), 128, 0, s>>>(lb, verified, B, S);

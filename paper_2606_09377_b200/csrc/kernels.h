@@ -68,6 +68,8 @@ void launch_init_d(float* d, const float* bias, int row0, int B, int R, cudaStre
 // d[br,b,r] += sum_j A[br,b,r,j] * bias[j / bias_div]   (unfused bias of a Linear / Conv2d layer)
 void launch_rowdot_bias(const AView& A, const float* bias, int bias_div, float* d, int B, int R,
                         cudaStream_t s);
+// out[c] = (a ? a[c] : 0) + (b ? b[c] : 0), c < n (summed conv biases of a residual Add's operands; crown_init)
+void launch_bias_sum(const float* a, const float* b, float* out, int n, cudaStream_t s);
 // out[2,B,R,n] contiguous = view a (+ view b)
 void launch_view_add(const AView& a, const AView* b, float* out, int B, int R, cudaStream_t s);
 // a9 -- verdict: verified[b] = min_s lb[b,s] > 0
