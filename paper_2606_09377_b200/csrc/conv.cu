@@ -588,6 +588,157 @@ conv_bwd_3x3s2_kernel(const float* __restrict__ A, long long sBr, long long sB, 
   }
 }
 
+// ---- a6, 3x3 / stride 1 / pad 1 with w % 4 == 0 and h * w / 4 <= 256 (the 32x32, 16x16 and 8x8 maps of a ResNet).
+// A thread owns a strip of FOUR ADJACENT pixels (y, 4q .. 4q+3) x CT input channels.  Per output channel it reads, for each
+// of the three image rows y-1 .. y+1, one aligned float4 and the two neighbours left and right of it (the tile is stored with
+// a 4-column left pad, so column 4q is 16-byte aligned) -- 9 shared-memory loads of A feed all 9 taps of all 4 pixels:
+//   in(y, 4q+t) += sum_{i,j} W[i][j] * a[y+1-i][4q+t+1-j]
+// The generic tiled kernel gives a thread four pixels that are XQ apart and loads every (tap, pixel) operand separately
+// (36 loads per output channel, each with its own address arithmetic): ncu showed 42 % FFMA in its instruction mix.
+template <int CT>
+__global__ void __launch_bounds__(256, 2)
+conv_bwd_3x3s1_kernel(const float* __restrict__ A, long long sBr, long long sB, long long ld, int B, int R,
+                      const float* __restrict__ W, const float* __restrict__ addend, float* __restrict__ out,
+                      int c_in, int c_out, int h, int w, int COC, int CG, int RB, int stage_floats) {
+  extern __shared__ __align__(16) float sm[];
+  __shared__ const float* rowp[4];
+  const int cgct = CG * CT;
+  const int wq = w >> 2;                           // strips per image row
+  const int PT = h * wq, PW = w + 8, tile = (h + 2) * PW;
+  const int w_floats = (COC * 9 * cgct + 3) & ~3;  // stage layout: Ws [COC][9][cgct], then As [RB][COC][tile] (16-byte aligned)
+  const int tid = threadIdx.x;
+  const int pt = tid % PT, cg = (tid / PT) % CG, rb = tid / (PT * CG);
+  const bool active = rb < RB;
+  const long long rows = 2LL * B * R;
+  const long long m_base = (long long)blockIdx.x * RB;
+  const int ci_base = blockIdx.y * cgct;
+  const int y = pt / wq, q = pt % wq;
+  const int a_off = y * PW + 4 + 4 * q;            // tile row y holds image row y - 1; image column x sits at tile column x + 4
+  if (tid < RB) {
+    const long long m = m_base + tid;
+    const float* ptr = nullptr;
+    if (m < rows) {
+      const int r = (int)(m % R);
+      const long long tt = m / R;
+      ptr = A + (tt / B) * sBr + (tt % B) * sB + (long long)r * ld;
+    }
+    rowp[tid] = ptr;
+  }
+  // both stages zeroed once: the halo (and rows past the end) stay zero, the copies touch the interior only
+  for (int i = tid; i < 2 * stage_floats; i += blockDim.x) sm[i] = 0.f;
+  __syncthreads();
+  const int epp = PT;                              // float4 elements of one (row, co) map: h * w / 4 = PT
+  auto fill = [&](int co0, int stage) {
+    float* Ws = sm + stage * stage_floats;
+    float* As = Ws + w_floats;
+    const int cc = min(COC, c_out - co0);
+    for (int idx = tid; idx < cc * 9 * cgct; idx += blockDim.x) {
+      const int c = idx % cgct, t2 = idx / cgct;
+      const int tap = t2 % 9, co = t2 / 9;
+      const int ci = ci_base + c;
+      if (ci < c_in) cp_async4(Ws + idx, W + ((long long)(co0 + co) * c_in + ci) * 9 + tap);
+    }
+    for (int idx = tid; idx < RB * cc * epp; idx += blockDim.x) {
+      const int e = idx % epp, pr = idx / epp;
+      const int co = pr % cc, r_ = pr / cc;
+      const float* base = rowp[r_];
+      if (base == nullptr) continue;
+      const int yy = e / wq, xq = e % wq;
+      const float* src = base + ((long long)(co0 + co) * h + yy) * w + 4 * xq;
+      float* dst = As + ((long long)r_ * COC + co) * tile + (yy + 1) * PW + 4 + 4 * xq;
+      const uint32_t d = static_cast<uint32_t>(__cvta_generic_to_shared(dst));
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(d), "l"(src) : "memory");
+    }
+    cp_async_commit();
+  };
+  float acc[4][CT];
+#pragma unroll
+  for (int t = 0; t < 4; ++t)
+#pragma unroll
+    for (int c = 0; c < CT; ++c) acc[t][c] = 0.f;
+  const int nchunks = (c_out + COC - 1) / COC;
+  fill(0, 0);
+  for (int ch = 0; ch < nchunks; ++ch) {
+    const int stage = ch & 1;
+    if (ch + 1 < nchunks) { fill((ch + 1) * COC, stage ^ 1); cp_async_wait<1>(); }
+    else cp_async_wait<0>();
+    __syncthreads();
+    if (active) {
+      const int cc = min(COC, c_out - ch * COC);
+      const float* Ws = sm + stage * stage_floats;
+      const float* ap = Ws + w_floats + (long long)rb * COC * tile + a_off;
+      const float* wp = Ws + cg * CT;
+      for (int co = 0; co < cc; ++co, ap += tile, wp += 9 * cgct) {
+        float a[3][6];                              // a[dy][k] = A_out[y - 1 + dy][4q - 1 + k]
+#pragma unroll
+        for (int dy = 0; dy < 3; ++dy) {
+          const float4 v = *reinterpret_cast<const float4*>(ap + dy * PW);
+          a[dy][0] = ap[dy * PW - 1]; a[dy][1] = v.x; a[dy][2] = v.y; a[dy][3] = v.z; a[dy][4] = v.w; a[dy][5] = ap[dy * PW + 4];
+        }
+#pragma unroll
+        for (int c4 = 0; c4 < CT; c4 += 4) {
+#pragma unroll
+          for (int i = 0; i < 3; ++i) {
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+              const float4 wv = *reinterpret_cast<const float4*>(wp + (i * 3 + j) * cgct + c4);
+              // image row y + 1 - i is tile row offset dy = 2 - i; pixel 4q + t reads column 4q + t + 1 - j = a[.][t + 2 - j]
+#pragma unroll
+              for (int t = 0; t < 4; ++t) {
+                const float av = a[2 - i][t + 2 - j];
+                acc[t][c4 + 0] = fmaf(av, wv.x, acc[t][c4 + 0]);
+                acc[t][c4 + 1] = fmaf(av, wv.y, acc[t][c4 + 1]);
+                acc[t][c4 + 2] = fmaf(av, wv.z, acc[t][c4 + 2]);
+                acc[t][c4 + 3] = fmaf(av, wv.w, acc[t][c4 + 3]);
+              }
+            }
+          }
+        }
+      }
+    }
+    __syncthreads();      // the stage is refilled by the next iteration's fill
+  }
+  const long long m = m_base + rb;
+  if (!active || m >= rows) return;
+#pragma unroll
+  for (int c = 0; c < CT; ++c) {
+    const int ci = ci_base + cg * CT + c;
+    if (ci >= c_in) continue;
+    const long long o = ((m * c_in + ci) * h + y) * (long long)w + 4 * q;
+    float4 r = make_float4(acc[0][c], acc[1][c], acc[2][c], acc[3][c]);
+    if (addend) { const float4 e = __ldg(reinterpret_cast<const float4*>(addend + o)); r.x += e.x; r.y += e.y; r.z += e.z; r.w += e.w; }
+    *reinterpret_cast<float4*>(out + o) = r;
+  }
+}
+
+static bool launch_conv_bwd_3x3s1(const AView& A, const float* W, const float* addend, float* out, int B, int R,
+                                  int c_in, int h, int w, int c_out, int pad, int ho, int wo, cudaStream_t s) {
+  if (pad != 1 || ho != h || wo != w || (w & 3) || h * (w >> 2) > 256 || h * (w >> 2) < 16) return false;
+  auto mis = [](const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) != 0; };
+  if (mis(A.p) || mis(out) || (addend && mis(addend)) || (A.ld & 3) || (A.sB & 3) || (A.sBr & 3)) return false;
+  const int CT = (c_in % 16 == 0) ? 16 : (c_in > 4 ? 8 : 4);
+  const int PT = h * (w >> 2);
+  const int groups = (c_in + CT - 1) / CT;
+  int CG = 256 / PT < groups ? 256 / PT : groups;
+  if (CG < 1) CG = 1;
+  int RB = 256 / (PT * CG);
+  if (RB < 1) RB = 1;
+  if (RB > 4) RB = 4;
+  const int tile = (h + 2) * (w + 8);
+  const size_t per_co = ((size_t)9 * CG * CT + (size_t)RB * tile) * sizeof(float);
+  int COC = (int)((44 * 1024) / per_co);           // two stages of <= 44 KB, two blocks per SM
+  if (COC < 1) return false;
+  if (COC > c_out) COC = c_out;
+  const int stage_floats = (int)(((((size_t)COC * 9 * CG * CT + 3) & ~(size_t)3) + (size_t)COC * RB * tile + 3) / 4 * 4);
+  const size_t smem = (size_t)2 * stage_floats * sizeof(float);
+  const long long rows = 2LL * B * R;
+  dim3 grid((unsigned)((rows + RB - 1) / RB), (unsigned)((groups + CG - 1) / CG));
+#define CROWN_S1_GO(CT_) conv_bwd_3x3s1_kernel<CT_><<<grid, 256, smem, s>>>(A.p, A.sBr, A.sB, A.ld, B, R, W, addend, out, c_in, c_out, h, w, COC, CG, RB, stage_floats)
+  if (CT == 16) CROWN_S1_GO(16); else if (CT == 8) CROWN_S1_GO(8); else CROWN_S1_GO(4);
+#undef CROWN_S1_GO
+  return true;
+}
+
 int conv_s2_supported(int c_in, int h, int w, int c_out, int kh, int kw, int stride, int pad, int ho, int wo) {
   (void)c_in; (void)c_out;
   return kh == 3 && kw == 3 && stride == 2 && pad == 1 && h == 2 * ho && w == 2 * wo && ho * wo <= 256 && ho * wo >= 16 &&
@@ -660,7 +811,8 @@ void launch_conv_transpose(const AView& A, const float* W, const float* addend, 
   if ((A.sB % 1 == 0) && rows < (1LL << 31)) {
     bool done = false;
     if (kh == 1 && kw == 1 && launch_conv_bwd_1x1(A, W, addend, out, B, R, c_in, h, w, c_out, stride, pad, ho, wo, s)) return;
-    if (kh == 3 && kw == 3 && stride == 1) done = launch_conv_bwd_ct<3, 3, 1>(A, W, addend, out, B, R, c_in, h, w, c_out, pad, ho, wo, s);
+    if (kh == 3 && kw == 3 && stride == 1 && launch_conv_bwd_3x3s1(A, W, addend, out, B, R, c_in, h, w, c_out, pad, ho, wo, s)) done = true;
+    else if (kh == 3 && kw == 3 && stride == 1) done = launch_conv_bwd_ct<3, 3, 1>(A, W, addend, out, B, R, c_in, h, w, c_out, pad, ho, wo, s);
     else if (kh == 3 && kw == 3 && stride == 2 && launch_conv_bwd_3x3s2(A, W, addend, out, B, R, c_in, h, w, c_out, pad, ho, wo, s)) done = true;
     else if (kh == 3 && kw == 3 && stride == 2) done = launch_conv_bwd_ct<3, 3, 2>(A, W, addend, out, B, R, c_in, h, w, c_out, pad, ho, wo, s);
     else if (kh == 1 && kw == 1 && stride == 1) done = launch_conv_bwd_ct<1, 1, 1>(A, W, addend, out, B, R, c_in, h, w, c_out, pad, ho, wo, s);
@@ -677,6 +829,9 @@ void launch_conv_transpose(const AView& A, const float* W, const float* addend, 
 
 int conv_init_device() {
   const int b1 = 96 * 1024;
+  if (cudaFuncSetAttribute(conv_bwd_3x3s1_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1) != cudaSuccess ||
+      cudaFuncSetAttribute(conv_bwd_3x3s1_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1) != cudaSuccess ||
+      cudaFuncSetAttribute(conv_bwd_3x3s1_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1) != cudaSuccess) return -1;
   if (cudaFuncSetAttribute(conv_bwd_3x3s2_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1) != cudaSuccess ||
       cudaFuncSetAttribute(conv_bwd_3x3s2_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1) != cudaSuccess) return -1;
   if (cudaFuncSetAttribute(conv_bwd_1x1_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1) != cudaSuccess ||
