@@ -57,7 +57,6 @@ struct RelaxDev {
   float* out; float* out_lo; float* d;
   int B, R, n;
   const int8_t* split; const float* beta_lo; const float* beta_up;   // NEXT-2 (BETA instantiations only)
-  int G;        // rows per group of the (group, property, row) order (shared input rows), 0 = plain (property, row) order
   int wpp;      // warps per (b, r) pair: 1, 2, 4 or 8 (all in one block); a function of n ONLY, so that the summation
                 // order of d does not depend on how the rows are chunked (chunked == unchunked bitwise)
 };
@@ -101,22 +100,14 @@ __global__ void __launch_bounds__(256) relax_kernel(RelaxDev p) {
   const int wi = (int)(warp % wpp);                       // this warp's slice of the row
   const bool valid = pair_raw < (long long)p.B * p.R;
   const int n_eff = valid ? p.n : 0;
-  // warps are dealt to (property, row) pairs property-major -- within GROUPS of G rows when the input rows are shared by all
-  // properties (start of a pass: rows of W_k, zero-stride view): (group, property, row in group).  A group's input (G rows,
-  // <= 24 MB) then stays in L2 while all B properties read it (ncu, cfg3: 10.4 GB of DRAM reads for 0.65 GB of distinct
-  // input without the grouping), and every property still writes G CONSECUTIVE rows.  (Dealing single rows round robin
-  // over the properties also removes the re-reads but measured 3-7 % slower: the writes then scatter over B distant rows.)
-  int b, r;
-  if (p.G > 0 && valid) {
-    const long long per = (long long)p.B * p.G;
-    const long long g = pair_raw / per, rem = pair_raw % per;
-    const int gr = min(p.G, p.R - (int)(g * p.G));
-    b = (int)(rem / gr); r = (int)(g * p.G + rem % gr);
-  } else {
-    const long long q = valid ? pair_raw : 0;
-    b = (int)(q / p.R); r = (int)(q % p.R);
-  }
-  const long long pair = (long long)b * p.R + r;
+  // warps are dealt to (property, row) pairs property-major.  At the start of a pass the input rows are shared by all
+  // properties (rows of W_k, zero-stride view) and come from DRAM once per property (ncu, cfg3: 10.4 GB read for 0.65 GB of
+  // distinct input).  Two orders that remove those re-reads were measured and dropped: single rows round robin over the
+  // properties (3-7 % slower: the writes scatter over B distant rows) and groups of rows small enough to stay in L2 with
+  // every property writing a whole group (1-3 % slower).  The kernel is bound by its STORES -- 41.6 GB in 8.59 ms = 4.8 TB/s
+  // of writes on cfg3 -- and the re-reads ride along for free.
+  const long long pair = valid ? pair_raw : 0;
+  const int b = (int)(pair / p.R), r = (int)(pair % p.R);
   const float* a0 = p.A + (long long)b * p.sB + (long long)r * p.ld;
   const float* a1 = a0 + p.sBr;
   const float4* cf = RELU ? p.coef + (long long)b * p.n : nullptr;
@@ -240,11 +231,6 @@ void launch_relax(const RelaxArgs& a, cudaStream_t s) {
   long long pairs = (long long)a.B * a.R;
   if (pairs <= 0 || a.n <= 0) return;
   p.wpp = warps_per_pair(a.n);
-  p.G = 0;
-  if (a.A.sB == 0 && a.B > 1) {                    // shared input rows: keep a group of them L2-resident across the properties
-    long long g = ((24LL << 20) / ((long long)a.n * 4)) / 8 * 8;
-    p.G = (int)(g < 8 ? 8 : (g > a.R ? a.R : g));
-  }
   int blocks = ceil_div(pairs * p.wpp * 32, 256);
   auto al16 = [](const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; };
   bool vec = (a.n % 4 == 0) && (p.ld % 4 == 0) && (p.sB % 4 == 0) && (p.sBr % 4 == 0) && al16(p.A) &&
