@@ -216,7 +216,7 @@ def test_host_entry_rejects_an_inverted_box():
         ctx.run_host(bad, hi, wl.C, wl.alpha, wl.intermediate, lb, ub, ver)
 
 
-@pytest.mark.parametrize("which", ["cfg1", "cfg2", "small_B1of3"])
+@pytest.mark.parametrize("which", ["cfg1", "cfg2", "small_B1of3", "cfg5"])
 def test_host_entry_equals_device_entry_bitwise(which):
     """crown_run_host (H2D / D2H inside; one packed copy per direction for small problems, direct copies above 1 MiB)
     returns exactly what crown_run returns on resident tensors, also for B below B_max and on repeated calls"""
@@ -224,6 +224,8 @@ def test_host_entry_equals_device_entry_bitwise(which):
         wl = W.make(1); Bmax = wl.B                      # 25 KB of inputs: packed path
     elif which == "cfg2":
         wl = W.make(2, B=24); Bmax = wl.B                # 1.4 MB of alpha: direct copies
+    elif which == "cfg5":
+        wl = W.make(5, B=2); Bmax = wl.B                 # 72 MB of alpha through the conv / residual graph
     else:
         wl = W.small_mlp([6, 9, 7, 3], seed=43, B=1, eps=0.1); Bmax = 3
     lo, hi = wl.box()
