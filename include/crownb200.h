@@ -187,7 +187,8 @@ int crown_run_host(crown_ctx* ctx, int B, const float* x_lo_host, const float* x
  * transpose of that pass: a forward sweep of the 2*B*S bound-attaining box corners through the
  * network with every ReLU replaced by the line the sign of the saved A selects; at A = 0 the one-sided derivative 0 is
  * taken (reading G23).  Every ReLU needs an alpha_lo and an alpha_up entry.  scratch_dev: caller-owned device memory of
- * at least crown_alpha_scratch_bytes(B, S) bytes, 256-byte aligned (saved A per ReLU, the sweep's vectors).
+ * at least crown_alpha_scratch_bytes(B, S) bytes, 256-byte aligned (saved A per ReLU, the sweep's vectors, TF32 limbs of the
+ * weights the sweep multiplies on the tensor cores).
  * Streamed layers are CROWN_EUNSUPPORTED here. */
 int crown_alpha_scratch_bytes(crown_ctx* ctx, int B, int S, size_t* out);
 

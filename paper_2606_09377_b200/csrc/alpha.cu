@@ -179,6 +179,16 @@ void launch_alpha_add(const float* a, const float* b, float* o, long long cnt, c
   alpha_add_kernel<<<ceil_div(cnt, 256), 256, 0, s>>>(a, b, o, cnt);
 }
 
+__global__ void __launch_bounds__(256) add_bias_rows_kernel(float* __restrict__ D, const float* __restrict__ bias, long long cnt, int N) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < cnt) D[i] += __ldg(bias + (int)(i % N));
+}
+void launch_add_bias_rows(float* D, const float* bias, long long M, int N, cudaStream_t s) {
+  const long long cnt = M * N;
+  if (cnt <= 0) return;
+  add_bias_rows_kernel<<<ceil_div(cnt, 256), 256, 0, s>>>(D, bias, cnt, N);
+}
+
 // ---- ReLU: forward value through the selected line, gradient w.r.t. alpha, optional in-place projected step ---------
 // element (b, s, j) for both branches.  A, Gin, Gout: [2, B, S, n]; coef [B, n] {dU, bU, dL_fixed, unstable};
 // alpha_lo / alpha_up [B, S, n].  step != nullptr: alpha <- clip(clip(alpha) +/- step[0] * dir(g), 0, 1) with

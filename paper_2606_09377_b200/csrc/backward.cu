@@ -182,7 +182,8 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
       case CROWN_RELU: {
         if ((rc = ensure_coef(i))) return rc;
         const int j = nd.in0;
-        if (A_save && A_save[i]) {   // alpha optimisation: keep A as it arrives at this ReLU, contiguous [2,B,R,n]
+        if (A_save && A_save[i] && cur.v.p != A_save[i]) {   // alpha optimisation: keep A as it arrives at this ReLU, contiguous
+                                                              // [2,B,R,n] (unless the contraction above already wrote it there)
           Scope sc(ctx, CROWN_K_MISC, 8.0 * 2 * B * R * ni.size);
           launch_view_add(cur.v, nullptr, A_save[i], B, R, s);
         }
@@ -272,8 +273,15 @@ int run_pass(crown_ctx* ctx, int B, int start, int row0, int R, const float* C_d
             release(ctx, cur);
             break;                      // nothing is contributed to the input node: the bound is finished below
           }
-          out.buf = new_buf(ps, D);
-          if (out.buf < 0) return fail(ctx, CROWN_ENOMEM, "backward: A-buffer pool exhausted");
+          // alpha / beta optimisation: the product that arrives at a ReLU whose A is kept goes straight into that buffer
+          // (one copy of A per ReLU and evaluation less)
+          float* direct = (!fr && A_save && r >= 0 && ctx->nodes[r].n.op == CROWN_RELU && A_save[r] &&
+                           ctx->nodes[r].n_consumers == 1 && ps.pend.find(r) == ps.pend.end() && !ni.streamed) ? A_save[r] : nullptr;
+          if (direct) { D = direct; out.buf = -1; }
+          else {
+            out.buf = new_buf(ps, D);
+            if (out.buf < 0) return fail(ctx, CROWN_ENOMEM, "backward: A-buffer pool exhausted");
+          }
           if (fr) {
             if ((rc = ensure_coef(r))) return rc;
             float* D_lo = nullptr;
@@ -683,6 +691,10 @@ struct AlphaScratch {
   std::vector<float*> G;           // per node [2,B,S,size]: d bound / d A_i (Flatten aliases its producer)
   float* lb = nullptr; float* ub = nullptr;   // [B,S] bounds of the current iterate
   float* step = nullptr;           // current step size (device scalar: the iteration is data-independent on the host)
+  // forward sweep through Linear layers on the tensor cores: the layer's weight split into TF32 limbs (not transposed:
+  // G_i = G_in . W_i^T wants W_i [n_out, n_in] as the K-major B operand) and the split of G_in
+  std::vector<float*> Wf_hi, Wf_lo;   // per Linear node (nullptr: CUDA-core kernel)
+  float* Gs_hi = nullptr; float* Gs_lo = nullptr;
   int last_relu = -1;
   size_t bytes = 0;
 };
@@ -705,7 +717,28 @@ void alpha_layout(crown_ctx* ctx, int B, int S, uint8_t* base, AlphaScratch& sc)
   }
   sc.lb = take((size_t)B * S); sc.ub = take((size_t)B * S);
   sc.step = take(2);                 // {alpha step, beta step}
+  sc.Wf_hi.assign(n, nullptr); sc.Wf_lo.assign(n, nullptr);
+  size_t kmax = 0;
+  if (ctx->opts.mma_scheme == 0)
+    for (int i = 0; i <= sc.last_relu; ++i) {
+      const NodeInfo& ni = ctx->nodes[i];
+      if (ni.n.op != CROWN_LINEAR || !gemm_tc_supported((int)rows, ni.n.n_out, ni.n.n_in)) continue;
+      sc.Wf_hi[i] = take((size_t)ni.n.n_out * ni.n.n_in);
+      sc.Wf_lo[i] = take((size_t)ni.n.n_out * ni.n.n_in);
+      kmax = std::max(kmax, (size_t)ni.n.n_in);
+    }
+  if (kmax) { sc.Gs_hi = take(rows * kmax); sc.Gs_lo = take(rows * kmax); }
   sc.bytes = off;
+}
+
+// TF32 limbs of the weights the forward sweep multiplies on the tensor cores (once per call: one pass over those W)
+void alpha_prepare(crown_ctx* ctx, const AlphaScratch& sc) {
+  for (size_t i = 0; i < ctx->nodes.size(); ++i) {
+    if (!sc.Wf_hi[i]) continue;
+    const crown_node& nd = ctx->nodes[i].n;
+    Scope scp(ctx, CROWN_K_MISC, 12.0 * nd.n_out * nd.n_in);
+    launch_split_tf32(nd.W_dev, nd.n_out, nd.n_in, 0, sc.Wf_hi[i], sc.Wf_lo[i], ctx->stream);
+  }
 }
 
 int alpha_check(crown_ctx* ctx, int B, int S, const float* C_dev, const float* const* l_dev, const float* const* u_dev,
@@ -756,6 +789,18 @@ int alpha_forward(crown_ctx* ctx, int B, int S, const AlphaScratch& sc, const fl
     const float* gin = nd.in0 < 0 ? sc.Gin : sc.G[nd.in0];
     switch (nd.op) {
       case CROWN_LINEAR: {
+        if (sc.Wf_hi[i]) {
+          // tensor cores (3xTF32): split G_in, contract with the limbs of W_i made by alpha_prepare, add the bias
+          { Scope scp(ctx, CROWN_K_MISC, 12.0 * M * nd.n_in); launch_split_tf32(gin, (int)M, nd.n_in, 0, sc.Gs_hi, sc.Gs_lo, s); }
+          const char* e = nullptr;
+          { Scope scp(ctx, CROWN_K_GEMM_TC, 8.0 * M * nd.n_in + 8.0 * nd.n_in * nd.n_out + 4.0 * M * nd.n_out, 2.0 * M * (double)nd.n_in * nd.n_out);
+            if (launch_gemm_tc(sc.Gs_hi, sc.Gs_lo, sc.Wf_hi[i], sc.Wf_lo[i], sc.G[i], nd.n_out, (int)M, nd.n_out, nd.n_in,
+                               ctx->opts.k_drain, ctx->num_sms, s, &e))
+              return fail(ctx, CROWN_ECUDA, std::string("alpha forward gemm_tc: ") + (e ? e : "?"));
+            ctx->launches += gemm_tc_num_panels(nd.n_in) - 1; }
+          if (nd.b_dev) { Scope scp(ctx, CROWN_K_MISC, 8.0 * M * nd.n_out); launch_add_bias_rows(sc.G[i], nd.b_dev, M, nd.n_out, s); }
+          break;
+        }
         Scope scp(ctx, CROWN_K_GEMM_FFMA, 4.0 * ((double)M * nd.n_in + (double)nd.n_in * nd.n_out + (double)M * nd.n_out),
                   2.0 * M * (double)nd.n_in * nd.n_out);
         launch_alpha_linear(gin, nd.W_dev, nd.b_dev, sc.G[i], (int)M, nd.n_out, nd.n_in, s);
@@ -811,6 +856,7 @@ static int beta_grad_impl(crown_ctx* ctx, int B, const float* C_dev, int S, cons
                        scratch_bytes, false, sc);
   if (rc) return rc;
   CK(ctx, cudaMemsetAsync(scratch_dev, 0, sc.bytes, ctx->stream));
+  alpha_prepare(ctx, sc);
   SplitSpec sp; sp.split = split_dev; sp.beta_lo = beta_lo_dev; sp.beta_up = beta_up_dev;
   rc = alpha_backward(ctx, B, S, C_dev, l_dev, u_dev, alpha_lo_dev, alpha_up_dev, x_lo_dev, x_hi_dev, sc, nullptr,
                       split_dev ? &sp : nullptr);
@@ -843,6 +889,7 @@ static int beta_ascent_impl(crown_ctx* ctx, int B, const float* C_dev, int S, co
         return fail(ctx, CROWN_EINVAL, std::string(who) + ": every split ReLU needs distinct beta_lo and beta_up tensors");
   cudaStream_t s = ctx->stream;
   CK(ctx, cudaMemsetAsync(scratch_dev, 0, sc.bytes, s));
+  alpha_prepare(ctx, sc);
   { Scope scp(ctx, CROWN_K_MISC); launch_alpha_set_step(sc.step, eta_alpha, s, eta_beta); }
   SplitSpec sp; sp.split = split_dev;
   sp.beta_lo = reinterpret_cast<const float* const*>(beta_lo_dev); sp.beta_up = reinterpret_cast<const float* const*>(beta_up_dev);

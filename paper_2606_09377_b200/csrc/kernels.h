@@ -146,6 +146,8 @@ void launch_alpha_linear(const float* G, const float* W, const float* bias, floa
 void launch_alpha_conv(const float* W, const float* bias, const float* in, float* out, long long M, int c_in, int h,
                        int w, int c_out, int kh, int kw, int stride, int pad, int ho, int wo, cudaStream_t s);
 void launch_alpha_add(const float* a, const float* b, float* o, long long cnt, cudaStream_t s);
+// D[m, j] += bias[j] for m < M, j < N (bias of a Linear layer after its tensor-core product in the forward sweep)
+void launch_add_bias_rows(float* D, const float* bias, long long M, int N, cudaStream_t s);
 // split / beta_lo / beta_up / gb_lo / gb_up (NEXT-2, reading G28; all nullptr = alpha only): d lb / d beta_lo = -s * Gin,
 // d ub / d beta_up = +s * Gin; step mode: beta <- max(max(beta, 0) +/- step[1] * dir, 0) in place.
 void launch_alpha_relu(const float* A, const float* Gin, const float4* coef, float* alpha_lo, float* alpha_up,
