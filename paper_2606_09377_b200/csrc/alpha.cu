@@ -189,6 +189,15 @@ void launch_add_bias_rows(float* D, const float* bias, long long M, int N, cudaS
   add_bias_rows_kernel<<<ceil_div(cnt, 256), 256, 0, s>>>(D, bias, cnt, N);
 }
 
+__global__ void __launch_bounds__(256) add_bias_div_kernel(float* __restrict__ D, const float* __restrict__ bias, long long cnt, int N, int div) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < cnt) D[i] += __ldg(bias + (int)((i / div) % N));
+}
+void launch_add_bias_div(float* D, const float* bias, long long cnt, int N, int div, cudaStream_t s) {
+  if (cnt <= 0) return;
+  add_bias_div_kernel<<<ceil_div(cnt, 256), 256, 0, s>>>(D, bias, cnt, N, div);
+}
+
 // ---- ReLU: forward value through the selected line, gradient w.r.t. alpha, optional in-place projected step ---------
 // element (b, s, j) for both branches.  A, Gin, Gout: [2, B, S, n]; coef [B, n] {dU, bU, dL_fixed, unstable};
 // alpha_lo / alpha_up [B, S, n].  step != nullptr: alpha <- clip(clip(alpha) +/- step[0] * dir(g), 0, 1) with

@@ -694,6 +694,7 @@ struct AlphaScratch {
   // forward sweep through Linear layers on the tensor cores: the layer's weight split into TF32 limbs (not transposed:
   // G_i = G_in . W_i^T wants W_i [n_out, n_in] as the K-major B operand) and the split of G_in
   std::vector<float*> Wf_hi, Wf_lo;   // per Linear node (nullptr: CUDA-core kernel)
+  std::vector<float*> Wk;             // per Conv2d node: flipped, role-swapped filters for the strip kernel (nullptr: gather kernel)
   float* Gs_hi = nullptr; float* Gs_lo = nullptr;
   int last_relu = -1;
   size_t bytes = 0;
@@ -728,6 +729,14 @@ void alpha_layout(crown_ctx* ctx, int B, int S, uint8_t* base, AlphaScratch& sc)
       kmax = std::max(kmax, (size_t)ni.n.n_in);
     }
   if (kmax) { sc.Gs_hi = take(rows * kmax); sc.Gs_lo = take(rows * kmax); }
+  sc.Wk.assign(n, nullptr);
+  for (int i = 0; i <= sc.last_relu; ++i) {
+    const NodeInfo& ni = ctx->nodes[i];
+    const crown_node& nd = ni.n;
+    if (nd.op == CROWN_CONV2D && nd.kh == 3 && nd.kw == 3 && nd.stride == 1 && nd.pad == 1 && (rows % 2) == 0 &&
+        conv3x3s1_points_supported(nd.c_in, nd.h_in, nd.w_in, nd.c_out))
+      sc.Wk[i] = take((size_t)nd.c_out * nd.c_in * 9);
+  }
   sc.bytes = off;
 }
 
@@ -738,6 +747,12 @@ void alpha_prepare(crown_ctx* ctx, const AlphaScratch& sc) {
     const crown_node& nd = ctx->nodes[i].n;
     Scope scp(ctx, CROWN_K_MISC, 12.0 * nd.n_out * nd.n_in);
     launch_split_tf32(nd.W_dev, nd.n_out, nd.n_in, 0, sc.Wf_hi[i], sc.Wf_lo[i], ctx->stream);
+  }
+  for (size_t i = 0; i < ctx->nodes.size(); ++i) {
+    if (!sc.Wk[i]) continue;
+    const crown_node& nd = ctx->nodes[i].n;
+    Scope scp(ctx, CROWN_K_MISC, 8.0 * nd.c_out * nd.c_in * 9);
+    launch_flip_conv_weights(nd.W_dev, sc.Wk[i], nd.c_out, nd.c_in, ctx->stream);
   }
 }
 
@@ -808,6 +823,10 @@ int alpha_forward(crown_ctx* ctx, int B, int S, const AlphaScratch& sc, const fl
       case CROWN_CONV2D: {
         Scope scp(ctx, CROWN_K_CONV, 4.0 * M * ((double)ni.size + (double)nd.c_in * nd.h_in * nd.w_in),
                   2.0 * M * (double)ni.size * nd.c_in * nd.kh * nd.kw);
+        if (sc.Wk[i] && launch_conv3x3s1_points(gin, sc.Wk[i], sc.G[i], M, nd.c_in, nd.h_in, nd.w_in, nd.c_out, s) == 0) {
+          if (nd.b_dev) launch_add_bias_div(sc.G[i], nd.b_dev, M * ni.size, nd.c_out, ni.h * ni.w, s);
+          break;
+        }
         launch_alpha_conv(nd.W_dev, nd.b_dev, gin, sc.G[i], M, nd.c_in, nd.h_in, nd.w_in, nd.c_out, nd.kh, nd.kw, nd.stride,
                           nd.pad, ni.h, ni.w, s);
         break; }

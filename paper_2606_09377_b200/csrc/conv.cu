@@ -739,6 +739,33 @@ static bool launch_conv_bwd_3x3s1(const AView& A, const float* W, const float* a
   return true;
 }
 
+// Forward 3x3 / stride 1 / pad 1 convolution of M points through the strip kernel (NEXT-1 forward sweep): conv(x, W) is the
+// transpose kernel run with the filter bank flipped and its channel roles swapped,
+//   out[m, co, y, x] = sum_ci sum_{i,j} Wk[ci][co][i][j] * in[m, ci, y+1-i, x+1-j],   Wk[ci][co][i][j] = W[co][ci][2-i][2-j]
+// (Wk is made by launch_flip_conv_weights).  `in` / `out` are [M, c, h, w] contiguous; the bias is added by the caller.
+int conv3x3s1_points_supported(int c_in, int h, int w, int c_out) {
+  (void)c_in; (void)c_out;
+  return (w & 3) == 0 && h * (w >> 2) <= 256 && h * (w >> 2) >= 16;
+}
+int launch_conv3x3s1_points(const float* in, const float* Wk, float* out, long long M, int c_in, int h, int w, int c_out,
+                            cudaStream_t s) {
+  if (M <= 0 || (M & 1)) return -1;
+  AView v; v.p = in; v.ld = (long long)c_in * h * w; v.n = c_in * h * w; v.sB = 0; v.sBr = (M / 2) * v.ld;
+  // rows m < M/2 as "branch 0", the rest as "branch 1" of a B = 1, R = M/2 problem; reduce channels = c_in, outputs = c_out
+  return launch_conv_bwd_3x3s1(v, Wk, nullptr, out, 1, (int)(M / 2), c_out, h, w, c_in, 1, h, w, s) ? 0 : -1;
+}
+__global__ void flip_conv_weights_kernel(const float* __restrict__ W, float* __restrict__ Wk, int c_out, int c_in) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= c_out * c_in * 9) return;
+  const int tap = i % 9, ci = (i / 9) % c_in, co = i / (9 * c_in);           // i indexes W[co][ci][tap]
+  Wk[((long long)ci * c_out + co) * 9 + (8 - tap)] = W[i];
+}
+void launch_flip_conv_weights(const float* W, float* Wk, int c_out, int c_in, cudaStream_t s) {
+  const int cnt = c_out * c_in * 9;
+  if (cnt <= 0) return;
+  flip_conv_weights_kernel<<<ceil_div(cnt, 256), 256, 0, s>>>(W, Wk, c_out, c_in);
+}
+
 int conv_s2_supported(int c_in, int h, int w, int c_out, int kh, int kw, int stride, int pad, int ho, int wo) {
   (void)c_in; (void)c_out;
   return kh == 3 && kw == 3 && stride == 2 && pad == 1 && h == 2 * ho && w == 2 * wo && ho * wo <= 256 && ho * wo >= 16 &&

@@ -145,6 +145,13 @@ void launch_alpha_linear(const float* G, const float* W, const float* bias, floa
                          cudaStream_t s);
 void launch_alpha_conv(const float* W, const float* bias, const float* in, float* out, long long M, int c_in, int h,
                        int w, int c_out, int kh, int kw, int stride, int pad, int ho, int wo, cudaStream_t s);
+// 3x3 / stride 1 / pad 1 forward conv of M points on the strip kernel of conv.cu (Wk = flipped, role-swapped filters)
+int conv3x3s1_points_supported(int c_in, int h, int w, int c_out);
+int launch_conv3x3s1_points(const float* in, const float* Wk, float* out, long long M, int c_in, int h, int w, int c_out,
+                            cudaStream_t s);
+void launch_flip_conv_weights(const float* W, float* Wk, int c_out, int c_in, cudaStream_t s);
+// D[i] += bias[(i / div) % N] (div = H*W: per-channel bias of a conv map; div = 1: per-column bias of a Linear output)
+void launch_add_bias_div(float* D, const float* bias, long long cnt, int N, int div, cudaStream_t s);
 void launch_alpha_add(const float* a, const float* b, float* o, long long cnt, cudaStream_t s);
 // D[m, j] += bias[j] for m < M, j < N (bias of a Linear layer after its tensor-core product in the forward sweep)
 void launch_add_bias_rows(float* D, const float* bias, long long M, int N, cudaStream_t s);
