@@ -274,6 +274,24 @@ int crown_gemm(crown_ctx* ctx, int scheme, int M, int N, int K,
 int crown_split_tf32(crown_ctx* ctx, const float* X_dev, int rows, int cols, int transpose,
                      float* hi_dev, float* lo_dev);
 
+/* The same contraction for callers that cannot allocate device memory (code under CUDA-graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): D[M,N] = A[M,K] . W[K,N], row-major fp32 DEVICE pointers, 3xTF32 on tcgen05
+ * (PAPER.md:66-68 Eq. 1, :128).  The TF32 limbs that crown_gemm takes from the caller live here in one file-scope
+ * device array inside the library (16 MiB, held by every GPU that loads the library until the process exits); the call
+ * needs no crown_ctx and calls no cudaMalloc / cudaFree / allocating library routine.  Work is queued on `stream`
+ * (a cudaStream_t of the CURRENT device, or NULL) and the call returns without synchronising.
+ *   limits: N >= 128, K >= 32, N % 4 == 0, K % 4 == 0, D_dev 16-byte aligned, and
+ *           round64(M*K) + round64(N*K) <= CROWN_GEMM_NOALLOC_MAX_ELEMS  (crown_gemm_noalloc_max_elems() returns it);
+ *           anything beyond is CROWN_EINVAL with the sizes in crown_gemm_noalloc_error() (thread-local text).
+ *   sharing: every call uses the same array, which keeps the previous call's contents; each call overwrites all it
+ *           reads, so nothing needs clearing.  Calls whose kernels may overlap on the GPU (different streams without
+ *           a dependency, or different host threads on different streams) RACE -- serialise them on one stream.
+ *   result: bitwise equal to crown_split_tf32 x 2 + crown_gemm(scheme 0) of a context with default options. */
+#define CROWN_GEMM_NOALLOC_MAX_ELEMS (1u << 21)
+int crown_gemm_noalloc(int M, int N, int K, const float* A_dev, const float* W_dev, float* D_dev, void* stream);
+int crown_gemm_noalloc_max_elems(void);
+const char* crown_gemm_noalloc_error(void);
+
 /* Introspection. */
 int crown_peak_bytes(crown_ctx* ctx, size_t* out);         /* high-water mark of workspace use   */
 int crown_row_chunk(crown_ctx* ctx, int* out);             /* rows per chunk of identity-start passes under mem_cap */

@@ -21,7 +21,7 @@ K_CLASSES = ["ibp", "coeff", "relax", "gemm_tc", "gemm_ffma", "concretize", "con
 EXPORTS = ["crown_h2d_bytes", "crown_workspace_bytes", "crown_init", "ibp_forward", "crown_backward", "concretize", "crown_verdict", "crown_run",
            "crown_run_host", "crown_alpha_scratch_bytes", "crown_alpha_grad", "crown_alpha_ascent", "crown_backward_split", "crown_beta_grad", "crown_beta_ascent", "crown_gemm", "crown_split_tf32", "crown_peak_bytes", "crown_row_chunk", "crown_launch_count", "crown_graph_replays",
            "crown_gemm_flops", "crown_timing", "crown_timing_read", "crown_last_error", "crown_destroy",
-           "crown_version"]
+           "crown_version", "crown_gemm_noalloc", "crown_gemm_noalloc_max_elems", "crown_gemm_noalloc_error"]
 
 
 class CrownNode(C.Structure):
@@ -93,8 +93,34 @@ def load_library() -> C.CDLL:
     lib.crown_timing_read.argtypes = [vp, i32, C.POINTER(C.c_double), C.POINTER(C.c_uint64),
                                       C.POINTER(C.c_double), C.POINTER(C.c_double)]
     lib.crown_destroy.argtypes = [vp]
+    lib.crown_gemm_noalloc.argtypes = [i32, i32, i32, vp, vp, vp, vp]
+    lib.crown_gemm_noalloc_max_elems.argtypes = []
+    lib.crown_gemm_noalloc_error.restype = C.c_char_p
+    lib.crown_gemm_noalloc_error.argtypes = []
     _lib = lib
     return lib
+
+
+def gemm_noalloc(A: torch.Tensor, W: torch.Tensor, out: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """D[M,N] = A[M,K] . W[K,N] through crown_gemm_noalloc: the 3xTF32 tcgen05 contraction with its operand limbs in the
+    library's static device scratch (no context, no device allocation inside the call; `out` lets the caller bring D
+    too).  Queued on torch's current stream of A's device.  Calls that overlap on the GPU race on the scratch."""
+    lib = load_library()
+    if not (A.is_cuda and W.is_cuda and A.dtype == torch.float32 and W.dtype == torch.float32
+            and A.is_contiguous() and W.is_contiguous() and A.dim() == 2 and W.dim() == 2 and A.shape[1] == W.shape[0]):
+        raise CrownError("gemm_noalloc: A [M,K] and W [K,N] must be contiguous float32 CUDA tensors")
+    M, K = A.shape
+    N = W.shape[1]
+    if out is None:
+        out = torch.empty(M, N, device=A.device)
+    elif not (out.is_cuda and out.dtype == torch.float32 and out.is_contiguous() and tuple(out.shape) == (M, N)):
+        raise CrownError("gemm_noalloc: out must be a contiguous float32 CUDA tensor [M,N]")
+    with torch.cuda.device(A.device):
+        rc = lib.crown_gemm_noalloc(M, N, K, A.data_ptr(), W.data_ptr(), out.data_ptr(),
+                                    torch.cuda.current_stream().cuda_stream)
+        if rc != 0:
+            raise CrownError(f"[{rc}] " + lib.crown_gemm_noalloc_error().decode())
+    return out
 
 
 def _ptr(t: Optional[torch.Tensor]) -> Optional[int]:

@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcrownb200.so")
-SOURCES = ["api.cu", "backward.cu", "elementwise.cu", "ibp.cu", "conv.cu", "conv_tc.cu", "alpha.cu", "gemm_ffma.cu", "gemm_tc.cu"]
+SOURCES = ["api.cu", "backward.cu", "elementwise.cu", "ibp.cu", "conv.cu", "conv_tc.cu", "alpha.cu", "gemm_ffma.cu", "gemm_tc.cu", "noalloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall", "--use_fast_math=false"]
 
