@@ -61,6 +61,13 @@ __device__ __forceinline__ float tf32_rn_bits(float x) {
   return __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xffffe000u);
 }
 
+// streaming 128-bit store under a predicate, without a branch around it (a branch per store keeps ptxas from moving the
+// shared-memory reads of the following stores above it)
+__device__ __forceinline__ void stg_stream4_if(bool on, float* p, const float4& v) {
+  asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.s32 q, %5, 0;\n\t@q st.global.L1::no_allocate.v4.f32 [%0], {%1,%2,%3,%4};\n\t}"
+               :: "l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w), "r"((int)on) : "memory");
+}
+
 struct EpiArgs {
   int mode = EPI_STORE;
   int B = 0, R = 0;              // row m -> branch m / (B*R), property (m / R) % B
@@ -204,6 +211,30 @@ gemm2_tf32x3_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_con
     uint32_t cnt = 0;
     for (int t = cluster_id; t < num_tiles; t += num_clusters) {
       int mb, nb; tile_coords(t, m_tiles, n_tiles, mb, nb);
+      const int row = mb * PAIR_M + (int)rank * BM + quad * 32 + lane;       // this thread's output row
+      const int row0 = mb * PAIR_M + (int)rank * BM + quad * 32;             // first row of the warp's slab
+      const int tcol0 = nb * BN + chalf * EC;                                 // first column of the warp (in this launch)
+      const bool rok = row < M;
+      const int rr = rok ? row : 0;
+      // EPI_RELAX: the warp's relaxation coefficients (lane = column) are requested before the tile's MMAs are waited
+      // for, so their global-memory latency (4 dependent round trips per tile otherwise, 22 % of the epilogue's stall
+      // samples in capture C of profiles/r2_gemm2.md) is hidden behind the drain.  The loaded values are kept raw; the
+      // branch-dependent selection happens where they are used (a consumer placed here would wait for the loads here).
+      float4 craw[EC / 32];
+      float braw[EC / 32];
+      if (ea.mode == EPI_RELAX) {
+        const float4* crow = ea.coef + (long long)((rr / ea.R) % ea.B) * ea.coef_ld + ea.col_off;
+#pragma unroll
+        for (int sl = 0; sl < EC / 32; ++sl) {
+          // columns past N take the last column's (finite) coefficients: their accumulators are exact zeros (the TMA
+          // zero-fills the missing rows of W) and they are never stored, so d and the output do not see them; an
+          // unconditional load leaves no select after it that would wait for the data here
+          const int cc = min(tcol0 + sl * 32 + lane, N - 1);
+          craw[sl] = __ldg(crow + cc);                                      // {dU, bU, dL, unstable}
+          braw[sl] = 0.f;
+          if (ea.bias) braw[sl] = __ldg(ea.bias + ea.col_off + cc);
+        }
+      }
       float acc[EC];
 #pragma unroll
       for (int i = 0; i < EC; ++i) acc[i] = 0.f;
@@ -227,11 +258,6 @@ gemm2_tf32x3_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_con
         if (lane == 0) mbar_arrive_cluster_relaxed(accempty_remote[buf]);
         ++cnt;
       }
-      const int row = mb * PAIR_M + (int)rank * BM + quad * 32 + lane;       // this thread's output row
-      const int row0 = mb * PAIR_M + (int)rank * BM + quad * 32;             // first row of the warp's slab
-      const int tcol0 = nb * BN + chalf * EC;                                 // first column of the warp (in this launch)
-      const bool rok = row < M;
-      const int rr = rok ? row : 0;
       // do the warp's 32 rows share (branch, property)?  Always for identity passes with R % 32 == 0 (the hot case).
       const bool uni = (ea.R & 31) == 0;
 
@@ -287,17 +313,17 @@ gemm2_tf32x3_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_con
         // (lane = column) and read back as broadcasts; (2) the hi limbs and (3) the lo limbs, written row-per-lane
         // (swizzled, conflict-free) and read back four rows per warp instruction, so the global stores are full
         // 128-byte row segments.
+        // The slab loop is NOT unrolled: fully unrolled the fused epilogue is 55 KB of straight-line code that eight warps
+        // walk through at eight different places (24 % of its stall samples were instruction-fetch stalls, one every 48
+        // instructions, capture C of profiles/r2_gemm2.md).  The body always works on acc[0..31] / craw[0]; the registers
+        // of the remaining slabs are moved down by one slab after each iteration.
         const bool upper = rr >= BR;
-        const float4* crow = ea.coef + (long long)((rr / ea.R) % ea.B) * ea.coef_ld + ea.col_off;
-#pragma unroll
+#pragma unroll 1
         for (int sl = 0; sl < EC / 32; ++sl) {
           const int col = tcol0 + sl * 32;
-          if (chalf * EC + sl * 32 >= BN || col >= N) continue;            // warp-uniform
-          float4 cf = make_float4(0.f, 0.f, 0.f, 0.f);
-          if (col + lane < N) {
-            const float4 c = __ldg(crow + col + lane);                      // {dU, bU, dL, unstable}
-            cf = make_float4(upper ? c.x : c.z, upper ? c.z : c.x, c.y, ea.bias ? __ldg(ea.bias + ea.col_off + col + lane) : 0.f);
-          }
+          if (chalf * EC + sl * 32 >= BN || col >= N) break;               // warp-uniform; later slabs are further out
+          // {slope for a > 0, slope for a <= 0, bU, bias}
+          const float4 cf = make_float4(upper ? craw[0].x : craw[0].z, upper ? craw[0].z : craw[0].x, craw[0].y, braw[0]);
           __syncwarp();
           asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};"
                        :: "r"(slab_base + (uint32_t)lane * 16u), "f"(cf.x), "f"(cf.y), "f"(cf.z), "f"(cf.w) : "memory");
@@ -307,12 +333,12 @@ gemm2_tf32x3_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_con
           for (int i = 0; i < 32; ++i) {
             float4 c;
             asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(c.x), "=f"(c.y), "=f"(c.z), "=f"(c.w) : "r"(slab_base + (uint32_t)i * 16u));
-            const float a = acc[sl * 32 + i];
+            const float a = acc[i];
             const float o = a * (a > 0.f ? c.x : c.y);     // == A+ s_pos + A- s_neg (one of the two terms is +-0)
             dsum = fmaf(upper ? fmaxf(a, 0.f) : fminf(a, 0.f), c.z, dsum);
             dsum = fmaf(o, c.w, dsum);
             hi[i] = tf32_rn_bits(o);
-            acc[sl * 32 + i] = tf32_rn_bits(o - hi[i]);    // lo limb, kept in the accumulator registers
+            acc[i] = tf32_rn_bits(o - hi[i]);    // lo limb, kept in the accumulator registers
           }
           if (rok) ea.part[(long long)row * ea.parts + ((ea.col_off + col) >> 5)] = dsum;
 #pragma unroll
@@ -320,7 +346,7 @@ gemm2_tf32x3_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_con
             __syncwarp();                                   // the slab's previous contents have been read by every lane
 #pragma unroll
             for (int c4 = 0; c4 < 8; ++c4) {
-              const int i = sl * 32 + c4 * 4;
+              const int i = c4 * 4;
               if (limb == 0)
                 asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};"
                              :: "r"(slab + (((uint32_t)c4 ^ sw) << 4)), "f"(hi[c4 * 4]), "f"(hi[c4 * 4 + 1]), "f"(hi[c4 * 4 + 2]), "f"(hi[c4 * 4 + 3]) : "memory");
@@ -329,17 +355,34 @@ gemm2_tf32x3_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_con
                              :: "r"(slab + (((uint32_t)c4 ^ sw) << 4)), "f"(acc[i]), "f"(acc[i + 1]), "f"(acc[i + 2]), "f"(acc[i + 3]) : "memory");
             }
             __syncwarp();
-            float* outp = limb == 0 ? ea.out_hi : ea.out_lo;
-            const int c4 = lane & 7;
+            const int c4 = lane & 7, r0 = lane >> 3;
+            // one pointer per lane, advanced by four rows per store (no per-store 64-bit index arithmetic)
+            float* outp = (limb == 0 ? ea.out_hi : ea.out_lo) + (long long)(row0 + r0) * ea.ldd + col + c4 * 4;
+            const long long step = 4 * ea.ldd;
+            const int rows_left = col + c4 * 4 < N ? M - row0 - r0 : 0;     // store row r0 + 4 it while 4 it < rows_left
+            // four shared-memory reads, then their four stores, twice (paired up one by one, every store would wait for
+            // its own read's latency; eight at once do not fit the register budget next to the 128 accumulators)
 #pragma unroll
-            for (int it = 0; it < 8; ++it) {
-              const int r = it * 4 + (lane >> 3);
-              float4 v;
-              asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
-                           : "r"(slab_base + (uint32_t)r * 128u + (((uint32_t)c4 ^ (uint32_t)(r & 7)) << 4)));
-              if (row0 + r < M && col + c4 * 4 < N)
-                stg_stream4(outp + (long long)(row0 + r) * ea.ldd + col + c4 * 4, v);
+            for (int half = 0; half < 2; ++half) {
+              float4 v[4];
+#pragma unroll
+              for (int q = 0; q < 4; ++q) {
+                const int r = (half * 4 + q) * 4 + r0;
+                asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v[q].x), "=f"(v[q].y), "=f"(v[q].z), "=f"(v[q].w)
+                             : "r"(slab_base + (uint32_t)r * 128u + (((uint32_t)c4 ^ (uint32_t)(r & 7)) << 4)));
+              }
+#pragma unroll
+              for (int q = 0; q < 4; ++q) {
+                stg_stream4_if((half * 4 + q) * 4 < rows_left, outp, v[q]);
+                outp += step;
+              }
             }
+          }
+          if (sl + 1 < EC / 32) {
+#pragma unroll
+            for (int i = 0; i < EC - 32; ++i) acc[i] = acc[i + 32];
+#pragma unroll
+            for (int q = 0; q + 1 < EC / 32; ++q) { craw[q] = craw[q + 1]; braw[q] = braw[q + 1]; }
           }
         }
         continue;
