@@ -403,15 +403,25 @@ gemm2_tf32x3_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_con
                          :: "r"(slab + (((uint32_t)c4 ^ sw) << 4)), "f"(acc[i]), "f"(acc[i + 1]), "f"(acc[i + 2]), "f"(acc[i + 3]) : "memory");
           }
           __syncwarp();
-          const int c4 = lane & 7;
+          // as in the fused epilogue: one pointer per lane, four reads then their four predicated stores, twice
+          const int c4 = lane & 7, r0 = lane >> 3;
+          float* outp = ea.out_hi + (long long)(row0 + r0) * ea.ldd + col + c4 * 4;
+          const long long step = 4 * ea.ldd;
+          const int rows_left = col + c4 * 4 < N ? M - row0 - r0 : 0;
 #pragma unroll
-          for (int it = 0; it < 8; ++it) {
-            const int r = it * 4 + (lane >> 3);
-            float4 v;
-            asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
-                         : "r"(slab_base + (uint32_t)r * 128u + (((uint32_t)c4 ^ (uint32_t)(r & 7)) << 4)));
-            if (row0 + r < M && col + c4 * 4 < N)
-              stg_stream4(ea.out_hi + (long long)(row0 + r) * ea.ldd + col + c4 * 4, v);
+          for (int half = 0; half < 2; ++half) {
+            float4 v[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+              const int r = (half * 4 + q) * 4 + r0;
+              asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v[q].x), "=f"(v[q].y), "=f"(v[q].z), "=f"(v[q].w)
+                           : "r"(slab_base + (uint32_t)r * 128u + (((uint32_t)c4 ^ (uint32_t)(r & 7)) << 4)));
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+              stg_stream4_if((half * 4 + q) * 4 < rows_left, outp, v[q]);
+              outp += step;
+            }
           }
         }
         continue;
