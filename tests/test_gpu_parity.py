@@ -146,6 +146,31 @@ def test_unfused_relaxation_path(cfg, kw):
     _close(_np(res2["ub"]), _np(res["ub"]), "fused vs unfused ub")
 
 
+@pytest.mark.parametrize("widths", [[200, 176, 272, 160, 7], [136, 144, 160, 192, 5]])
+def test_fused_epilogues_on_ragged_widths(widths):
+    """a4 / a8 fused into the contraction where the row length is NOT a multiple of the 32-column pieces the epilogue works in
+    (176 = 5.5, 144 = 4.5, 200 = 6.25, 136 = 4.25 pieces): the last piece of a row reads clamped coefficient columns and stores
+    only the columns that exist.  The passes that start at the 160- / 192-row layers take the fused path (rows % 32 == 0)."""
+    wl = W.small_mlp(widths, seed=17, B=3, eps=0.03, S=4)
+    ctx, res = _check_workload(wl, free_running=False)
+    assert ctx.gemm_flops() > 0
+    lo, hi = wl.box()
+    ctx1 = _ctx(wl.net, wl.B, wl.S, disable_epi_fusion=1, disable_conc_fusion=1)
+    n_relax = []
+    for c in (ctx, ctx1):           # a plain (non-graph) run with per-class timing on counts the relaxation kernels
+        c.timing(True)
+        r = c.run(lo, hi, wl.C, wl.alpha, wl.intermediate)
+        n_relax.append(c.timing_read()["relax"]["launches"])
+        c.timing(False)
+    res1 = r
+    assert n_relax[0] < n_relax[1], f"the fused epilogue was not taken ({n_relax}): the test does not exercise it"
+    for i in wl.net.relu_ids():
+        _close(_np(res["pre"][i][0]), _np(res1["pre"][i][0]), f"fused vs unfused l of relu {i}")
+        _close(_np(res["pre"][i][1]), _np(res1["pre"][i][1]), f"fused vs unfused u of relu {i}")
+    _close(_np(res["lb"]), _np(res1["lb"]), "fused vs unfused lb")
+    _close(_np(res["ub"]), _np(res1["ub"]), "fused vs unfused ub")
+
+
 def test_cfg3_scaled_chunked_equals_unchunked():
     import torch
     wl = W.make(3, scale=16, B=2)
