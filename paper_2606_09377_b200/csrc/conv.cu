@@ -204,7 +204,7 @@ conv_bwd_tiled_kernel(const float* __restrict__ A, long long sBr, long long sB, 
     rowp[tid] = ptr;
   }
   // zero both stages once: the halo (and rows past the end) stay zero, the copies only touch the interior
-  for (int i = tid; i < 2 * g.stage_floats; i += blockDim.x) smem_f[i] = 0.f;
+  for (int i = tid; i < g.stage_floats / 2; i += blockDim.x) reinterpret_cast<float4*>(smem_f)[i] = make_float4(0.f, 0.f, 0.f, 0.f);   // stage_floats % 4 == 0
   // this thread's share of a tile: source offset inside one (row, co) map, or -1 for halo elements
   int soff[kConvFillMax], doff[kConvFillMax];
 #pragma unroll
@@ -448,6 +448,20 @@ conv_bwd_1x1_kernel(const float* __restrict__ A, long long sBr, long long sB, lo
     const int ci = ci0 + c;
     if (ci >= c_in) break;
     const long long base = (m * c_in + ci) * (long long)(h * w);
+    if (stride == 2 && (w & 1) == 0 && 2 * py + 1 < h &&
+        ((reinterpret_cast<uintptr_t>(out) | reinterpret_cast<uintptr_t>(addend)) & 7) == 0) {
+      // the 2 x 2 input block of this output pixel as two 8-byte stores: {value, 0} and {0, 0} (+ the addend); one
+      // 4-byte store per input pixel left every second lane of a store instruction idle
+      const long long o = base + (long long)(2 * py) * w + 2 * px;        // even: 8-byte aligned (h * w and w are even)
+      float2 r0 = make_float2(acc[c], 0.f), r1 = make_float2(0.f, 0.f);
+      if (addend) {
+        const float2 e0 = __ldg(reinterpret_cast<const float2*>(addend + o)), e1 = __ldg(reinterpret_cast<const float2*>(addend + o + w));
+        r0.x += e0.x; r0.y += e0.y; r1.x += e1.x; r1.y += e1.y;
+      }
+      *reinterpret_cast<float2*>(out + o) = r0;
+      *reinterpret_cast<float2*>(out + o + w) = r1;
+      continue;
+    }
     for (int dy = 0; dy < stride; ++dy) {
       const int y = py * stride + dy;
       if (y >= h) break;
@@ -501,7 +515,7 @@ conv_bwd_3x3s2_kernel(const float* __restrict__ A, long long sBr, long long sB, 
     rowp[tid] = ptr;
   }
   // both stages zeroed once: the halo column / row (and rows past the end) stay zero, the copies touch the interior only
-  for (int i = tid; i < 2 * stage_floats; i += blockDim.x) sm[i] = 0.f;
+  for (int i = tid; i < stage_floats / 2; i += blockDim.x) reinterpret_cast<float4*>(sm)[i] = make_float4(0.f, 0.f, 0.f, 0.f);   // stage_floats % 4 == 0
   int soff[2];                                      // this thread's (up to two) elements of a (row, co) tile
 #pragma unroll
   for (int k = 0; k < 2; ++k) {
@@ -515,11 +529,13 @@ conv_bwd_3x3s2_kernel(const float* __restrict__ A, long long sBr, long long sB, 
     float* Ws = sm + stage * stage_floats;
     float* As = Ws + w_floats;
     const int cc = min(COC, c_out - co0);
-    for (int idx = tid; idx < cc * 9 * cgct; idx += blockDim.x) {
-      const int c = idx % cgct, t2 = idx / cgct;
-      const int tap = t2 % 9, co = t2 / 9;
+    for (int j = tid; j < 9 * cgct; j += blockDim.x) {     // (tap, c) fixed per thread, the loop walks the output channels: no division per copy
+      const int c = j % cgct, tap = j / cgct;
       const int ci = ci_base + c;
-      if (ci < c_in) cp_async4(Ws + idx, W + ((long long)(co0 + co) * c_in + ci) * 9 + tap);
+      if (ci >= c_in) continue;
+      const float* src = W + ((long long)co0 * c_in + ci) * 9 + tap;
+      float* dst = Ws + j;
+      for (int co = 0; co < cc; ++co, src += (long long)c_in * 9, dst += 9 * cgct) cp_async4(dst, src);
     }
     for (int r_ = 0; r_ < RB; ++r_) {
       const float* base = rowp[r_];
@@ -625,29 +641,56 @@ conv_bwd_3x3s1_kernel(const float* __restrict__ A, long long sBr, long long sB, 
     rowp[tid] = ptr;
   }
   // both stages zeroed once: the halo (and rows past the end) stay zero, the copies touch the interior only
-  for (int i = tid; i < 2 * stage_floats; i += blockDim.x) sm[i] = 0.f;
+  for (int i = tid; i < stage_floats / 2; i += blockDim.x) reinterpret_cast<float4*>(sm)[i] = make_float4(0.f, 0.f, 0.f, 0.f);   // stage_floats % 4 == 0
   __syncthreads();
   const int epp = PT;                              // float4 elements of one (row, co) map: h * w / 4 = PT
+  // The fill loops carry no division: ncu's per-instruction samples had 44 % of this kernel's time in their index
+  // arithmetic (idx % epp, / epp, % cc, / cc, ... once per 16 copied bytes) against 34 % in the FFMA loop.
+  //   filters: element j of a [9][cgct] slab (tap, c) is fixed per thread; the loop walks the output channels;
+  //   A tiles: with 256 % epp == 0 (the 32x32, 16x16 and 8x8 maps) a thread's float4 position e inside a map is fixed and
+  //   its (row, co) pair advances by 256 / epp per step, carried as two counters; other map sizes take the general loop.
+  const bool fixed_e = (blockDim.x % epp) == 0;
+  const int fe = tid % epp, fpr0 = tid / epp, fstep = blockDim.x / epp;
+  const int fyy = fe / wq, fxq = fe % wq;
+  const long long fsrc_off = (long long)fyy * w + 4 * fxq;
+  const int fdst_off = (fyy + 1) * PW + 4 + 4 * fxq;
   auto fill = [&](int co0, int stage) {
     float* Ws = sm + stage * stage_floats;
     float* As = Ws + w_floats;
     const int cc = min(COC, c_out - co0);
-    for (int idx = tid; idx < cc * 9 * cgct; idx += blockDim.x) {
-      const int c = idx % cgct, t2 = idx / cgct;
-      const int tap = t2 % 9, co = t2 / 9;
+    for (int j = tid; j < 9 * cgct; j += blockDim.x) {
+      const int c = j % cgct, tap = j / cgct;
       const int ci = ci_base + c;
-      if (ci < c_in) cp_async4(Ws + idx, W + ((long long)(co0 + co) * c_in + ci) * 9 + tap);
+      if (ci >= c_in) continue;
+      const float* src = W + ((long long)co0 * c_in + ci) * 9 + tap;
+      float* dst = Ws + j;
+      for (int co = 0; co < cc; ++co, src += (long long)c_in * 9, dst += 9 * cgct) cp_async4(dst, src);
     }
-    for (int idx = tid; idx < RB * cc * epp; idx += blockDim.x) {
-      const int e = idx % epp, pr = idx / epp;
-      const int co = pr % cc, r_ = pr / cc;
-      const float* base = rowp[r_];
-      if (base == nullptr) continue;
-      const int yy = e / wq, xq = e % wq;
-      const float* src = base + ((long long)(co0 + co) * h + yy) * w + 4 * xq;
-      float* dst = As + ((long long)r_ * COC + co) * tile + (yy + 1) * PW + 4 + 4 * xq;
-      const uint32_t d = static_cast<uint32_t>(__cvta_generic_to_shared(dst));
-      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(d), "l"(src) : "memory");
+    if (fixed_e) {
+      int co = fpr0 % cc, r_ = fpr0 / cc;          // one division per fill and thread
+      for (int pr = fpr0; pr < RB * cc; pr += fstep) {
+        const float* base = rowp[r_];
+        if (base != nullptr) {
+          const float* src = base + (long long)(co0 + co) * h * w + fsrc_off;
+          float* dst = As + ((long long)r_ * COC + co) * tile + fdst_off;
+          const uint32_t d = static_cast<uint32_t>(__cvta_generic_to_shared(dst));
+          asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(d), "l"(src) : "memory");
+        }
+        co += fstep;
+        while (co >= cc) { co -= cc; ++r_; }
+      }
+    } else {
+      for (int idx = tid; idx < RB * cc * epp; idx += blockDim.x) {
+        const int e = idx % epp, pr = idx / epp;
+        const int co = pr % cc, r_ = pr / cc;
+        const float* base = rowp[r_];
+        if (base == nullptr) continue;
+        const int yy = e / wq, xq = e % wq;
+        const float* src = base + ((long long)(co0 + co) * h + yy) * w + 4 * xq;
+        float* dst = As + ((long long)r_ * COC + co) * tile + (yy + 1) * PW + 4 + 4 * xq;
+        const uint32_t d = static_cast<uint32_t>(__cvta_generic_to_shared(dst));
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(d), "l"(src) : "memory");
+      }
     }
     cp_async_commit();
   };
