@@ -250,6 +250,38 @@ def test_boundary_calls_one_by_one():
             _close(g, oub, "ub")
 
 
+@pytest.mark.parametrize("side", [12, 20])
+def test_conv_backward_on_map_sizes_off_the_fast_paths(side):
+    """ResNets on 12 x 12 and 20 x 20 images: the strip kernel's staging takes its general loop (h w / 4 = 36 / 100 does not
+    divide the block size), the 6 x 6 / 10 x 10 maps after the stride-2 block are not a multiple of 4 wide and fall back to
+    the generic tiled kernel, the 1x1 skip and the stride-2 3x3 kernels run on maps the benchmark never uses.  Parity on
+    lb / ub and on the input-layer coefficients A^0."""
+    rng = np.random.Generator(np.random.PCG64(W.SEED_BASE + 7100 + side))
+    net = W.resnet(rng, in_shape=(3, side, side), stem=8, blocks=((8, 1), (16, 2), (16, 1)), fc=24, n_classes=6)
+    B, S = 2, 5
+    x0 = rng.random((B, net.n_in)).astype(np.float32)
+    C = rng.standard_normal((B, S, net.n_out)).astype(np.float32)
+    al = [rng.random((B, S, net.nodes[i].size)).astype(np.float32) for i in net.relu_ids()]
+    wl = W.Workload(cfg=5, name=f"resnet{side}", net=net, x0=x0, eps=np.full((B,), 2.0 / 255.0, np.float32), C=C,
+                    labels=np.zeros(B, int), alpha=al, intermediate="ibp", eps_set=(2.0 / 255.0,))
+    ctx, res = _check_workload(wl, free_running=False)
+    lo, hi = wl.box()
+    ald = {i: a for i, a in zip(wl.net.relu_ids(), wl.alpha)}
+    out = ctx.crown_backward(wl.B, len(wl.net.nodes) - 1, res["pre"], Cmat=wl.C, alpha_lo=ald, alpha_up=ald,
+                             box=(lo, hi), want_A=True)
+    A, d = _np(out["A"]), _np(out["d"])
+    for p in range(wl.B):
+        forced = {i: (_np(l)[p].astype(np.float64), _np(u)[p].astype(np.float64)) for i, (l, u) in res["pre"].items()}
+        alp = {i: a[p] for i, a in ald.items()}
+        _, _, (A_lo, A_up, d_lo, d_up) = O.final_bounds(wl.net, lo[p], hi[p], wl.C[p], forced, alp, alp)
+        for br, ref in ((0, A_lo), (1, A_up)):
+            sc = np.abs(ref).max(axis=-1, keepdims=True)       # as in the tensor-core test: cancelling sums over many paths
+            err = np.abs(A[br, p] - ref) - (ATOL * sc + RTOL * np.abs(ref))
+            assert np.all(err <= 0), f"A^0 branch {br} prop {p}: worst excess {err.max():.3e}"
+        _close(d[0, p], d_lo, "d_lo")
+        _close(d[1, p], d_up, "d_up")
+
+
 def test_tensor_core_conv_backward_small_resnet():
     """A 16 x 16, 32-channel ResNet (stem + 2 residual blocks): the 3x3 stride-1 BoundConv backward steps with 32
     channels run as the per-tap implicit GEMM on tcgen05 (conv_tc.cu), one of them with the residual fork's other
