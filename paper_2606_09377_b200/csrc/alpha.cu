@@ -210,7 +210,7 @@ alpha_relu_kernel(const float* __restrict__ A, const float* __restrict__ Gin, co
                   float* alpha_lo, float* alpha_up, float* __restrict__ Gout, float* __restrict__ g_lo,
                   float* __restrict__ g_up, const float* __restrict__ step, int mode, int B, int S, int n,
                   const int8_t* __restrict__ split, float* beta_lo, float* beta_up, float* __restrict__ gb_lo,
-                  float* __restrict__ gb_up) {
+                  float* __restrict__ gb_up, const float* __restrict__ gin_bias, float* __restrict__ Gout_lo) {
   const long long per_br = (long long)B * S * n;
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= per_br) return;
@@ -218,12 +218,22 @@ alpha_relu_kernel(const float* __restrict__ A, const float* __restrict__ Gin, co
   const float4 c = __ldg(coef + (long long)b * n + j);
   const bool unstable = c.w != 0.f;
   const float aL = A[i], aU = A[per_br + i];
-  const float gL = Gin[i], gU = Gin[per_br + i];
+  // gin_bias: the bias of the Linear that produced Gin, added here instead of in a pass of its own over Gin
+  const float gb = gin_bias ? __ldg(gin_bias + j) : 0.f;
+  const float gL = Gin[i] + gb, gU = Gin[per_br + i] + gb;
   const float alL = alpha_lo[i], alU = alpha_up[i];
   const float sL = unstable ? clip01f(alL) : c.z, sU = unstable ? clip01f(alU) : c.z;
   const float dU = c.x, bU = c.y;
-  Gout[i] = aL > 0.f ? sL * gL : (aL < 0.f ? fmaf(dU, gL, bU) : 0.f);
-  Gout[per_br + i] = aU > 0.f ? fmaf(dU, gU, bU) : (aU < 0.f ? sU * gU : 0.f);
+  const float oL = aL > 0.f ? sL * gL : (aL < 0.f ? fmaf(dU, gL, bU) : 0.f);
+  const float oU = aU > 0.f ? fmaf(dU, gU, bU) : (aU < 0.f ? sU * gU : 0.f);
+  if (Gout_lo) {        // the only consumer is a tensor-core Linear: its operand limbs are written here (no split pass)
+    float h, l;
+    tf32_split(oL, h, l); Gout[i] = h; Gout_lo[i] = l;
+    tf32_split(oU, h, l); Gout[per_br + i] = h; Gout_lo[per_br + i] = l;
+  } else {
+    Gout[i] = oL;
+    Gout[per_br + i] = oU;
+  }
   const float dl = unstable ? fmaxf(aL, 0.f) * gL : 0.f;
   const float du = unstable ? fminf(aU, 0.f) * gU : 0.f;
   if (step) {
@@ -252,11 +262,12 @@ alpha_relu_kernel(const float* __restrict__ A, const float* __restrict__ Gin, co
 
 void launch_alpha_relu(const float* A, const float* Gin, const float4* coef, float* alpha_lo, float* alpha_up,
                        float* Gout, float* g_lo, float* g_up, const float* step, int mode, int B, int S, int n,
-                       cudaStream_t s, const int8_t* split, float* beta_lo, float* beta_up, float* gb_lo, float* gb_up) {
+                       cudaStream_t s, const int8_t* split, float* beta_lo, float* beta_up, float* gb_lo, float* gb_up,
+                       const float* gin_bias, float* Gout_lo) {
   const long long cnt = (long long)B * S * n;
   if (cnt <= 0) return;
   alpha_relu_kernel<<<ceil_div(cnt, 256), 256, 0, s>>>(A, Gin, coef, alpha_lo, alpha_up, Gout, g_lo, g_up, step, mode,
-                                                      B, S, n, split, beta_lo, beta_up, gb_lo, gb_up);
+                                                      B, S, n, split, beta_lo, beta_up, gb_lo, gb_up, gin_bias, Gout_lo);
 }
 
 // ---- best-so-far bounds over the iterates (every iterate is sound): lb_best = max, ub_best = min; the step size

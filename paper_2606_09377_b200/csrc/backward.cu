@@ -798,6 +798,18 @@ int alpha_forward(crown_ctx* ctx, int B, int S, const AlphaScratch& sc, const fl
   cudaStream_t s = ctx->stream;
   const long long M = 2LL * B * S;
   { Scope scp(ctx, CROWN_K_MISC, 4.0 * M * ctx->n0 * 2); launch_alpha_corner(sc.A0, x_lo, x_hi, sc.Gin, B, S, ctx->n0, s); }
+  // Two passes over G are folded into the ReLU kernel where the graph is a plain chain: the bias of a tensor-core Linear
+  // whose only consumer is a ReLU is added when that ReLU reads G (deferred_bias), and a ReLU whose only consumer is a
+  // tensor-core Linear writes that contraction's TF32 limbs itself (presplit).
+  const int nn = (int)ctx->nodes.size();
+  std::vector<const float*> deferred_bias(nn, nullptr);
+  std::vector<char> presplit(nn, 0);
+  auto sole_consumer = [&](int i) -> int {      // the one node that reads node i, or -1
+    if (ctx->nodes[i].n_consumers != 1) return -1;
+    for (int k = i + 1; k < nn; ++k)
+      if (ctx->nodes[k].n.in0 == i || (ctx->nodes[k].n.op == CROWN_ADD && ctx->nodes[k].n.in1 == i)) return k;
+    return -1;
+  };
   for (int i = 0; i <= sc.last_relu; ++i) {
     const NodeInfo& ni = ctx->nodes[i];
     const crown_node& nd = ni.n;
@@ -806,6 +818,7 @@ int alpha_forward(crown_ctx* ctx, int B, int S, const AlphaScratch& sc, const fl
       case CROWN_LINEAR: {
         if (sc.Wf_hi[i]) {
           // tensor cores (3xTF32): split G_in, contract with the limbs of W_i made by alpha_prepare, add the bias
+          if (!(nd.in0 >= 0 && presplit[nd.in0]))
           { Scope scp(ctx, CROWN_K_MISC, 12.0 * M * nd.n_in); launch_split_tf32(gin, (int)M, nd.n_in, 0, sc.Gs_hi, sc.Gs_lo, s); }
           const char* e = nullptr;
           { Scope scp(ctx, CROWN_K_GEMM_TC, 8.0 * M * nd.n_in + 8.0 * nd.n_in * nd.n_out + 4.0 * M * nd.n_out, 2.0 * M * (double)nd.n_in * nd.n_out);
@@ -813,7 +826,11 @@ int alpha_forward(crown_ctx* ctx, int B, int S, const AlphaScratch& sc, const fl
                                ctx->opts.k_drain, ctx->num_sms, s, &e))
               return fail(ctx, CROWN_ECUDA, std::string("alpha forward gemm_tc: ") + (e ? e : "?"));
             ctx->launches += gemm_tc_num_panels(nd.n_in) - 1; }
-          if (nd.b_dev) { Scope scp(ctx, CROWN_K_MISC, 8.0 * M * nd.n_out); launch_add_bias_rows(sc.G[i], nd.b_dev, M, nd.n_out, s); }
+          if (nd.b_dev) {
+            const int k = sole_consumer(i);
+            if (k >= 0 && k <= sc.last_relu && ctx->nodes[k].n.op == CROWN_RELU) deferred_bias[i] = nd.b_dev;
+            else { Scope scp(ctx, CROWN_K_MISC, 8.0 * M * nd.n_out); launch_add_bias_rows(sc.G[i], nd.b_dev, M, nd.n_out, s); }
+          }
           break;
         }
         Scope scp(ctx, CROWN_K_GEMM_FFMA, 4.0 * ((double)M * nd.n_in + (double)nd.n_in * nd.n_out + (double)M * nd.n_out),
@@ -839,12 +856,17 @@ int alpha_forward(crown_ctx* ctx, int B, int S, const AlphaScratch& sc, const fl
         break;                                  // aliases its producer
       case CROWN_RELU: {
         const bool sp = bs && bs->split && bs->split[i];
-        Scope scp(ctx, CROWN_K_RELAX, 4.0 * ni.size * (3.0 * M + 2.0 * B * S + (sp ? 2.0 * B * S : 0.0)));
-        launch_alpha_relu(sc.Asave[i], gin, coef_ptr(ctx, i), alpha_lo[i], alpha_up[i], sc.G[i],
+        const int k = sole_consumer(i);
+        // k == i + 1: nothing between the two may reuse the limb scratch
+        const bool limbs = k == i + 1 && k <= sc.last_relu && ctx->nodes[k].n.op == CROWN_LINEAR && ctx->nodes[k].n.in0 == i && sc.Wf_hi[k];
+        presplit[i] = limbs ? 1 : 0;
+        Scope scp(ctx, CROWN_K_RELAX, 4.0 * ni.size * ((limbs ? 4.0 : 3.0) * M + 2.0 * B * S + (sp ? 2.0 * B * S : 0.0)));
+        launch_alpha_relu(sc.Asave[i], gin, coef_ptr(ctx, i), alpha_lo[i], alpha_up[i], limbs ? sc.Gs_hi : sc.G[i],
                           g_lo ? g_lo[i] : nullptr, g_up ? g_up[i] : nullptr, step, mode, B, S, ni.size, s,
                           sp ? bs->split[i] : nullptr, sp && bs->beta_lo ? bs->beta_lo[i] : nullptr,
                           sp && bs->beta_up ? bs->beta_up[i] : nullptr, sp && bs->gb_lo ? bs->gb_lo[i] : nullptr,
-                          sp && bs->gb_up ? bs->gb_up[i] : nullptr);
+                          sp && bs->gb_up ? bs->gb_up[i] : nullptr, nd.in0 >= 0 ? deferred_bias[nd.in0] : nullptr,
+                          limbs ? sc.Gs_lo : nullptr);
         break; }
       default:
         return fail(ctx, CROWN_EUNSUPPORTED, "crown_alpha: unsupported op");

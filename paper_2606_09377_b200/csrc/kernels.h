@@ -160,7 +160,9 @@ void launch_add_bias_rows(float* D, const float* bias, long long M, int N, cudaS
 void launch_alpha_relu(const float* A, const float* Gin, const float4* coef, float* alpha_lo, float* alpha_up,
                        float* Gout, float* g_lo, float* g_up, const float* step, int mode, int B, int S, int n,
                        cudaStream_t s, const int8_t* split = nullptr, float* beta_lo = nullptr, float* beta_up = nullptr,
-                       float* gb_lo = nullptr, float* gb_up = nullptr);
+                       float* gb_lo = nullptr, float* gb_up = nullptr,
+                       const float* gin_bias = nullptr,   // [n]: added to Gin on the fly (the bias of the Linear that made Gin)
+                       float* Gout_lo = nullptr);         // non-null: Gout / Gout_lo receive the TF32 limbs of the output
 void launch_alpha_best(const float* lb, const float* ub, float* lb_best, float* ub_best, float* step, float decay,
                        int first, int count, cudaStream_t s);
 void launch_alpha_set_step(float* step, float v, cudaStream_t s, float v_beta = 0.f);   // step[0] = alpha step, step[1] = beta step
