@@ -31,11 +31,54 @@ alpha_corner_kernel(const float* __restrict__ A0, const float* __restrict__ x_lo
   G[i] = br == 0 ? xc - sg * xr : xc + sg * xr;
 }
 
+// the same, one block per (branch, property, spec) row and four columns per thread: no 64-bit division per element (the scalar
+// kernel above spends ~100 instructions per element on them: 287 us for the 231 MB of cfg2's 4096 sub-domains).  G_lo != nullptr:
+// G / G_lo receive the TF32 limbs of the corner (the operand of the first Linear's contraction, no split pass).
+__global__ void __launch_bounds__(256)
+alpha_corner_rows_kernel(const float* __restrict__ A0, const float* __restrict__ x_lo, const float* __restrict__ x_hi,
+                         float* __restrict__ G, float* __restrict__ G_lo, int B, int S, int n0) {
+  const long long row = blockIdx.x;                      // (br * B + b) * S + s
+  const int br = (int)(row / ((long long)B * S));
+  const int b = (int)((row / S) % B);
+  const float4* l4 = reinterpret_cast<const float4*>(x_lo + (long long)b * n0);
+  const float4* h4 = reinterpret_cast<const float4*>(x_hi + (long long)b * n0);
+  float4* g4 = reinterpret_cast<float4*>(G + row * n0);
+  float4* gl4 = G_lo ? reinterpret_cast<float4*>(G_lo + row * n0) : nullptr;
+  const float sgn = br == 0 ? -1.f : 1.f;
+  for (int j = threadIdx.x; j < (n0 >> 2); j += blockDim.x) {
+    const float4 a = ldg_stream4(A0 + row * n0 + 4 * j), lo = __ldg(l4 + j), hi = __ldg(h4 + j);
+    float4 g;
+    // x_c -/+ sign(a) x_r; sign(0) = 0: one-sided derivative 0 at the kink (reading G23)
+    g.x = fmaf(sgn * (a.x > 0.f ? 1.f : (a.x < 0.f ? -1.f : 0.f)), 0.5f * (hi.x - lo.x), 0.5f * (lo.x + hi.x));
+    g.y = fmaf(sgn * (a.y > 0.f ? 1.f : (a.y < 0.f ? -1.f : 0.f)), 0.5f * (hi.y - lo.y), 0.5f * (lo.y + hi.y));
+    g.z = fmaf(sgn * (a.z > 0.f ? 1.f : (a.z < 0.f ? -1.f : 0.f)), 0.5f * (hi.z - lo.z), 0.5f * (lo.z + hi.z));
+    g.w = fmaf(sgn * (a.w > 0.f ? 1.f : (a.w < 0.f ? -1.f : 0.f)), 0.5f * (hi.w - lo.w), 0.5f * (lo.w + hi.w));
+    if (gl4) {
+      float4 h, l;
+      tf32_split(g.x, h.x, l.x); tf32_split(g.y, h.y, l.y); tf32_split(g.z, h.z, l.z); tf32_split(g.w, h.w, l.w);
+      g4[j] = h; gl4[j] = l;
+    } else {
+      g4[j] = g;
+    }
+  }
+}
+
 void launch_alpha_corner(const float* A0, const float* x_lo, const float* x_hi, float* G, int B, int S, int n0,
-                         cudaStream_t s) {
+                         cudaStream_t s, float* G_lo) {
   const long long cnt = 2LL * B * S * n0;
   if (cnt <= 0) return;
+  auto mis = [](const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) != 0; };
+  if ((n0 & 3) == 0 && !mis(A0) && !mis(x_lo) && !mis(x_hi) && !mis(G) && !(G_lo && mis(G_lo))) {
+    alpha_corner_rows_kernel<<<(unsigned)(2LL * B * S), 256, 0, s>>>(A0, x_lo, x_hi, G, G_lo, B, S, n0);
+    return;
+  }
+  // G_lo is only offered by the caller when the vector path applies (alpha_corner_limbs_ok)
   alpha_corner_kernel<<<ceil_div(cnt, 256), 256, 0, s>>>(A0, x_lo, x_hi, G, B, S, n0);
+}
+
+bool alpha_corner_limbs_ok(const float* A0, const float* x_lo, const float* x_hi, const float* G, const float* G_lo, int n0) {
+  auto mis = [](const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) != 0; };
+  return (n0 & 3) == 0 && !mis(A0) && !mis(x_lo) && !mis(x_hi) && !mis(G) && !mis(G_lo);
 }
 
 // ---- Linear: D[M,N] = G[M,K] . W[N,K]^T + bias[N]  (W row-major [n_out, n_in] as the network stores it) ------------

@@ -797,7 +797,13 @@ int alpha_forward(crown_ctx* ctx, int B, int S, const AlphaScratch& sc, const fl
                   const float* step, int mode, const BetaSweep* bs = nullptr) {
   cudaStream_t s = ctx->stream;
   const long long M = 2LL * B * S;
-  { Scope scp(ctx, CROWN_K_MISC, 4.0 * M * ctx->n0 * 2); launch_alpha_corner(sc.A0, x_lo, x_hi, sc.Gin, B, S, ctx->n0, s); }
+  // the corner of the box per row; when the input feeds exactly one tensor-core Linear (node 0), its limbs are written
+  // straight into that contraction's operand scratch
+  const bool corner_limbs = ctx->input_consumers == 1 && sc.last_relu >= 0 && ctx->nodes[0].n.op == CROWN_LINEAR &&
+                            ctx->nodes[0].n.in0 < 0 && sc.Wf_hi[0] && sc.Gs_hi &&
+                            alpha_corner_limbs_ok(sc.A0, x_lo, x_hi, sc.Gs_hi, sc.Gs_lo, ctx->n0);
+  { Scope scp(ctx, CROWN_K_MISC, 4.0 * M * ctx->n0 * (corner_limbs ? 3 : 2));
+    launch_alpha_corner(sc.A0, x_lo, x_hi, corner_limbs ? sc.Gs_hi : sc.Gin, B, S, ctx->n0, s, corner_limbs ? sc.Gs_lo : nullptr); }
   // Two passes over G are folded into the ReLU kernel where the graph is a plain chain: the bias of a tensor-core Linear
   // whose only consumer is a ReLU is added when that ReLU reads G (deferred_bias), and a ReLU whose only consumer is a
   // tensor-core Linear writes that contraction's TF32 limbs itself (presplit).
@@ -818,7 +824,7 @@ int alpha_forward(crown_ctx* ctx, int B, int S, const AlphaScratch& sc, const fl
       case CROWN_LINEAR: {
         if (sc.Wf_hi[i]) {
           // tensor cores (3xTF32): split G_in, contract with the limbs of W_i made by alpha_prepare, add the bias
-          if (!(nd.in0 >= 0 && presplit[nd.in0]))
+          if (!(nd.in0 >= 0 ? presplit[nd.in0] != 0 : (corner_limbs && i == 0)))
           { Scope scp(ctx, CROWN_K_MISC, 12.0 * M * nd.n_in); launch_split_tf32(gin, (int)M, nd.n_in, 0, sc.Gs_hi, sc.Gs_lo, s); }
           const char* e = nullptr;
           { Scope scp(ctx, CROWN_K_GEMM_TC, 8.0 * M * nd.n_in + 8.0 * nd.n_in * nd.n_out + 4.0 * M * nd.n_out, 2.0 * M * (double)nd.n_in * nd.n_out);

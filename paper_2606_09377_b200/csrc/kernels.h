@@ -140,7 +140,8 @@ int launch_conv_transpose_tc(const AView& A, const float* W, const float* addend
 
 // NEXT-1 -- alpha optimisation: kernels of the forward sweep G = d bound / d A (alpha.cu).
 void launch_alpha_corner(const float* A0, const float* x_lo, const float* x_hi, float* G, int B, int S, int n0,
-                         cudaStream_t s);
+                         cudaStream_t s, float* G_lo = nullptr);   // G_lo: write TF32 limbs (only when alpha_corner_limbs_ok)
+bool alpha_corner_limbs_ok(const float* A0, const float* x_lo, const float* x_hi, const float* G, const float* G_lo, int n0);
 void launch_alpha_linear(const float* G, const float* W, const float* bias, float* D, int M, int N, int K,
                          cudaStream_t s);
 void launch_alpha_conv(const float* W, const float* bias, const float* in, float* out, long long M, int c_in, int h,
