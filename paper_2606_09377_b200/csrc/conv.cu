@@ -486,7 +486,9 @@ conv_bwd_1x1_kernel(const float* __restrict__ A, long long sBr, long long sB, lo
 // with warp-sized classes the block waited for its 4-tap warps (profiles/r2_conv.md: 8 and 12.6 TFLOP/s).
 // Block = RB rows x CG channel groups x (ho * wo) pixel threads; A_out tiles (zero halo right / below) and the filter slice
 // [co][tap][ci] are staged COC output channels at a time.
-template <int CT>
+// P = 2: a thread owns TWO horizontally adjacent positions (p, q), (p, q + 1) of A_out, i.e. a 2 x 4 block of input pixels: every
+// filter tap loaded from shared memory feeds two FFMAs instead of one (P = 1 runs 36 broadcast LDS.128 per 144 FFMAs, 40 % FMA pipe).
+template <int CT, int P>
 __global__ void __launch_bounds__(256, 2)
 conv_bwd_3x3s2_kernel(const float* __restrict__ A, long long sBr, long long sB, long long ld, int B, int R,
                       const float* __restrict__ W, const float* __restrict__ addend, float* __restrict__ out,
@@ -494,7 +496,8 @@ conv_bwd_3x3s2_kernel(const float* __restrict__ A, long long sBr, long long sB, 
   extern __shared__ __align__(16) float sm[];
   __shared__ const float* rowp[4];
   const int cgct = CG * CT;
-  const int PT = ho * wo, PW = wo + 1, tile = (ho + 1) * PW;
+  const int wq = wo / P;                           // thread columns per row of A_out (wo % P == 0)
+  const int PT = ho * wq, PW = wo + 1, tile = (ho + 1) * PW;
   const int w_floats = COC * 9 * cgct;             // stage layout: Ws [COC][9][cgct], then As [RB][COC][tile]
   const int tid = threadIdx.x;
   const int pt = tid % PT, cg = (tid / PT) % CG, rb = tid / (PT * CG);
@@ -502,7 +505,7 @@ conv_bwd_3x3s2_kernel(const float* __restrict__ A, long long sBr, long long sB, 
   const long long rows = 2LL * B * R;
   const long long m_base = (long long)blockIdx.x * RB;
   const int ci_base = blockIdx.y * cgct;
-  const int p = pt / wo, q = pt % wo;
+  const int p = pt / wq, q = (pt % wq) * P;
   const int a_off = p * PW + q;
   if (tid < RB) {
     const long long m = m_base + tid;
@@ -540,9 +543,9 @@ conv_bwd_3x3s2_kernel(const float* __restrict__ A, long long sBr, long long sB, 
     for (int r_ = 0; r_ < RB; ++r_) {
       const float* base = rowp[r_];
       if (base == nullptr) continue;
-      base += (long long)co0 * PT;
+      base += (long long)co0 * (ho * wo);
       float* dst = As + r_ * COC * tile;
-      for (int co = 0; co < cc; ++co, base += PT, dst += tile) {
+      for (int co = 0; co < cc; ++co, base += ho * wo, dst += tile) {
 #pragma unroll
         for (int k = 0; k < 2; ++k)
           if (soff[k] >= 0) cp_async4(dst + tid + k * (int)blockDim.x, base + soff[k]);
@@ -550,9 +553,9 @@ conv_bwd_3x3s2_kernel(const float* __restrict__ A, long long sBr, long long sB, 
     }
     cp_async_commit();
   };
-  float acc[4][CT];
+  float acc[4 * P][CT];
 #pragma unroll
-  for (int k = 0; k < 4; ++k)
+  for (int k = 0; k < 4 * P; ++k)
 #pragma unroll
     for (int c = 0; c < CT; ++c) acc[k][c] = 0.f;
   const int nchunks = (c_out + COC - 1) / COC;
@@ -568,18 +571,24 @@ conv_bwd_3x3s2_kernel(const float* __restrict__ A, long long sBr, long long sB, 
       const float* ap = Ws + w_floats + rb * COC * tile + a_off;
       const float* wp = Ws + cg * CT;
       for (int co = 0; co < cc; ++co, ap += tile, wp += 9 * cgct) {
-        const float a00 = ap[0], a01 = ap[1], a10 = ap[PW], a11 = ap[PW + 1];
+        float a0[P + 1], a1[P + 1];                 // A_out rows p and p + 1, columns q .. q + P
+#pragma unroll
+        for (int u = 0; u <= P; ++u) { a0[u] = ap[u]; a1[u] = ap[PW + u]; }
 #pragma unroll
         for (int c4 = 0; c4 < CT; c4 += 4) {
           float4 w[9];
 #pragma unroll
           for (int t = 0; t < 9; ++t) w[t] = *reinterpret_cast<const float4*>(wp + t * cgct + c4);
 #define CROWN_S2_STEP(C_, F_) \
-          acc[0][c4 + C_] = fmaf(w[4].F_, a00, acc[0][c4 + C_]); \
-          acc[1][c4 + C_] = fmaf(w[3].F_, a01, fmaf(w[5].F_, a00, acc[1][c4 + C_])); \
-          acc[2][c4 + C_] = fmaf(w[1].F_, a10, fmaf(w[7].F_, a00, acc[2][c4 + C_])); \
-          acc[3][c4 + C_] = fmaf(w[0].F_, a11, fmaf(w[2].F_, a10, fmaf(w[6].F_, a01, fmaf(w[8].F_, a00, acc[3][c4 + C_]))));
-          CROWN_S2_STEP(0, x) CROWN_S2_STEP(1, y) CROWN_S2_STEP(2, z) CROWN_S2_STEP(3, w)
+          acc[4 * u + 0][c4 + C_] = fmaf(w[4].F_, a00, acc[4 * u + 0][c4 + C_]); \
+          acc[4 * u + 1][c4 + C_] = fmaf(w[3].F_, a01, fmaf(w[5].F_, a00, acc[4 * u + 1][c4 + C_])); \
+          acc[4 * u + 2][c4 + C_] = fmaf(w[1].F_, a10, fmaf(w[7].F_, a00, acc[4 * u + 2][c4 + C_])); \
+          acc[4 * u + 3][c4 + C_] = fmaf(w[0].F_, a11, fmaf(w[2].F_, a10, fmaf(w[6].F_, a01, fmaf(w[8].F_, a00, acc[4 * u + 3][c4 + C_]))));
+#pragma unroll
+          for (int u = 0; u < P; ++u) {
+            const float a00 = a0[u], a01 = a0[u + 1], a10 = a1[u], a11 = a1[u + 1];
+            CROWN_S2_STEP(0, x) CROWN_S2_STEP(1, y) CROWN_S2_STEP(2, z) CROWN_S2_STEP(3, w)
+          }
 #undef CROWN_S2_STEP
         }
       }
@@ -589,10 +598,34 @@ conv_bwd_3x3s2_kernel(const float* __restrict__ A, long long sBr, long long sB, 
   const long long m = m_base + rb;
   if (!active || m >= rows) return;
   const int h = 2 * ho, w_ = 2 * wo;
+  const long long plane = (long long)h * w_;
+  const long long o0 = ((m * c_in + ci_base + cg * CT) * h + 2 * p) * (long long)w_ + 2 * q;     // even: 8-byte aligned (P = 2: 16)
+  if (P == 2) {
+    // a position pair is four adjacent input columns: one 16-byte store per input row; four channels' addends at a time
+#pragma unroll
+    for (int c0 = 0; c0 < CT; c0 += 4) {
+      float4 e0[4], e1[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        e0[k] = make_float4(0.f, 0.f, 0.f, 0.f); e1[k] = e0[k];
+        if (addend && ci_base + cg * CT + c0 + k < c_in) {
+          const long long o = o0 + (c0 + k) * plane;
+          e0[k] = __ldg(reinterpret_cast<const float4*>(addend + o)); e1[k] = __ldg(reinterpret_cast<const float4*>(addend + o + w_));
+        }
+      }
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const int c = c0 + k;
+        if (ci_base + cg * CT + c >= c_in) continue;
+        const long long o = o0 + c * plane;
+        *reinterpret_cast<float4*>(out + o) = make_float4(acc[0][c] + e0[k].x, acc[1][c] + e0[k].y, acc[4 * (P - 1)][c] + e0[k].z, acc[4 * (P - 1) + 1][c] + e0[k].w);
+        *reinterpret_cast<float4*>(out + o + w_) = make_float4(acc[2][c] + e1[k].x, acc[3][c] + e1[k].y, acc[4 * (P - 1) + 2][c] + e1[k].z, acc[4 * (P - 1) + 3][c] + e1[k].w);
+      }
+    }
+    return;
+  }
   // eight channels at a time: their sixteen addend loads are issued together, then added and stored (one channel at a time
   // every add waited for its own load: 23 - 45 % of this kernel's samples sat on those FADDs)
-  const long long plane = (long long)h * w_;
-  const long long o0 = ((m * c_in + ci_base + cg * CT) * h + 2 * p) * (long long)w_ + 2 * q;     // even: 8-byte aligned
 #pragma unroll
   for (int c0 = 0; c0 < CT; c0 += 8) {
     float2 e0[8], e1[8];
@@ -840,8 +873,12 @@ static bool launch_conv_bwd_3x3s2(const AView& A, const float* W, const float* a
                                   int c_in, int h, int w, int c_out, int pad, int ho, int wo, cudaStream_t s) {
   if (!conv_s2_supported(c_in, h, w, c_out, 3, 3, 2, pad, ho, wo)) return false;
   if ((reinterpret_cast<uintptr_t>(out) & 7) || (addend && (reinterpret_cast<uintptr_t>(addend) & 7))) return false;
-  const int CT = (c_in % 16 == 0) ? 16 : 8;
-  const int PT = ho * wo;
+  // two positions per thread (P = 2) with 8 channels where the map is even-wide and the 16-byte stores are aligned; else one
+  // position with 8 / 16 channels
+  const bool p2 = (wo % 2 == 0) && ho * (wo / 2) >= 8 && !(reinterpret_cast<uintptr_t>(out) & 15) &&
+                  !(addend && (reinterpret_cast<uintptr_t>(addend) & 15));
+  const int CT = p2 ? 8 : ((c_in % 16 == 0) ? 16 : 8);
+  const int PT = p2 ? ho * (wo / 2) : ho * wo;
   const int groups = (c_in + CT - 1) / CT;
   int CG = 256 / PT < groups ? 256 / PT : groups;
   if (CG < 1) CG = 1;
@@ -859,8 +896,9 @@ static bool launch_conv_bwd_3x3s2(const AView& A, const float* W, const float* a
   const long long rows = 2LL * B * R;
   const int threads = 256;                          // the element -> thread map of the staging assumes blockDim = 256
   dim3 grid((unsigned)((rows + RB - 1) / RB), (unsigned)((groups + CG - 1) / CG));
-  if (CT == 16) conv_bwd_3x3s2_kernel<16><<<grid, threads, smem, s>>>(A.p, A.sBr, A.sB, A.ld, B, R, W, addend, out, c_in, c_out, ho, wo, COC, CG, RB, stage_floats);
-  else conv_bwd_3x3s2_kernel<8><<<grid, threads, smem, s>>>(A.p, A.sBr, A.sB, A.ld, B, R, W, addend, out, c_in, c_out, ho, wo, COC, CG, RB, stage_floats);
+  if (p2) conv_bwd_3x3s2_kernel<8, 2><<<grid, threads, smem, s>>>(A.p, A.sBr, A.sB, A.ld, B, R, W, addend, out, c_in, c_out, ho, wo, COC, CG, RB, stage_floats);
+  else if (CT == 16) conv_bwd_3x3s2_kernel<16, 1><<<grid, threads, smem, s>>>(A.p, A.sBr, A.sB, A.ld, B, R, W, addend, out, c_in, c_out, ho, wo, COC, CG, RB, stage_floats);
+  else conv_bwd_3x3s2_kernel<8, 1><<<grid, threads, smem, s>>>(A.p, A.sBr, A.sB, A.ld, B, R, W, addend, out, c_in, c_out, ho, wo, COC, CG, RB, stage_floats);
   return true;
 }
 
@@ -923,8 +961,9 @@ int conv_init_device() {
   if (cudaFuncSetAttribute(conv_bwd_3x3s1_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1) != cudaSuccess ||
       cudaFuncSetAttribute(conv_bwd_3x3s1_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1) != cudaSuccess ||
       cudaFuncSetAttribute(conv_bwd_3x3s1_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1) != cudaSuccess) return -1;
-  if (cudaFuncSetAttribute(conv_bwd_3x3s2_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1) != cudaSuccess ||
-      cudaFuncSetAttribute(conv_bwd_3x3s2_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1) != cudaSuccess) return -1;
+  if (cudaFuncSetAttribute(conv_bwd_3x3s2_kernel<16, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1) != cudaSuccess ||
+      cudaFuncSetAttribute(conv_bwd_3x3s2_kernel<8, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1) != cudaSuccess ||
+      cudaFuncSetAttribute(conv_bwd_3x3s2_kernel<8, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1) != cudaSuccess) return -1;
   if (cudaFuncSetAttribute(conv_bwd_1x1_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1) != cudaSuccess ||
       cudaFuncSetAttribute(conv_bwd_1x1_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1) != cudaSuccess ||
       cudaFuncSetAttribute(conv_bwd_1x1_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, b1) != cudaSuccess) return -1;
