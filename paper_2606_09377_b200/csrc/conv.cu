@@ -15,11 +15,14 @@ namespace crownb200 {
 // are 8..32 wide with 3..64 channels and B = 8 images: the kernel is latency-bound, parallelism is what it lacks);
 // the CS partial sums are added in slice order through shared memory (deterministic).
 constexpr int kIbpConvCO = 4;
+// KS > 0: square KS x KS filter known at compile time (the tap loops unroll, same order of operations); KS = 0: any kh x kw
+template <int KS>
 __global__ void __launch_bounds__(512)
 ibp_conv_kernel(const float* __restrict__ W, const float* __restrict__ bias, const float* __restrict__ l_in,
                 const float* __restrict__ u_in, int relu_in, float* __restrict__ l_out,
-                float* __restrict__ u_out, int c_in, int h, int w, int c_out, int kh, int kw, int stride,
+                float* __restrict__ u_out, int c_in, int h, int w, int c_out, int kh_, int kw_, int stride,
                 int pad, int ho, int wo) {
+  const int kh = KS > 0 ? KS : kh_, kw = KS > 0 ? KS : kw_;
   extern __shared__ float sw[];   // [kIbpConvCO][c_in*kh*kw] filters, then [CS][PIX][2*kIbpConvCO] partial sums
   const int co0 = blockIdx.y * kIbpConvCO, b = blockIdx.z;
   const int fsz = c_in * kh * kw;
@@ -41,9 +44,11 @@ ibp_conv_kernel(const float* __restrict__ W, const float* __restrict__ bias, con
   for (int o = 0; o < kIbpConvCO; ++o) { c[o] = 0.f; r[o] = 0.f; }
   if (live)
     for (int ci = threadIdx.y; ci < c_in; ci += CS)
+#pragma unroll
       for (int i = 0; i < kh; ++i) {
         const int y = p * stride + i - pad;
         if (y < 0 || y >= h) continue;
+#pragma unroll
         for (int j = 0; j < kw; ++j) {
           const int x = q * stride + j - pad;
           if (x < 0 || x >= w) continue;
@@ -93,8 +98,12 @@ void launch_ibp_conv(const float* W, const float* bias, const float* l_in, const
   while (cs < 8 && cs * 2 <= c_in && pix * cs * 2 <= 512) cs *= 2;
   dim3 grid(ceil_div(ho * wo, pix), ceil_div(c_out, kIbpConvCO), B), block(pix, cs);
   size_t smem = ((size_t)kIbpConvCO * c_in * kh * kw + (cs > 1 ? (size_t)cs * pix * 2 * kIbpConvCO : 0)) * sizeof(float);
-  ibp_conv_kernel<<<grid, block, smem, s>>>(W, bias, l_in, u_in, relu_in, l_out, u_out, c_in, h, w, c_out,
-                                            kh, kw, stride, pad, ho, wo);
+  if (kh == 3 && kw == 3)
+    ibp_conv_kernel<3><<<grid, block, smem, s>>>(W, bias, l_in, u_in, relu_in, l_out, u_out, c_in, h, w, c_out, kh, kw, stride, pad, ho, wo);
+  else if (kh == 1 && kw == 1)
+    ibp_conv_kernel<1><<<grid, block, smem, s>>>(W, bias, l_in, u_in, relu_in, l_out, u_out, c_in, h, w, c_out, kh, kw, stride, pad, ho, wo);
+  else
+    ibp_conv_kernel<0><<<grid, block, smem, s>>>(W, bias, l_in, u_in, relu_in, l_out, u_out, c_in, h, w, c_out, kh, kw, stride, pad, ho, wo);
 }
 
 // ---- a6: A_in = conv^T(A_out, W) (+ addend: the other incoming A of a residual fork).
